@@ -1,0 +1,194 @@
+"""Seeded synthetic filterbank workloads (the five BASELINE.json configs).
+
+This module serves BOTH the oracle-side tests and the CUDA-side tests/bench, so
+it holds none of the method's arithmetic: no delay formula, no dedispersion
+sum.  Anything that depends on the delay table (``max_delay`` for the row
+length, the sweep of an injected pulse) is passed in by the caller, who gets it
+from whichever implementation it is exercising.
+
+The inputs stand in for HTRU survey recordings (Sec. 1: 1024
+channels over 400 MHz centred at 1381.8 MHz, 64 us, 2 bits per sample), which
+are not available here.  Recipes follow SURVEY.md Sec. 8(d); DESIGN.md restates
+them.  NumPy only (no torch, no CUDA).
+"""
+from __future__ import annotations
+
+import hashlib
+import math
+from dataclasses import dataclass, replace
+from typing import Callable
+
+import numpy as np
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    nchans: int
+    f_top: float          # MHz, frequency of channel 0
+    df: float             # MHz, channel spacing (negative)
+    dt: float             # s
+    nbits: int            # 2 or 8
+    ndm: int
+    dm_lo: float
+    dm_hi: float
+    nsamps_out: int
+    out_dtype: str        # "u32" | "f32"
+    nbeams: int
+    seed: int
+    kind: str             # "uniform2" | "gauss2" | "gauss2_pulses" | "gauss8"
+    npulses: int = 0
+
+    def dms(self) -> np.ndarray:
+        """Trial DM list: inclusive linear spacing (numpy.linspace), float64."""
+        return np.linspace(self.dm_lo, self.dm_hi, self.ndm, dtype=np.float64)
+
+    def obs_seconds(self) -> float:
+        return self.nsamps_out * self.dt
+
+    def dm_trial_samples(self) -> int:
+        return self.nbeams * self.ndm * self.nsamps_out
+
+    def adds(self) -> int:
+        return self.dm_trial_samples() * self.nchans
+
+    def scaled(self, **kw) -> "Workload":
+        return replace(self, **kw)
+
+
+CONFIGS: dict[str, Workload] = {
+    "tiny": Workload("tiny", 64, 1581.8, -6.25, 64e-6, 2, 32, 0.0, 200.0, 4096, "u32", 1, 1001,
+                     "uniform2"),
+    "htru_gulp": Workload("htru_gulp", 1024, 1581.8, -0.390625, 64e-6, 2, 1200, 0.0, 1000.0, 65536,
+                          "u32", 1, 1002, "gauss2"),
+    "htru_long_pulses": Workload("htru_long_pulses", 1024, 1581.8, -0.390625, 64e-6, 2, 1200, 0.0,
+                                 1000.0, 524288, "f32", 1, 1003, "gauss2_pulses", npulses=16),
+    "wide8": Workload("wide8", 4096, 1500.0, -0.09765625, 64e-6, 8, 2048, 0.0, 2000.0, 131072,
+                      "u32", 1, 1004, "gauss8"),
+    "beams13": Workload("beams13", 1024, 1581.8, -0.390625, 64e-6, 2, 1200, 0.0, 1000.0, 65536,
+                        "u32", 13, 1100, "gauss2"),
+}
+CONFIG_ORDER = ["tiny", "htru_gulp", "htru_long_pulses", "wide8", "beams13"]
+
+
+def _phi(x: float) -> float:
+    """Standard normal CDF."""
+    return 0.5 * (1.0 + math.erf(x / math.sqrt(2.0)))
+
+
+# Quantiser thresholds at -1, 0, +1 sigma expressed on the uniform variate.
+_THR = np.array([_phi(-1.0), 0.5, _phi(1.0)], dtype=np.float64)
+
+
+def row_stride_bytes(nsamps_in: int, nbits: int) -> int:
+    """Tight packed row length in bytes."""
+    return (nsamps_in * nbits + 7) // 8
+
+
+def pack2(levels: np.ndarray) -> np.ndarray:
+    """Pack 2-bit levels (values 0..3, 1-D) LSB-first, 4 per byte, zero padded."""
+    n = levels.shape[0]
+    nb = (n + 3) // 4
+    buf = np.zeros(nb * 4, dtype=np.uint8)
+    buf[:n] = levels
+    q = buf.reshape(nb, 4)
+    return (q[:, 0] | (q[:, 1] << 2) | (q[:, 2] << 4) | (q[:, 3] << 6)).astype(np.uint8)
+
+
+def unpack2(row: np.ndarray, nsamps: int) -> np.ndarray:
+    """Inverse of :func:`pack2` (test helper; a layout statement, not the method)."""
+    sh = np.arange(4, dtype=np.uint8) * 2
+    return ((row[:, None] >> sh[None, :]) & 3).reshape(-1)[:nsamps].astype(np.uint8)
+
+
+def _rng(seed: int, stream: int) -> np.random.Generator:
+    return np.random.Generator(np.random.Philox(key=np.array([seed, stream], dtype=np.uint64)))
+
+
+@dataclass(frozen=True)
+class Pulses:
+    dm: np.ndarray        # float64 [npulses]
+    width: np.ndarray     # int64   [npulses]
+    t0: np.ndarray        # int64   [npulses]
+
+
+def pulse_params(w: Workload) -> Pulses:
+    """Seeded pulse list for the injected-pulse config: DM uniform 50..900, width
+    1..64 samples, start uniform over the output span.  Stream key (seed, 1<<48)
+    is used by no data row."""
+    u = _rng(w.seed, 1 << 48).random((w.npulses, 3))
+    dm = 50.0 + 850.0 * u[:, 0]
+    width = 1 + np.floor(64.0 * u[:, 1]).astype(np.int64)
+    t0 = np.floor(u[:, 2] * (w.nsamps_out - width)).astype(np.int64)
+    return Pulses(dm, width, t0)
+
+
+def generate(w: Workload, max_delay: int, beam: int = 0,
+             pulse_sweep: np.ndarray | None = None, pulses: Pulses | None = None) -> np.ndarray:
+    """Packed input of one beam: uint8 [nchans, row_stride], channel-major, tight rows.
+
+    ``max_delay`` comes from the caller's delay table (nsamps_in = nsamps_out +
+    max_delay).  For ``gauss2_pulses``, ``pulse_sweep[c][p]`` is the delay in
+    samples of pulse p at channel c (same source) and ``pulses`` the output of
+    :func:`pulse_params`.
+    """
+    nsamps_in = w.nsamps_out + int(max_delay)
+    stride = row_stride_bytes(nsamps_in, w.nbits)
+    out = np.zeros((w.nchans, stride), dtype=np.uint8)
+    seed = w.seed + beam if w.nbeams > 1 else w.seed
+    if w.kind == "gauss2_pulses":
+        if pulse_sweep is None or pulses is None:
+            raise ValueError("gauss2_pulses needs pulse_sweep and pulses")
+        kmax = w.npulses
+        thr_k = np.array([[_phi(j - k) for j in (-1.0, 0.0, 1.0)] for k in range(kmax + 1)])
+    for c in range(w.nchans):
+        g = _rng(seed, (beam << 32) | c)
+        if w.kind == "uniform2":
+            u = g.random(nsamps_in)
+            lev = (u * 4).astype(np.uint8)
+            out[c] = pack2(lev)
+        elif w.kind in ("gauss2", "gauss2_pulses"):
+            u = g.random(nsamps_in)
+            lev = np.searchsorted(_THR, u, side="right").astype(np.uint8)
+            if w.kind == "gauss2_pulses":
+                # k[t] = number of pulse sweeps covering sample t of this channel;
+                # a +1 sigma shift per pulse before quantisation == thresholds Phi(j-k).
+                diff = np.zeros(nsamps_in + 1, dtype=np.int32)
+                for p in range(w.npulses):
+                    a = int(pulses.t0[p]) + int(pulse_sweep[c, p])
+                    b = a + int(pulses.width[p])
+                    a, b = min(a, nsamps_in), min(b, nsamps_in)
+                    diff[a] += 1
+                    diff[b] -= 1
+                k = np.cumsum(diff[:-1])
+                idx = np.nonzero(k)[0]
+                if idx.size:
+                    t = thr_k[k[idx]]
+                    uu = u[idx]
+                    lev[idx] = ((uu >= t[:, 0]).astype(np.uint8) + (uu >= t[:, 1])
+                                + (uu >= t[:, 2])).astype(np.uint8)
+            out[c] = pack2(lev)
+        elif w.kind == "gauss8":
+            gs = g.standard_normal(nsamps_in)
+            out[c] = np.clip(np.floor(128.0 + 16.0 * gs + 0.5), 0, 255).astype(np.uint8)
+        else:
+            raise ValueError(w.kind)
+    return out
+
+
+def generate_all_beams(w: Workload, max_delay: int, **kw) -> np.ndarray:
+    """uint8 [nbeams, nchans, row_stride] -- beams contiguous."""
+    return np.stack([generate(w, max_delay, beam=b, **kw) for b in range(w.nbeams)])
+
+
+def random_small(seed: int, nchans: int, nsamps_in: int, nbits: int) -> np.ndarray:
+    """Uniform random packed rows for the random-shape parity cases."""
+    g = _rng(seed, 7)
+    if nbits == 8:
+        return g.integers(0, 256, size=(nchans, nsamps_in), dtype=np.uint8)
+    lev = (g.random((nchans, nsamps_in)) * 4).astype(np.uint8)
+    return np.stack([pack2(lev[c]) for c in range(nchans)])
+
+
+def sha256(a: np.ndarray) -> str:
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
