@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- DM-trial-samples/s of direct incoherent dedispersion on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config htru_gulp] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (delay table already built in
+set_dm_list; unpack/bit-plane pre-pass + gather-sum + output write) over one
+synthetic HTRU-shaped gulp already resident in HBM.  Prints ONE JSON line.
+N > 1 (torchrun): every rank dedisperses its own independently seeded beam
+(replicas, no data-path collective) -- "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+from paper_1112_0065_b200 import workloads as W  # noqa: E402
+
+SM_COUNT_NOMINAL = 148
+ADDS_PER_CLK_PER_SM = 128          # FP32/INT32 lane-adds per clock per SM
+PAPER_CONTEXT = [
+    "paper context (PAPER.md:22): whole CPU pipeline > 30 min per 10-min observation (unnamed CPU cluster)",
+    "paper context (PAPER.md:48): dedispersion ~20 min (unnamed CPU) -> 2.5 min (unnamed 2011 CUDA GPU) "
+    "per 10-min observation = 7.5e7 DM-trial-samples/s, RTF 4.0",
+]
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    return json.loads(p.read_text()) if p.exists() else {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [s.strip() for s in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # samples under load = upper half (idle samples before/after the kernels drag the median)
+        hi = sorted(sm)[len(sm) // 2:]
+        return {"sm_mhz": statistics.median(hi), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_setup(ngpus: int):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    return rank, world, local
+
+
+def cpu_baseline(w: W.Workload, seconds_hint: str = "") -> dict:
+    """The oracle as it stands, on this box's host cores, on a bounded sample."""
+    import oracle
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w.scaled(nbeams=1), md)
+    stride = max(1, w.ndm // 240)
+    sub = np.ascontiguousarray(delay[:, ::stride])
+    t0 = time.perf_counter()
+    _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)
+    dt = time.perf_counter() - t0
+    units = sub.shape[1] * w.nsamps_out
+    return {"value": units / dt, "unit": "DM-trial-samples/s", "cores": used, "kind": "oracle",
+            "sample": f"{sub.shape[1]} of {w.ndm} DM trials (every {stride}th) x {w.nsamps_out} samples "
+                      f"x {w.nchans} channels of {w.name}, one pass, {dt:.2f} s",
+            "rtf": (w.nsamps_out * w.dt) / (dt * w.ndm / sub.shape[1])}
+
+
+def ncu_traffic_bytes(config: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (or None)."""
+    p = ROOT / "profiles" / "traffic.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text()).get(config)
+        except (ValueError, OSError):
+            return None
+    return None
+
+
+def run_ours(args) -> None:
+    import torch
+    import paper_1112_0065_b200 as dd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    rank, world, local = dist_setup(args.gpus)
+    w = W.CONFIGS[args.config]
+    dev = torch.device("cuda", torch.cuda.current_device())
+    props = torch.cuda.get_device_properties(dev)
+    stream = torch.cuda.current_stream()
+
+    plan = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+    t0 = time.perf_counter()
+    dd.dedisp_set_dm_list(plan, list(w.dms()))
+    set_dm_ms = (time.perf_counter() - t0) * 1e3
+    md = dd.dedisp_get_max_delay(plan)
+    kw = {}
+    if w.kind == "gauss2_pulses":   # pulse sweeps from the product's own delay builder
+        pp = W.pulse_params(w)
+        p2 = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+        dd.dedisp_set_dm_list(p2, list(pp.dm))
+        kw = dict(pulse_sweep=dd.dedisp_get_delay_table(p2), pulses=pp)
+        dd.dedisp_destroy(p2)
+    # each rank gets its own seeded beam(s): beam index offset by rank
+    beams = [W.generate(w, md, beam=b + rank * w.nbeams, **kw) for b in range(w.nbeams)]
+    host_in = torch.from_numpy(np.stack(beams)).pin_memory()
+    nb, nch, stride = host_in.shape
+    assert stride == dd.dedisp_get_in_row_stride_bytes(plan, w.nsamps_out, w.nbits)
+    x = host_in.to(dev)
+    f32 = w.out_dtype == "f32"
+    code = dd.DEDISP_OUT_F32 if f32 else dd.DEDISP_OUT_U32
+    out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=torch.float32 if f32 else torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    in_bs, out_bs = nch * stride, w.ndm * w.nsamps_out * 4
+
+    def step():
+        dd.dedisp_execute_batch(plan, nb, w.nsamps_out, x, in_bs, w.nbits, out, out_bs, code,
+                                stream.cuda_stream)
+
+    dd.dedisp_set_timing(plan, True)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = dd.dedisp_get_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    main_ms, pre_ms = [], []
+    torch.cuda.synchronize()
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()                 # L2 flush between timed iterations (outside the events)
+        a.record(stream)
+        step()
+        b.record(stream)
+        pm, mm = dd.dedisp_get_last_kernel_ms(plan)   # waits for this step's kernels
+        pre_ms.append(pm)
+        main_ms.append(mm)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    launches = dd.dedisp_get_launch_count() - launches0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.barrier()
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_ms = float(total_ms.item())
+    ms_per_step = total_ms / args.steps
+    units_step = w.dm_trial_samples() * world
+    value = units_step / (ms_per_step * 1e-3)
+
+    # ---- end to end through the public host-buffer call (H2D + kernels + D2H inside the timing)
+    host_out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=out.dtype).pin_memory()
+    dd.dedisp_set_timing(plan, False)
+    e2e_steps = max(2, min(args.steps, 5))
+    dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+    e2e_s = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = units_step / float(e2e_s.item())
+    same = bool(torch.equal(host_out.to(dev), out))
+    kernel_used = dd.dedisp_get_last_kernel(plan)
+    dd.dedisp_destroy(plan)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks = measured_peaks()
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak = props.multi_processor_count * ADDS_PER_CLK_PER_SM * sm_max_mhz * 1e6   # adds/s
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0)) * 1e9
+    adds = w.adds()
+    in_bytes, out_bytes = nb * in_bs, nb * out_bs
+    t_alu, t_hbm = adds / alu_peak, (in_bytes + out_bytes) / hbm_peak
+    mm = statistics.mean(main_ms) * 1e-3
+    achieved = adds / mm
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
+                "frac": achieved / alu_peak, "traffic": ncu_traffic_bytes(args.config),
+                "kernel": "bitslice_dedisperse" if kernel_used == 2 else "direct_kernel",
+                "kernel_ms": mm * 1e3, "prepass_ms": statistics.mean(pre_ms),
+                "kernel_share_of_step": mm * 1e3 / ms_per_step,
+                "peak_source": f"{props.multi_processor_count} SMs x {ADDS_PER_CLK_PER_SM} adds/clk x "
+                               f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz); see DESIGN.md",
+                "hbm_frac": ((in_bytes + out_bytes) / mm) / hbm_peak,
+                "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
+    try:
+        probe = {n: dd.dedisp_probe_alu_rate(i) / 1e12 for i, n in
+                 enumerate(["iadd3", "lop3", "shf", "fadd", "imad", "lop3+imad"])}
+    except Exception as e:  # noqa: BLE001
+        probe = {"error": str(e)}
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(w)
+    for line in PAPER_CONTEXT:
+        log(line)
+    res = {
+        "metric": "DM-trial samples/sec", "value": value, "unit": "DM-trial-samples/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
+        "data": "synthetic",
+        "config": {"workload": w.name, "nchans": w.nchans, "ndm": w.ndm, "nsamps_out": w.nsamps_out,
+                   "nbits": w.nbits, "nbeams_per_gpu": w.nbeams, "out_dtype": w.out_dtype,
+                   "max_delay": md, "l2": "256 MiB flush buffer zeroed between timed iterations",
+                   "parallelism": f"replicas x{world} (one seeded beam set per GPU, no collective)"},
+        "real_time_factor": w.obs_seconds() / (ms_per_step * 1e-3),
+        "roofline": roofline, "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": in_bytes,
+                "d2h_bytes_per_step": out_bytes, "steps": e2e_steps, "matches_device_run": same},
+        "gpu_launches": launches, "clocks": clocks, "alu_probe_Tlaneops": probe,
+        "set_dm_list_ms": set_dm_ms, "wall_s_timed_region": wall,
+        "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
+        "paper_context": {"gpu_2011_dm_trial_samples_per_s": 7.5e7, "cpu_dm_trial_samples_per_s": 9.4e6,
+                          "source": "PAPER.md:48, unnamed hardware; context, not target"},
+    }
+    print(json.dumps(res), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args) -> None:
+    """The oracle, as it stands, on the host cores: the base contract's reference arm."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w = W.CONFIGS[args.config]
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w.scaled(nbeams=1), md)
+    stride = max(1, w.ndm // 120)
+    sub = np.ascontiguousarray(delay[:, ::stride])
+    units = sub.shape[1] * w.nsamps_out
+    used = 0
+    for _ in range(args.warmup):
+        oracle.dedisperse(sub, x, w.nbits, w.nsamps_out)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)
+    dt = (time.perf_counter() - t0) / args.steps
+    value = units / dt
+    sample = (f"{sub.shape[1]} of {w.ndm} DM trials (every {stride}th) x {w.nsamps_out} samples x "
+              f"{w.nchans} channels of {w.name} per step")
+    res = {"impl": "reference", "metric": "DM-trial samples/sec", "value": value,
+           "unit": "DM-trial-samples/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
+           "data": "synthetic",
+           "config": {"workload": w.name, "nchans": w.nchans, "ndm": w.ndm, "nsamps_out": w.nsamps_out,
+                      "nbits": w.nbits, "sample": sample},
+           "cpu_baseline": {"value": value, "unit": "DM-trial-samples/s", "cores": used,
+                            "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": 0,
+                   "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(res), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

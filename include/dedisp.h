@@ -1,0 +1,158 @@
+/*
+ * dedisp.h -- C ABI of libdedisp_b200: direct (brute-force) incoherent
+ * dedispersion on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (BASELINE.json:north_star; Sec. 2.2 "each dispersion
+ * trial involves a complete integration over frequency channels"
+ * Sec. 2.2 "the most common 'direct' dedispersion algorithm"):
+ *
+ *     out[d][t] = sum_{c=0}^{nchans-1} in[c][ t + delay[c][d] ]
+ *     delay[c][d] = round( 4148.808 * DM_d * ( f_c^-2 - f_top^-2 ) / dt )
+ *     f_c = f_top + c*df          (MHz; dt in seconds; DM in pc cm^-3)
+ *
+ * round() is to nearest, ties away from zero, on the IEEE double value of the
+ * expression evaluated as ((4148.808*DM) * (1/(f_c*f_c) - 1/(f_top*f_top))) / dt
+ * with one rounding per operation (no FMA contraction).
+ *
+ * Every step (delay table, unpack, gather-sum, output conversion) runs in CUDA
+ * kernels.  There is no CPU fallback: without a usable CUDA device every call
+ * that needs one returns DEDISP_ERR_CUDA.
+ *
+ * Layouts
+ *   in   packed samples, channel-major: nchans rows, each row holds
+ *        nsamps_in = nsamps_out + max_delay samples, time contiguous.
+ *        2-bit: 4 samples per byte, LSB first: sample t of a row is
+ *               (row[t>>2] >> (2*(t&3))) & 3.   8-bit: one unsigned byte per sample.
+ *        Row stride is TIGHT: dedisp_get_in_row_stride_bytes() =
+ *        ceil(nsamps_in*nbits/8) bytes; no alignment is required of the base
+ *        pointer or of the rows.  Bits past the last sample of a row are never read
+ *        as samples.
+ *   out  [ndm][nsamps_out], t fastest, tight, uint32 or float32 (exact: every sum
+ *        is < 2^24).  The base pointer must be 4-byte aligned.
+ *   batch  in[beam][c][t], out[beam][d][t] with caller-given beam strides in bytes.
+ *
+ * Ownership: the plan and everything it allocates on the device belong to the
+ * library (released by dedisp_destroy).  in/out buffers and the stream belong to
+ * the caller.  Host arrays passed in are copied before the call returns.
+ *
+ * Threading: a plan is not thread-safe; distinct plans are independent.
+ *
+ * Errors: every entry point returns a dedisp_status (or a value documented
+ * below); nothing throws or aborts across the ABI.
+ */
+#ifndef DEDISP_B200_H
+#define DEDISP_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dedisp_plan_s *dedisp_plan; /* opaque, library-owned */
+
+typedef enum {
+    DEDISP_OK = 0,
+    DEDISP_ERR_INVALID_ARG = 1,       /* null pointer, non-positive size, bad geometry */
+    DEDISP_ERR_NO_DM_LIST = 2,        /* execute/getter before dedisp_set_dm_list */
+    DEDISP_ERR_UNSUPPORTED_NBITS = 3, /* in_nbits not in {2, 8} */
+    DEDISP_ERR_UNSUPPORTED_DTYPE = 4, /* out_dtype not U32/F32 */
+    DEDISP_ERR_OVERFLOW = 5,          /* nchans*(2^nbits-1) >= 2^24, or a delay beyond int32 */
+    DEDISP_ERR_ALLOC = 6,             /* host or device allocation failed */
+    DEDISP_ERR_CUDA = 7               /* CUDA runtime error; see dedisp_get_last_cuda_error */
+} dedisp_status;
+
+typedef enum { DEDISP_OUT_U32 = 0, DEDISP_OUT_F32 = 1 } dedisp_out_dtype;
+
+/* Kernel selection (diagnostics and A/B evidence; default AUTO). */
+typedef enum {
+    DEDISP_KERNEL_AUTO = 0,     /* bit-sliced tiled kernel when the plan fits it, else DIRECT */
+    DEDISP_KERNEL_DIRECT = 1,   /* one thread per output group, reads packed input from global */
+    DEDISP_KERNEL_BITSLICE = 2  /* TMA-staged (DM x time) tiles, bit-plane carry-save adders */
+} dedisp_kernel;
+
+/* Create a plan for nchans channels, sample time dt_s (s), channel 0 at f_top_mhz,
+ * channel spacing df_mhz (MHz, must be < 0 so that delays are >= 0).
+ * host-only; rejects nchans < 1, dt <= 0, f_top <= 0, df >= 0,
+ * f_top + (nchans-1)*df <= 0, non-finite values.  (north_star: dedisp_plan_create) */
+dedisp_status dedisp_plan_create(dedisp_plan *plan, int nchans, double dt_s, double f_top_mhz,
+                                 double df_mhz);
+
+/* Copy ndm trial DMs (HOST pointer, doubles, any order, duplicates allowed; each
+ * finite and >= 0) and build the delay table ON THE DEVICE (fp64, rule above).
+ * May be called again to replace the list.  Synchronous.
+ * (north_star: dedisp_set_dm_list, subsystem (a).) */
+dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int ndm);
+
+/* Dedisperse one beam.  in_dev/out_dev are DEVICE pointers (layouts above);
+ * cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).
+ * Only enqueues work on the stream; does not synchronise.
+ * (north_star: dedisp_execute, subsystems (b),(c).) */
+dedisp_status dedisp_execute(dedisp_plan plan, long long nsamps_out, const void *in_dev,
+                             int in_nbits, void *out_dev, dedisp_out_dtype out_dtype,
+                             void *cuda_stream);
+
+/* Same for nbeams independent beams in one batched launch (north_star subsystem (d),
+ * BASELINE.json configs[4]; 13 beams: PAPER.md:18).  Beam b reads
+ * in_dev + b*in_beam_stride_bytes and writes out_dev + b*out_beam_stride_bytes
+ * (out stride a multiple of 4). */
+dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamps_out,
+                                   const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
+                                   void *out_dev, size_t out_beam_stride_bytes,
+                                   dedisp_out_dtype out_dtype, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers (tight beam strides): copies the
+ * packed input host->device, runs dedisp_execute_batch, copies the result back
+ * and synchronises.  Device staging buffers are owned and reused by the plan.
+ * Pinned host memory gives full PCIe rate; pageable memory works too. */
+dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps_out,
+                                  const void *in_host, int in_nbits, void *out_host,
+                                  dedisp_out_dtype out_dtype);
+
+/* Release the plan and all device memory it owns.  NULL is accepted. */
+dedisp_status dedisp_destroy(dedisp_plan plan);
+
+/* ---- getters (valid after dedisp_set_dm_list unless noted) ---- */
+
+/* Largest entry of the delay table in samples, or -1 without a DM list. */
+int dedisp_get_max_delay(dedisp_plan plan);
+int dedisp_get_nchans(dedisp_plan plan); /* valid after create */
+int dedisp_get_ndm(dedisp_plan plan);    /* 0 without a DM list */
+
+/* ceil((nsamps_out + max_delay) * in_nbits / 8); 0 on error. */
+size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, int in_nbits);
+
+/* Copy the device-built delay table to host_out[nchans][ndm] (int32, d fastest). */
+dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out);
+
+/* Force a kernel variant for subsequent executes (default DEDISP_KERNEL_AUTO).
+ * Forcing BITSLICE on a plan it cannot serve makes execute return INVALID_ARG. */
+dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which);
+/* Variant the last execute on this plan used (DEDISP_KERNEL_DIRECT/BITSLICE), 0 if none. */
+int dedisp_get_last_kernel(dedisp_plan plan);
+
+/* Per-kernel device timing (for the bench's roofline line).  When enabled, execute
+ * records CUDA events on the caller's stream around the pre-pass (bit-plane unpack)
+ * and around the dominant gather-sum kernel.  dedisp_get_last_kernel_ms waits for
+ * the last execute's events and returns both durations in milliseconds
+ * (prepass 0 when the DIRECT kernel ran). */
+dedisp_status dedisp_set_timing(dedisp_plan plan, int enable);
+dedisp_status dedisp_get_last_kernel_ms(dedisp_plan plan, float *prepass_ms, float *main_ms);
+
+/* Number of kernel launches this library has issued in this process (all plans). */
+unsigned long long dedisp_get_launch_count(void);
+
+/* Last cudaError_t seen by this plan (0 = cudaSuccess) and its text. */
+int dedisp_get_last_cuda_error(dedisp_plan plan);
+const char *dedisp_get_error_string(dedisp_status status);
+
+/* Register-only instruction-rate probe used by the bench to MEASURE the ALU
+ * roofline denominator on the device it runs on.  which: 0 = IADD3 (u32 add),
+ * 1 = LOP3, 2 = SHF funnel shift, 3 = FADD, 4 = IMAD, 5 = LOP3+IMAD mix.
+ * Writes lane-operations per second (warp instructions * 32 / s) to *lane_ops_per_s. */
+dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_B200_H */

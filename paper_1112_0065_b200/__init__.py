@@ -1,1 +1,193 @@
-"""B200-native direct incoherent dedispersion (arxiv/paper_1112_0065 hot path)."""
+"""B200-native direct incoherent dedispersion (hot path of arxiv/paper_1112_0065).
+
+Thin ctypes binding over the C ABI in ``include/dedisp.h`` -- same names, argument
+marshalling only.  Every step of the path (delay table, unpack, gather-sum, output
+conversion) runs in the CUDA kernels of ``libdedisp_b200.so``; PyTorch is used by
+callers for device memory and streams only.  There is no CPU fallback: if the
+library is not built or no CUDA device is usable, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libdedisp_b200.so"
+
+DEDISP_OK = 0
+DEDISP_ERR_INVALID_ARG = 1
+DEDISP_ERR_NO_DM_LIST = 2
+DEDISP_ERR_UNSUPPORTED_NBITS = 3
+DEDISP_ERR_UNSUPPORTED_DTYPE = 4
+DEDISP_ERR_OVERFLOW = 5
+DEDISP_ERR_ALLOC = 6
+DEDISP_ERR_CUDA = 7
+DEDISP_OUT_U32 = 0
+DEDISP_OUT_F32 = 1
+DEDISP_KERNEL_AUTO = 0
+DEDISP_KERNEL_DIRECT = 1
+DEDISP_KERNEL_BITSLICE = 2
+
+# every symbol include/dedisp.h declares: (restype, argtypes)
+_vp, _i, _ll, _sz, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_size_t, ctypes.c_double
+ABI = {
+    "dedisp_plan_create": (_i, [ctypes.POINTER(_vp), _i, _d, _d, _d]),
+    "dedisp_set_dm_list": (_i, [_vp, ctypes.POINTER(_d), _i]),
+    "dedisp_execute": (_i, [_vp, _ll, _vp, _i, _vp, _i, _vp]),
+    "dedisp_execute_batch": (_i, [_vp, _i, _ll, _vp, _sz, _i, _vp, _sz, _i, _vp]),
+    "dedisp_execute_host": (_i, [_vp, _i, _ll, _vp, _i, _vp, _i]),
+    "dedisp_destroy": (_i, [_vp]),
+    "dedisp_get_max_delay": (_i, [_vp]),
+    "dedisp_get_nchans": (_i, [_vp]),
+    "dedisp_get_ndm": (_i, [_vp]),
+    "dedisp_get_in_row_stride_bytes": (_sz, [_vp, _ll, _i]),
+    "dedisp_get_delay_table": (_i, [_vp, ctypes.POINTER(ctypes.c_int32)]),
+    "dedisp_set_kernel": (_i, [_vp, _i]),
+    "dedisp_get_last_kernel": (_i, [_vp]),
+    "dedisp_set_timing": (_i, [_vp, _i]),
+    "dedisp_get_last_kernel_ms": (_i, [_vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
+    "dedisp_get_launch_count": (ctypes.c_ulonglong, []),
+    "dedisp_get_last_cuda_error": (_i, [_vp]),
+    "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
+    "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
+}
+
+_lib = None
+
+
+class DedispError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = lib().dedisp_get_error_string(status).decode()
+        super().__init__(f"{where}: {msg} (status {status}, cudaError {cuda_error})")
+
+
+def lib() -> ctypes.CDLL:
+    """Load libdedisp_b200.so (built in-tree by ``paper_1112_0065_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is not built: run `python -m paper_1112_0065_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(str(LIB_PATH))
+        for name, (res, args) in ABI.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array or plain int."""
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    return x.ctypes.data
+
+
+def _check(plan, st: int, where: str):
+    if st != DEDISP_OK:
+        ce = lib().dedisp_get_last_cuda_error(plan) if plan else 0
+        raise DedispError(st, where, ce)
+
+
+def dedisp_plan_create(nchans: int, dt: float, f_top: float, df: float) -> int:
+    h = _vp()
+    st = lib().dedisp_plan_create(ctypes.byref(h), nchans, dt, f_top, df)
+    _check(None, st, "dedisp_plan_create")
+    return h.value
+
+
+def dedisp_set_dm_list(plan: int, dms) -> None:
+    arr = (ctypes.c_double * len(dms))(*[float(v) for v in dms])
+    _check(plan, lib().dedisp_set_dm_list(plan, arr, len(dms)), "dedisp_set_dm_list")
+
+
+def dedisp_execute(plan: int, nsamps_out: int, in_ptr, in_nbits: int, out_ptr, out_dtype: int,
+                   stream: int = 0) -> None:
+    st = lib().dedisp_execute(plan, nsamps_out, _ptr(in_ptr), in_nbits, _ptr(out_ptr), out_dtype,
+                              stream or None)
+    _check(plan, st, "dedisp_execute")
+
+
+def dedisp_execute_batch(plan: int, nbeams: int, nsamps_out: int, in_ptr, in_beam_stride: int,
+                         in_nbits: int, out_ptr, out_beam_stride: int, out_dtype: int,
+                         stream: int = 0) -> None:
+    st = lib().dedisp_execute_batch(plan, nbeams, nsamps_out, _ptr(in_ptr), in_beam_stride, in_nbits,
+                                    _ptr(out_ptr), out_beam_stride, out_dtype, stream or None)
+    _check(plan, st, "dedisp_execute_batch")
+
+
+def dedisp_execute_host(plan: int, nbeams: int, nsamps_out: int, in_host, in_nbits: int, out_host,
+                        out_dtype: int) -> None:
+    st = lib().dedisp_execute_host(plan, nbeams, nsamps_out, _ptr(in_host), in_nbits,
+                                   _ptr(out_host), out_dtype)
+    _check(plan, st, "dedisp_execute_host")
+
+
+def dedisp_destroy(plan: int) -> None:
+    lib().dedisp_destroy(plan)
+
+
+def dedisp_get_max_delay(plan: int) -> int:
+    return lib().dedisp_get_max_delay(plan)
+
+
+def dedisp_get_nchans(plan: int) -> int:
+    return lib().dedisp_get_nchans(plan)
+
+
+def dedisp_get_ndm(plan: int) -> int:
+    return lib().dedisp_get_ndm(plan)
+
+
+def dedisp_get_in_row_stride_bytes(plan: int, nsamps_out: int, in_nbits: int) -> int:
+    return lib().dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits)
+
+
+def dedisp_get_delay_table(plan: int):
+    import numpy as np
+    out = np.empty((dedisp_get_nchans(plan), dedisp_get_ndm(plan)), dtype=np.int32)
+    st = lib().dedisp_get_delay_table(plan, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
+    _check(plan, st, "dedisp_get_delay_table")
+    return out
+
+
+def dedisp_set_kernel(plan: int, which: int) -> None:
+    _check(plan, lib().dedisp_set_kernel(plan, which), "dedisp_set_kernel")
+
+
+def dedisp_get_last_kernel(plan: int) -> int:
+    return lib().dedisp_get_last_kernel(plan)
+
+
+def dedisp_get_launch_count() -> int:
+    return int(lib().dedisp_get_launch_count())
+
+
+def dedisp_probe_alu_rate(which: int) -> float:
+    v = _d()
+    _check(None, lib().dedisp_probe_alu_rate(which, ctypes.byref(v)), "dedisp_probe_alu_rate")
+    return v.value
+
+
+def dedisp_get_last_cuda_error(plan: int) -> int:
+    return lib().dedisp_get_last_cuda_error(plan)
+
+
+def dedisp_get_error_string(status: int) -> str:
+    return lib().dedisp_get_error_string(status).decode()
+
+
+def dedisp_set_timing(plan: int, enable: bool) -> None:
+    _check(plan, lib().dedisp_set_timing(plan, int(enable)), "dedisp_set_timing")
+
+
+def dedisp_get_last_kernel_ms(plan: int) -> tuple[float, float]:
+    """(prepass_ms, main_ms) of the last execute; needs dedisp_set_timing(plan, True)."""
+    a, b = ctypes.c_float(), ctypes.c_float()
+    _check(plan, lib().dedisp_get_last_kernel_ms(plan, ctypes.byref(a), ctypes.byref(b)),
+           "dedisp_get_last_kernel_ms")
+    return a.value, b.value

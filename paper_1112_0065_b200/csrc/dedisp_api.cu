@@ -1,0 +1,281 @@
+// dedisp_api.cu -- the C ABI of libdedisp_b200.so (include/dedisp.h): plan
+// management, argument validation, kernel dispatch.  No arithmetic of the method
+// happens on the host: the delay table, the unpack, the gather-sum and the output
+// conversion are all CUDA kernels.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "dedisp_internal.h"
+
+unsigned long long g_launch_count = 0;
+
+namespace {
+
+bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+dedisp_status check_exec_args(dedisp_plan plan, int nbeams, long long nsamps_out, const void *in,
+                              int nbits, void *out, dedisp_out_dtype dt)
+{
+    if (!plan || !in || !out || nbeams < 1 || nsamps_out < 1) return DEDISP_ERR_INVALID_ARG;
+    if (plan->ndm < 1 || !plan->d_delay) return DEDISP_ERR_NO_DM_LIST;
+    if (nbits != 2 && nbits != 8) return DEDISP_ERR_UNSUPPORTED_NBITS;
+    if (dt != DEDISP_OUT_U32 && dt != DEDISP_OUT_F32) return DEDISP_ERR_UNSUPPORTED_DTYPE;
+    const long long maxv = (nbits == 2) ? 3 : 255;
+    if ((long long)plan->nchans * maxv >= (1ll << 24)) return DEDISP_ERR_OVERFLOW;
+    if (((uintptr_t)out & 3u) != 0) return DEDISP_ERR_INVALID_ARG;
+    return DEDISP_OK;
+}
+
+void free_dm_state(dedisp_plan p)
+{
+    if (p->d_delay) cudaFree(p->d_delay);
+    p->d_delay = nullptr;
+    p->ndm = 0;
+    p->max_delay = -1;
+    p->dms.clear();
+    bitslice_release(p);
+}
+
+}  // namespace
+
+extern "C" {
+
+dedisp_status dedisp_plan_create(dedisp_plan *plan, int nchans, double dt_s, double f_top_mhz,
+                                 double df_mhz)
+{
+    if (!plan) return DEDISP_ERR_INVALID_ARG;
+    *plan = nullptr;
+    if (nchans < 1 || !finite_pos(dt_s) || !finite_pos(f_top_mhz) || !std::isfinite(df_mhz) ||
+        !(df_mhz < 0.0))
+        return DEDISP_ERR_INVALID_ARG;
+    if (!(f_top_mhz + (double)(nchans - 1) * df_mhz > 0.0)) return DEDISP_ERR_INVALID_ARG;
+    dedisp_plan p = new (std::nothrow) dedisp_plan_s;
+    if (!p) return DEDISP_ERR_ALLOC;
+    p->nchans = nchans;
+    p->dt = dt_s;
+    p->f_top = f_top_mhz;
+    p->df = df_mhz;
+    *plan = p;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int ndm)
+{
+    if (!plan || !dms_host || ndm < 1) return DEDISP_ERR_INVALID_ARG;
+    for (int i = 0; i < ndm; ++i)
+        if (!std::isfinite(dms_host[i]) || dms_host[i] < 0.0) return DEDISP_ERR_INVALID_ARG;
+    DEDISP_CUDA_TRY(plan, cudaGetDevice(&plan->device));
+    free_dm_state(plan);
+    plan->dms.assign(dms_host, dms_host + ndm);
+
+    double *d_dms = nullptr;
+    int *d_flags = nullptr;  // [0] max_delay, [1] overflow
+    const size_t tbl = (size_t)plan->nchans * (size_t)ndm * sizeof(int32_t);
+    cudaError_t e = cudaMalloc(&d_dms, sizeof(double) * ndm);
+    if (e == cudaSuccess) e = cudaMalloc(&d_flags, 2 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&plan->d_delay, tbl);
+    if (e != cudaSuccess) {
+        plan->last_cuda_error = (int)e;
+        cudaFree(d_dms);
+        cudaFree(d_flags);
+        free_dm_state(plan);
+        return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
+    }
+    int flags[2] = {0, 0};
+    e = cudaMemcpy(d_dms, dms_host, sizeof(double) * ndm, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(d_flags, 0, 2 * sizeof(int));
+    if (e == cudaSuccess)
+        e = launch_delay_table(plan->nchans, plan->dt, plan->f_top, plan->df, d_dms, ndm,
+                               plan->d_delay, d_flags, d_flags + 1, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(flags, d_flags, sizeof(flags), cudaMemcpyDeviceToHost);
+    cudaFree(d_dms);
+    cudaFree(d_flags);
+    if (e != cudaSuccess) {
+        plan->last_cuda_error = (int)e;
+        free_dm_state(plan);
+        return DEDISP_ERR_CUDA;
+    }
+    if (flags[1]) {
+        free_dm_state(plan);
+        return DEDISP_ERR_OVERFLOW;
+    }
+    plan->ndm = ndm;
+    plan->max_delay = flags[0];
+    dedisp_status st = bitslice_prepare(plan);
+    if (st != DEDISP_OK) free_dm_state(plan);
+    return st;
+}
+
+dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamps_out,
+                                   const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
+                                   void *out_dev, size_t out_beam_stride_bytes,
+                                   dedisp_out_dtype out_dtype, void *cuda_stream)
+{
+    dedisp_status st = check_exec_args(plan, nbeams, nsamps_out, in_dev, in_nbits, out_dev, out_dtype);
+    if (st != DEDISP_OK) return st;
+    if (nbeams > 1 && (out_beam_stride_bytes & 3u)) return DEDISP_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t row_stride = dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits);
+    const int f32 = (out_dtype == DEDISP_OUT_F32);
+    const uint8_t *in = (const uint8_t *)in_dev;
+
+    if (plan->want != DEDISP_KERNEL_DIRECT) {
+        st = bitslice_execute(plan, nbeams, nsamps_out, in, row_stride, in_beam_stride_bytes,
+                              in_nbits, out_dev, out_beam_stride_bytes, f32, s);
+        if (st == DEDISP_OK) {
+            plan->last_kernel = DEDISP_KERNEL_BITSLICE;
+            return DEDISP_OK;
+        }
+        // INVALID_ARG from bitslice_execute means "plan does not fit this kernel"
+        if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE) return st;
+    }
+    if (plan->timing) cudaEventRecord(plan->ev[2], s);
+    // grid.z limit of the direct kernel
+    for (int b0 = 0; b0 < nbeams; b0 += 65535) {
+        const int nb = (nbeams - b0 < 65535) ? nbeams - b0 : 65535;
+        DEDISP_CUDA_TRY(plan, launch_direct(plan->d_delay, plan->nchans, plan->ndm, nsamps_out,
+                                            in + (size_t)b0 * in_beam_stride_bytes, row_stride,
+                                            in_beam_stride_bytes, in_nbits,
+                                            (uint8_t *)out_dev + (size_t)b0 * out_beam_stride_bytes,
+                                            out_beam_stride_bytes, f32, nb, s));
+    }
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[3], s);
+        plan->timing_valid = true;
+        plan->timing_has_prepass = false;
+    }
+    plan->last_kernel = DEDISP_KERNEL_DIRECT;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_execute(dedisp_plan plan, long long nsamps_out, const void *in_dev,
+                             int in_nbits, void *out_dev, dedisp_out_dtype out_dtype,
+                             void *cuda_stream)
+{
+    return dedisp_execute_batch(plan, 1, nsamps_out, in_dev, 0, in_nbits, out_dev, 0, out_dtype,
+                                cuda_stream);
+}
+
+dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps_out,
+                                  const void *in_host, int in_nbits, void *out_host,
+                                  dedisp_out_dtype out_dtype)
+{
+    if (!plan || !in_host || !out_host || nbeams < 1 || nsamps_out < 1) return DEDISP_ERR_INVALID_ARG;
+    if (plan->ndm < 1) return DEDISP_ERR_NO_DM_LIST;
+    if (in_nbits != 2 && in_nbits != 8) return DEDISP_ERR_UNSUPPORTED_NBITS;
+    const size_t row = dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits);
+    const size_t in_beam = row * (size_t)plan->nchans;
+    const size_t out_beam = (size_t)plan->ndm * (size_t)nsamps_out * 4;
+    const size_t in_bytes = in_beam * nbeams, out_bytes = out_beam * nbeams;
+    if (!plan->host_stream)
+        DEDISP_CUDA_TRY(plan, cudaStreamCreateWithFlags(&plan->host_stream, cudaStreamNonBlocking));
+    if (plan->in_stage_bytes < in_bytes) {
+        cudaFree(plan->d_in_stage);
+        plan->d_in_stage = nullptr;
+        plan->in_stage_bytes = 0;
+        if (cudaMalloc(&plan->d_in_stage, in_bytes) != cudaSuccess) return DEDISP_ERR_ALLOC;
+        plan->in_stage_bytes = in_bytes;
+    }
+    if (plan->out_stage_bytes < out_bytes) {
+        cudaFree(plan->d_out_stage);
+        plan->d_out_stage = nullptr;
+        plan->out_stage_bytes = 0;
+        if (cudaMalloc(&plan->d_out_stage, out_bytes) != cudaSuccess) return DEDISP_ERR_ALLOC;
+        plan->out_stage_bytes = out_bytes;
+    }
+    cudaStream_t s = plan->host_stream;
+    DEDISP_CUDA_TRY(plan, cudaMemcpyAsync(plan->d_in_stage, in_host, in_bytes, cudaMemcpyHostToDevice, s));
+    dedisp_status st = dedisp_execute_batch(plan, nbeams, nsamps_out, plan->d_in_stage, in_beam,
+                                            in_nbits, plan->d_out_stage, out_beam, out_dtype, s);
+    if (st != DEDISP_OK) return st;
+    DEDISP_CUDA_TRY(plan, cudaMemcpyAsync(out_host, plan->d_out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
+    DEDISP_CUDA_TRY(plan, cudaStreamSynchronize(s));
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_destroy(dedisp_plan plan)
+{
+    if (!plan) return DEDISP_OK;
+    free_dm_state(plan);
+    cudaFree(plan->d_planes);
+    cudaFree(plan->d_in_stage);
+    cudaFree(plan->d_out_stage);
+    if (plan->host_stream) cudaStreamDestroy(plan->host_stream);
+    for (int i = 0; i < 4; ++i)
+        if (plan->ev[i]) cudaEventDestroy(plan->ev[i]);
+    delete plan;
+    return DEDISP_OK;
+}
+
+int dedisp_get_max_delay(dedisp_plan plan) { return (plan && plan->ndm > 0) ? plan->max_delay : -1; }
+int dedisp_get_nchans(dedisp_plan plan) { return plan ? plan->nchans : 0; }
+int dedisp_get_ndm(dedisp_plan plan) { return plan ? plan->ndm : 0; }
+
+size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, int in_nbits)
+{
+    if (!plan || plan->ndm < 1 || nsamps_out < 1 || (in_nbits != 2 && in_nbits != 8)) return 0;
+    const unsigned long long n = (unsigned long long)nsamps_out + (unsigned long long)plan->max_delay;
+    return (size_t)((n * (unsigned)in_nbits + 7) / 8);
+}
+
+dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out)
+{
+    if (!plan || !host_out) return DEDISP_ERR_INVALID_ARG;
+    if (plan->ndm < 1 || !plan->d_delay) return DEDISP_ERR_NO_DM_LIST;
+    DEDISP_CUDA_TRY(plan, cudaMemcpy(host_out, plan->d_delay,
+                                     (size_t)plan->nchans * plan->ndm * sizeof(int32_t),
+                                     cudaMemcpyDeviceToHost));
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which)
+{
+    if (!plan || (int)which < 0 || (int)which > 2) return DEDISP_ERR_INVALID_ARG;
+    plan->want = which;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_set_timing(dedisp_plan plan, int enable)
+{
+    if (!plan) return DEDISP_ERR_INVALID_ARG;
+    if (enable)
+        for (int i = 0; i < 4; ++i)
+            if (!plan->ev[i]) DEDISP_CUDA_TRY(plan, cudaEventCreate(&plan->ev[i]));
+    plan->timing = enable != 0;
+    plan->timing_valid = false;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_get_last_kernel_ms(dedisp_plan plan, float *prepass_ms, float *main_ms)
+{
+    if (!plan || !prepass_ms || !main_ms) return DEDISP_ERR_INVALID_ARG;
+    if (!plan->timing || !plan->timing_valid) return DEDISP_ERR_INVALID_ARG;
+    *prepass_ms = 0.f;
+    DEDISP_CUDA_TRY(plan, cudaEventSynchronize(plan->ev[3]));
+    DEDISP_CUDA_TRY(plan, cudaEventElapsedTime(main_ms, plan->ev[2], plan->ev[3]));
+    if (plan->timing_has_prepass)
+        DEDISP_CUDA_TRY(plan, cudaEventElapsedTime(prepass_ms, plan->ev[0], plan->ev[1]));
+    return DEDISP_OK;
+}
+
+int dedisp_get_last_kernel(dedisp_plan plan) { return plan ? plan->last_kernel : 0; }
+unsigned long long dedisp_get_launch_count(void) { return g_launch_count; }
+int dedisp_get_last_cuda_error(dedisp_plan plan) { return plan ? plan->last_cuda_error : 0; }
+
+const char *dedisp_get_error_string(dedisp_status s)
+{
+    switch (s) {
+        case DEDISP_OK: return "ok";
+        case DEDISP_ERR_INVALID_ARG: return "invalid argument";
+        case DEDISP_ERR_NO_DM_LIST: return "no DM list set";
+        case DEDISP_ERR_UNSUPPORTED_NBITS: return "unsupported in_nbits (2 or 8)";
+        case DEDISP_ERR_UNSUPPORTED_DTYPE: return "unsupported output dtype";
+        case DEDISP_ERR_OVERFLOW: return "sum or delay out of range";
+        case DEDISP_ERR_ALLOC: return "allocation failed";
+        case DEDISP_ERR_CUDA: return "CUDA error";
+    }
+    return "unknown status";
+}
+
+}  // extern "C"

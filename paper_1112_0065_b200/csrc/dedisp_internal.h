@@ -1,0 +1,81 @@
+// dedisp_internal.h -- private declarations shared by the translation units of
+// libdedisp_b200.so.  Not part of the ABI (see include/dedisp.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "dedisp.h"
+
+// Geometry of the bit-sliced tiled kernel (bitslice_kernel.cu).
+struct BitsliceGeom {
+    bool usable = false;     // plan can be served by the bit-sliced kernel
+    int nbits = 0;           // geometry was derived for this sample width
+    int nchans_pad = 0;      // channels padded to a multiple of the chunk size
+    int ndm_pad = 0;         // DM trials padded to a multiple of 32 (lanes)
+    int ngroups = 0;         // ndm_pad / 32
+    int win_words = 0;       // smem words per (channel, plane) window
+    int nplanes_acc = 0;     // accumulator bit planes
+};
+
+struct dedisp_plan_s {
+    int nchans = 0;
+    double dt = 0, f_top = 0, df = 0;
+    int ndm = 0;
+    std::vector<double> dms;
+    int device = 0;
+    int32_t *d_delay = nullptr;   // [nchans][ndm]
+    int max_delay = -1;
+    dedisp_kernel want = DEDISP_KERNEL_AUTO;
+    int last_kernel = 0;
+    int last_cuda_error = 0;
+    // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
+    BitsliceGeom geom[2];         // [0]: 2-bit, [1]: 8-bit
+    uint32_t *d_rel[2] = {nullptr, nullptr};   // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
+    int32_t *d_ws[2] = {nullptr, nullptr};     // [ngroups][nchans_pad] window start word
+    uint32_t *d_planes = nullptr; // bit-plane copy of the input
+    size_t planes_bytes = 0;
+    // dedisp_execute_host staging
+    void *d_in_stage = nullptr;
+    size_t in_stage_bytes = 0;
+    void *d_out_stage = nullptr;
+    size_t out_stage_bytes = 0;
+    cudaStream_t host_stream = nullptr;
+    // optional per-kernel timing: ev[0..1] around the pre-pass, ev[2..3] around the main kernel
+    bool timing = false;
+    bool timing_valid = false;
+    bool timing_has_prepass = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+};
+
+extern unsigned long long g_launch_count;
+
+#define DEDISP_CUDA_TRY(plan, expr)                         \
+    do {                                                    \
+        cudaError_t e_ = (expr);                            \
+        if (e_ != cudaSuccess) {                            \
+            if (plan) (plan)->last_cuda_error = (int)e_;    \
+            return DEDISP_ERR_CUDA;                         \
+        }                                                   \
+    } while (0)
+
+// delay_table.cu
+cudaError_t launch_delay_table(int nchans, double dt, double f_top, double df, const double *d_dms,
+                               int ndm, int32_t *d_delay, int *d_max_delay, int *d_overflow,
+                               cudaStream_t s);
+
+// direct_kernel.cu
+cudaError_t launch_direct(const int32_t *d_delay, int nchans, int ndm, long long nsamps_out,
+                          const uint8_t *in, size_t row_stride, size_t in_beam_stride, int nbits,
+                          void *out, size_t out_beam_stride, int out_f32, int nbeams,
+                          cudaStream_t s);
+
+// bitslice_kernel.cu
+dedisp_status bitslice_prepare(dedisp_plan plan);   // called at the end of set_dm_list
+void bitslice_release(dedisp_plan plan);
+// returns DEDISP_OK, or DEDISP_ERR_INVALID_ARG when the plan cannot use this kernel
+dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
+                               const uint8_t *in, size_t row_stride, size_t in_beam_stride,
+                               int nbits, void *out, size_t out_beam_stride, int out_f32,
+                               cudaStream_t s);

@@ -1,0 +1,90 @@
+// probe.cu -- register-only instruction-rate probe (dedisp_probe_alu_rate).
+// The bench uses it to MEASURE the ALU roofline denominator on the device it is
+// running on instead of trusting a spec sheet.
+// Each kernel runs 8 independent dependency chains per thread, 2048 iterations of
+// 8 ops, on 2 CTAs of 1024 threads per SM; results are folded and stored so that
+// nothing is optimised away.
+#include "dedisp_internal.h"
+
+#define CHAINS 8
+#define ITERS 2048
+
+template <int WHICH>
+__global__ void __launch_bounds__(1024) probe_kernel(uint32_t *out, uint32_t seed)
+{
+    uint32_t r[CHAINS];
+    float f[CHAINS];
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) {
+        r[i] = seed * (threadIdx.x + 1) + i * 0x9e3779b9u;
+        f[i] = (float)(r[i] & 1023);
+    }
+    uint32_t k = seed | 1u, m = seed * 7u + 3u;
+    for (int it = 0; it < ITERS; ++it) {
+#pragma unroll
+        for (int i = 0; i < CHAINS; ++i) {
+            if (WHICH == 0)  // IADD3
+                asm volatile("add.u32 %0, %0, %1;" : "+r"(r[i]) : "r"(k));
+            else if (WHICH == 1)  // LOP3 (majority)
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0xE8;" : "+r"(r[i]) : "r"(k), "r"(m));
+            else if (WHICH == 2)  // SHF funnel
+                asm volatile("shf.r.wrap.b32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k), "r"(m));
+            else if (WHICH == 3)  // FADD
+                asm volatile("add.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(1.5f));
+            else if (WHICH == 4)  // IMAD
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k), "r"(m));
+            else {  // alternate LOP3 (alu pipe) and IMAD (fma pipe)
+                if (i & 1)
+                    asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[i]) : "r"(k), "r"(m));
+                else
+                    asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k), "r"(m));
+            }
+        }
+    }
+    uint32_t acc = 0;
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) acc ^= r[i] ^ __float_as_uint(f[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s)
+{
+    if (!lane_ops_per_s || which < 0 || which > 5) return DEDISP_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return DEDISP_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return DEDISP_ERR_CUDA;
+    const int blocks = 2 * sms, threads = 1024;
+    uint32_t *d = nullptr;
+    if (cudaMalloc(&d, (size_t)blocks * threads * 4) != cudaSuccess) return DEDISP_ERR_ALLOC;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, 0);
+        switch (which) {
+            case 0: probe_kernel<0><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 1: probe_kernel<1><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 2: probe_kernel<2><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 3: probe_kernel<3><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 4: probe_kernel<4><<<blocks, threads>>>(d, 12345u + rep); break;
+            default: probe_kernel<5><<<blocks, threads>>>(d, 12345u + rep); break;
+        }
+        ++g_launch_count;
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) {
+            cudaFree(d);
+            return DEDISP_ERR_CUDA;
+        }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    const double ops = (double)blocks * threads * (double)ITERS * CHAINS;
+    *lane_ops_per_s = ops / (best * 1e-3);
+    return DEDISP_OK;
+}

@@ -1,0 +1,235 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by
+element, tolerance 0 (integer sums; BASELINE.json:north_star "GPU output must be
+bit-exact against the oracle")."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+import oracle  # noqa: E402
+import paper_1112_0065_b200 as dd  # noqa: E402
+from paper_1112_0065_b200 import workloads as W  # noqa: E402
+from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs  # noqa: E402
+
+KERNELS = [dd.DEDISP_KERNEL_AUTO, dd.DEDISP_KERNEL_DIRECT]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device (no CPU fallback exists)"
+
+
+# ------------------------------------------------------------ delay table (a1)
+@pytest.mark.parametrize("name", ["tiny", "htru_gulp", "wide8"])
+def test_device_delay_table_equals_oracle(name):
+    w = W.CONFIGS[name]
+    want, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    got = dd.dedisp_get_delay_table(p)
+    assert dd.dedisp_get_max_delay(p) == md
+    assert np.array_equal(got, want)
+    assert dd.dedisp_get_in_row_stride_bytes(p, w.nsamps_out, w.nbits) == \
+        oracle.row_stride_bytes(w.nsamps_out + md, w.nbits)
+    dd.dedisp_destroy(p)
+
+
+def test_delay_table_unsorted_duplicate_dms_and_reset():
+    dms = [300.0, 0.0, 12.5, 300.0, 77.7, 1.0]
+    want, md = oracle.delay_table(96, 64e-6, 1400.0, -3.0, dms)
+    p = make_plan(96, 64e-6, 1400.0, -3.0, dms)
+    assert np.array_equal(dd.dedisp_get_delay_table(p), want) and dd.dedisp_get_max_delay(p) == md
+    dd.dedisp_set_dm_list(p, [5.0])      # replace the list
+    want2, md2 = oracle.delay_table(96, 64e-6, 1400.0, -3.0, [5.0])
+    assert np.array_equal(dd.dedisp_get_delay_table(p), want2) and dd.dedisp_get_max_delay(p) == md2
+    dd.dedisp_destroy(p)
+
+
+def test_delay_rounding_ties_away_on_device():
+    K = 4148.808
+    dms = [0.5, 1.5, 2.5, 3.5, 4.5]
+    want, _ = oracle.delay_table(2, K * 0.75, 2.0, -1.0, dms)
+    p = make_plan(2, K * 0.75, 2.0, -1.0, dms)
+    got = dd.dedisp_get_delay_table(p)
+    assert np.array_equal(got, want) and got[1, 0] == 1 and got[1, 2] == 3
+    dd.dedisp_destroy(p)
+
+
+# ------------------------------------------------------------ small cases
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_hand_worked_example(kernel, golden_dir):
+    from test_oracle_pins import _read_hand
+    h = _read_hand(golden_dir)
+    dms = [float(v) for v in h["dms"]]
+    packed = np.array([[int(b, 16) for b in r] for r in h["packed"]], dtype=np.uint8)[None]
+    want = np.array([[int(v) for v in r] for r in h["out"]], dtype=np.uint32)
+    p = make_plan(4, 1e-3, 1500.0, -100.0, dms, kernel)
+    assert np.array_equal(gpu_dedisperse(p, packed, 2, 6)[0], want)
+    dd.dedisp_destroy(p)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("out_dtype", ["u32", "f32"])
+def test_tiny_config(kernel, out_dtype):
+    w = W.CONFIGS["tiny"]
+    delay, md, x = oracle_inputs(w)
+    want = oracle.dedisperse(delay, x[0], 2, w.nsamps_out)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), kernel)
+    got = gpu_dedisperse(p, x, 2, w.nsamps_out, out_dtype)[0]
+    if out_dtype == "f32":
+        assert got.dtype == np.float32 and np.array_equal(got, oracle.to_f32(want))
+    else:
+        assert np.array_equal(got, want)
+    dd.dedisp_destroy(p)
+
+
+SHAPES = [  # nchans, ndm, nsamps_out, nbits, dm_hi, df
+    (1, 1, 1, 2, 0.0, -1.0), (3, 1, 5, 2, 50.0, -20.0), (37, 5, 333, 2, 120.0, -7.0),
+    (64, 33, 4097, 2, 90.0, -4.0), (130, 70, 2049, 2, 300.0, -2.5), (100, 31, 1000, 8, 150.0, -3.0),
+    (257, 3, 77, 8, 40.0, -1.0), (1024, 40, 3000, 2, 1000.0, -0.390625), (5, 64, 8192, 8, 10.0, -50.0),
+]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("shape", SHAPES)
+def test_random_shapes(kernel, shape):
+    nchans, ndm, nso, nbits, dm_hi, df = shape
+    dms = np.linspace(0.0, dm_hi, ndm)
+    delay, md = oracle.delay_table(nchans, 64e-6, 1500.0, df, dms)
+    x = W.random_small(nchans * 1000 + ndm, nchans, nso + md, nbits)
+    want = oracle.dedisperse(delay, x, nbits, nso)
+    p = make_plan(nchans, 64e-6, 1500.0, df, dms, kernel)
+    for od in ("u32", "f32"):
+        got = gpu_dedisperse(p, x[None], nbits, nso, od)[0]
+        assert np.array_equal(got, want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_unsorted_dm_list_and_big_steps(kernel):
+    dms = [250.0, 0.0, 999.0, 3.0, 3.0, 500.0, 42.0]
+    delay, md = oracle.delay_table(200, 64e-6, 1500.0, -1.5, dms)
+    x = W.random_small(99, 200, 1500 + md, 2)
+    want = oracle.dedisperse(delay, x, 2, 1500)
+    p = make_plan(200, 64e-6, 1500.0, -1.5, dms, kernel)
+    assert np.array_equal(gpu_dedisperse(p, x[None], 2, 1500)[0], want)
+    dd.dedisp_destroy(p)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_extreme_values_and_impulse(kernel):
+    w = W.CONFIGS["tiny"]
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    nin = w.nsamps_out + md
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), kernel)
+    ones = np.full((1, w.nchans, W.row_stride_bytes(nin, 2)), 0xFF, np.uint8)
+    assert (gpu_dedisperse(p, ones, 2, w.nsamps_out) == 3 * w.nchans).all()
+    full8 = np.full((1, w.nchans, nin), 255, np.uint8)
+    assert (gpu_dedisperse(p, full8, 8, w.nsamps_out) == 255 * w.nchans).all()
+    u8 = np.zeros((w.nchans, nin), np.uint8)
+    for c in range(w.nchans):
+        u8[c, 1000 + delay[c, 16]] = 3
+    got = gpu_dedisperse(p, np.stack([W.pack2(r) for r in u8])[None], 2, w.nsamps_out)[0]
+    assert got[16, 1000] == 3 * w.nchans and (got == 3 * w.nchans).sum() == 1
+    dd.dedisp_destroy(p)
+
+
+def test_max_channels_8bit_no_overflow():
+    # 4096 channels of 255: the largest sum the ABI admits (1 044 480 < 2^24), f32 exact
+    dms = [0.0, 30.0]
+    delay, md = oracle.delay_table(4096, 64e-6, 1500.0, -0.09765625, dms)
+    x = np.full((1, 4096, 300 + md), 255, np.uint8)
+    p = make_plan(4096, 64e-6, 1500.0, -0.09765625, dms)
+    got = gpu_dedisperse(p, x, 8, 300, "f32")
+    assert (got == np.float32(4096 * 255)).all()
+    dd.dedisp_destroy(p)
+
+
+# ------------------------------------------------------------ batch / strides / streams / host
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_batch_with_padded_beam_strides_and_side_stream(kernel):
+    w = W.CONFIGS["beams13"].scaled(nchans=48, ndm=40, nsamps_out=3000, df=-8.0, dm_hi=300.0)
+    delay, md, x = oracle_inputs(w)
+    nb, nch, stride = x.shape
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), kernel)
+    in_bs, out_bs = nch * stride + 13, (w.ndm * w.nsamps_out + 5) * 4
+    xin = torch.zeros(nb * in_bs, dtype=torch.uint8, device="cuda")
+    for b in range(nb):
+        xin[b * in_bs: b * in_bs + nch * stride] = torch.from_numpy(x[b].ravel()).cuda()
+    out = torch.zeros(nb * out_bs // 4, dtype=torch.int32, device="cuda")
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        dd.dedisp_execute_batch(p, nb, w.nsamps_out, xin, in_bs, 2, out, out_bs, dd.DEDISP_OUT_U32,
+                                s.cuda_stream)
+    s.synchronize()
+    got = out.cpu().numpy().view(np.uint32)
+    for b in range(nb):
+        want = oracle.dedisperse(delay, x[b], 2, w.nsamps_out)
+        o = got[b * out_bs // 4: b * out_bs // 4 + w.ndm * w.nsamps_out].reshape(w.ndm, -1)
+        assert np.array_equal(o, want), b
+        assert not got[b * out_bs // 4 + w.ndm * w.nsamps_out: (b + 1) * out_bs // 4].any()
+    dd.dedisp_destroy(p)
+
+
+def test_unaligned_input_pointer():
+    w = W.CONFIGS["tiny"]
+    delay, md, x = oracle_inputs(w)
+    want = oracle.dedisperse(delay, x[0], 2, w.nsamps_out)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    buf = torch.zeros(x.size + 16, dtype=torch.uint8, device="cuda")
+    for off in (1, 3, 8):
+        buf[off: off + x.size] = torch.from_numpy(x.ravel()).cuda()
+        out = torch.zeros((w.ndm, w.nsamps_out), dtype=torch.int32, device="cuda")
+        dd.dedisp_execute(p, w.nsamps_out, buf.data_ptr() + off, 2, out, dd.DEDISP_OUT_U32,
+                          torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), want), off
+    dd.dedisp_destroy(p)
+
+
+def test_execute_host_end_to_end():
+    w = W.CONFIGS["beams13"].scaled(nchans=64, ndm=48, nsamps_out=5000, df=-6.0, dm_hi=200.0, nbeams=3)
+    delay, md, x = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    xin = torch.from_numpy(x).pin_memory()
+    for od, code in (("u32", dd.DEDISP_OUT_U32), ("f32", dd.DEDISP_OUT_F32)):
+        out = torch.empty((3, w.ndm, w.nsamps_out),
+                          dtype=torch.int32 if od == "u32" else torch.float32).pin_memory()
+        dd.dedisp_execute_host(p, 3, w.nsamps_out, xin, 2, out, code)
+        for b in range(3):
+            want = oracle.dedisperse(delay, x[b], 2, w.nsamps_out)
+            got = out[b].numpy()
+            assert np.array_equal(got.view(np.uint32) if od == "u32" else got,
+                                  want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
+def test_execute_errors():
+    p = make_plan(8, 64e-6, 1500.0, -10.0, [0.0, 10.0])
+    x = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
+    o = torch.zeros(1 << 16, dtype=torch.int32, device="cuda")
+    cases = [((p, 100, x, 4, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_UNSUPPORTED_NBITS),
+             ((p, 100, x, 2, o, 5), dd.DEDISP_ERR_UNSUPPORTED_DTYPE),
+             ((p, 0, x, 2, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_INVALID_ARG),
+             ((p, 100, 0, 2, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_INVALID_ARG),
+             ((p, 100, x, 2, o.data_ptr() + 2, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_INVALID_ARG)]
+    for args, code in cases:
+        with pytest.raises(dd.DedispError) as e:
+            dd.dedisp_execute(*args)
+        assert e.value.status == code
+    dd.dedisp_destroy(p)
+    big = make_plan(70000, 64e-6, 1500.0, -0.01, [0.0])
+    with pytest.raises(dd.DedispError) as e:   # 70000*255 >= 2^24
+        dd.dedisp_execute(big, 10, x, 8, o, dd.DEDISP_OUT_U32)
+    assert e.value.status == dd.DEDISP_ERR_OVERFLOW
+    dd.dedisp_destroy(big)
+
+
+def test_launch_counter_and_probe():
+    n0 = dd.dedisp_get_launch_count()
+    p = make_plan(8, 64e-6, 1500.0, -10.0, [0.0, 10.0])
+    assert dd.dedisp_get_launch_count() > n0
+    dd.dedisp_destroy(p)
+    r = dd.dedisp_probe_alu_rate(0)
+    assert 1e12 < r < 1e15
