@@ -13,7 +13,8 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libdedisp_b200.so"
-SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_kernel.cu", "probe.cu"]
+SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
+           "probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=false", "-Xptxas", "-v"]
 

@@ -1,0 +1,180 @@
+// bitslice_prepare.cu -- set-up kernels of the tiled path:
+//   * tile tables (window start per (DM group, channel); per-lane offset/shift words)
+//     derived ON THE DEVICE from the device delay table (north_star subsystem (a));
+//   * the unpack pre-pass (north_star subsystem (b)): packed 2-bit rows -> bit planes,
+//     read with 128-bit loads whatever the row alignment, de-interleaved in registers.
+#include <algorithm>
+#include <numeric>
+
+#include "bitslice_common.cuh"
+#include "dedisp_internal.h"
+
+// One block per DM group g (32 sorted trial DMs = 32 lanes), threads over channels.
+//   ws[g][c]        = (delay[c][lane 0] >> 5) rounded down to a multiple of 4 words
+//   rel[g][c][lane] = (((delay[c][d_lane] >> 5) - ws) * 4) << 16 | (delay[c][d_lane] & 31)
+// Padding lanes repeat the group's last real DM; padding channels get zeros.
+__global__ void bitslice_tables_kernel(const int32_t *__restrict__ delay, int nchans, int ndm,
+                                       const int32_t *__restrict__ sorted,  // [ngroups*32], -1 = pad
+                                       int nchans_pad, int32_t *__restrict__ ws,
+                                       uint32_t *__restrict__ rel, int *max_off_words)
+{
+    const int g = blockIdx.x;
+    int worst = 0;
+    for (int c = threadIdx.x; c < nchans_pad; c += blockDim.x) {
+        const size_t row = (size_t)g * nchans_pad + c;
+        if (c >= nchans) {
+            ws[row] = 0;
+            for (int l = 0; l < 32; ++l) rel[row * 32 + l] = 0;
+            continue;
+        }
+        const int32_t *dl = delay + (size_t)c * ndm;
+        const int d0 = sorted[g * 32];
+        const int w0 = (dl[d0] >> 5) & ~3;
+        ws[row] = w0;
+        int last = d0;
+        for (int l = 0; l < 32; ++l) {
+            const int d = sorted[g * 32 + l];
+            if (d >= 0) last = d;
+            const int dv = dl[last];
+            const int off = (dv >> 5) - w0;   // >= 0 because the list is sorted ascending
+            worst = max(worst, off);
+            rel[row * 32 + l] = ((uint32_t)(off * 4) << 16) | (uint32_t)(dv & 31);
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) worst = max(worst, __shfl_xor_sync(0xffffffffu, worst, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(max_off_words, worst);
+}
+
+// ---- unpack pre-pass -------------------------------------------------------
+__device__ __forceinline__ uint32_t even_bits_to_low16(uint32_t x)
+{
+    x &= 0x55555555u;
+    x = (x | (x >> 1)) & 0x33333333u;
+    x = (x | (x >> 2)) & 0x0f0f0f0fu;
+    x = (x | (x >> 4)) & 0x00ff00ffu;
+    x = (x | (x >> 8)) & 0x0000ffffu;
+    return x;
+}
+
+// Thread i of a row turns input bytes [16i, 16i+16) (64 two-bit samples) into two
+// words of plane 0 and two words of plane 1.  The two aligned 16-byte vectors that
+// cover those bytes are loaded with 128-bit loads and byte-aligned in registers.
+__global__ void __launch_bounds__(128)
+planes2_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride,
+               int nchans, const uint8_t *valid_begin, const uint8_t *valid_end,
+               uint32_t *__restrict__ planes, int row_pitch, int nchans_pad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 64-sample block
+    const int c = blockIdx.y, b = blockIdx.z;
+    if (2 * i >= row_pitch) return;
+    uint32_t r[4] = {0u, 0u, 0u, 0u};
+    const long long nvalid = (long long)row_stride - 16ll * i;   // bytes of this row still valid
+    if (c < nchans && nvalid > 0) {
+        const uint8_t *a = in + (size_t)b * in_beam_stride + (size_t)c * row_stride + 16u * (size_t)i;
+        const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)15;
+        const int m = (int)((uintptr_t)a & 15);
+        uint4 lo = make_uint4(0, 0, 0, 0), hi = make_uint4(0, 0, 0, 0);
+        // a 16-byte block is loaded only if it overlaps the caller's buffer
+        if (a0 + 16 > (uintptr_t)valid_begin && a0 < (uintptr_t)valid_end)
+            lo = __ldg(reinterpret_cast<const uint4 *>(a0));
+        if (m && a0 + 16 < (uintptr_t)valid_end) hi = __ldg(reinterpret_cast<const uint4 *>(a0 + 16));
+        const uint32_t v[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+        const int q = m >> 2, sh = (m & 3) * 8;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t x0 = v[k], x1 = v[k + 1];
+            if (q == 1) { x0 = v[k + 1]; x1 = v[k + 2]; }
+            if (q == 2) { x0 = v[k + 2]; x1 = v[k + 3]; }
+            if (q == 3) { x0 = v[k + 3]; x1 = v[k + 4 < 8 ? k + 4 : 7]; }
+            r[k] = __funnelshift_r(x0, x1, sh);
+            // zero the bytes past the end of the row
+            const long long nb = nvalid - 4 * k;
+            if (nb <= 0) r[k] = 0;
+            else if (nb < 4) r[k] &= (1u << (8 * (int)nb)) - 1u;
+        }
+    }
+    if (c < nchans_pad) {
+        uint2 p0, p1;
+        p0.x = even_bits_to_low16(r[0]) | (even_bits_to_low16(r[1]) << 16);
+        p0.y = even_bits_to_low16(r[2]) | (even_bits_to_low16(r[3]) << 16);
+        p1.x = even_bits_to_low16(r[0] >> 1) | (even_bits_to_low16(r[1] >> 1) << 16);
+        p1.y = even_bits_to_low16(r[2] >> 1) | (even_bits_to_low16(r[3] >> 1) << 16);
+        uint32_t *row0 = planes + (((size_t)b * nchans_pad + c) * 2) * (size_t)row_pitch;
+        *reinterpret_cast<uint2 *>(row0 + 2 * i) = p0;
+        *reinterpret_cast<uint2 *>(row0 + row_pitch + 2 * i) = p1;
+    }
+}
+
+cudaError_t launch_planes2(const uint8_t *in, size_t in_beam_stride, size_t row_stride, int nchans,
+                           int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
+                           cudaStream_t s)
+{
+    const uint8_t *vend = in + (size_t)(nbeams - 1) * in_beam_stride + (size_t)nchans * row_stride;
+    dim3 block(128), grid((row_pitch / 2 + 127) / 128, nchans_pad, nbeams);
+    planes2_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
+                                          row_pitch, nchans_pad);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+// ---- host side of set_dm_list ------------------------------------------------
+void bitslice_release(dedisp_plan p)
+{
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(p->d_rel[k]);
+        cudaFree(p->d_ws[k]);
+        p->d_rel[k] = nullptr;
+        p->d_ws[k] = nullptr;
+        p->geom[k] = BitsliceGeom();
+    }
+    cudaFree(p->d_order);
+    p->d_order = nullptr;
+}
+
+dedisp_status bitslice_prepare(dedisp_plan p)
+{
+    // Only the 2-bit geometry exists so far; 8-bit plans run the DIRECT kernel.
+    BitsliceGeom &G = p->geom[0];
+    G = BitsliceGeom();
+    G.nbits = 2;
+    if ((long long)p->nchans * 3 >= 4096) return DEDISP_OK;   // 12 accumulator planes
+    const int ndm = p->ndm;
+    G.ndm_pad = (ndm + 31) / 32 * 32;
+    G.ngroups = G.ndm_pad / 32;
+    G.nchans_pad = (p->nchans + bs::CH - 1) / bs::CH * bs::CH;
+    G.nplanes_acc = 12;
+    // trial DMs sorted ascending (stable) -> lanes of a group have nearby, monotone delays
+    std::vector<int32_t> sorted(G.ndm_pad, -1);
+    std::iota(sorted.begin(), sorted.begin() + ndm, 0);
+    std::stable_sort(sorted.begin(), sorted.begin() + ndm,
+                     [&](int a, int b) { return p->dms[a] < p->dms[b]; });
+    int *d_max = nullptr;
+    const size_t nrows = (size_t)G.ngroups * G.nchans_pad;
+    cudaError_t e = cudaMalloc(&p->d_order, sizeof(int32_t) * G.ndm_pad);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws[0], sizeof(int32_t) * nrows);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_rel[0], sizeof(uint32_t) * nrows * 32);
+    if (e == cudaSuccess) e = cudaMalloc(&d_max, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(d_max, 0, sizeof(int));
+    if (e == cudaSuccess)
+        e = cudaMemcpy(p->d_order, sorted.data(), sizeof(int32_t) * G.ndm_pad, cudaMemcpyHostToDevice);
+    int max_off = 0;
+    if (e == cudaSuccess) {
+        bitslice_tables_kernel<<<G.ngroups, 256>>>(p->d_delay, p->nchans, ndm, p->d_order,
+                                                   G.nchans_pad, p->d_ws[0], p->d_rel[0], d_max);
+        ++g_launch_count;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(&max_off, d_max, sizeof(int), cudaMemcpyDeviceToHost);
+    cudaFree(d_max);
+    if (e != cudaSuccess) {
+        p->last_cuda_error = (int)e;
+        return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
+    }
+    // a thread reads words off + warp*W + j, j = 0..W  =>  off_max + TILE_WORDS + 1 words
+    const int need = max_off + bs::TILE_WORDS + 1;
+    if (need <= bs::WIN_SMALL) G.win_words = bs::WIN_SMALL;
+    else if (need <= bs::WIN_LARGE) G.win_words = bs::WIN_LARGE;
+    else return DEDISP_OK;   // DM steps too coarse for a tile window: DIRECT kernel serves the plan
+    G.usable = true;
+    return DEDISP_OK;
+}

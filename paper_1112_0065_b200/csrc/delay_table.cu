@@ -14,9 +14,9 @@ __global__ void delay_table_kernel(int nchans, double dt, double f_top, double d
                                    int32_t *__restrict__ delay, int *max_delay, int *overflow)
 {
     const int d = blockIdx.x * blockDim.x + threadIdx.x;
-    const int c = blockIdx.y;
     int v = 0;
-    if (d < ndm) {
+    for (int c = blockIdx.y; c < nchans; c += gridDim.y) {
+        if (d >= ndm) break;
         const double fc = __dadd_rn(f_top, __dmul_rn((double)c, df));
         const double a = __dsub_rn(__ddiv_rn(1.0, __dmul_rn(fc, fc)),
                                    __ddiv_rn(1.0, __dmul_rn(f_top, f_top)));
@@ -30,8 +30,8 @@ __global__ void delay_table_kernel(int nchans, double dt, double f_top, double d
             atomicExch(overflow, 1);
             r = 0.0;
         }
-        v = (int)r;
-        delay[(size_t)c * ndm + d] = v;
+        delay[(size_t)c * ndm + d] = (int)r;
+        v = max(v, (int)r);
     }
     // block max -> one atomic per warp
     for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
@@ -42,7 +42,7 @@ cudaError_t launch_delay_table(int nchans, double dt, double f_top, double df, c
                                int ndm, int32_t *d_delay, int *d_max_delay, int *d_overflow,
                                cudaStream_t s)
 {
-    dim3 block(128), grid((ndm + 127) / 128, nchans);
+    dim3 block(128), grid((ndm + 127) / 128, nchans < 65535 ? nchans : 65535);
     delay_table_kernel<<<grid, block, 0, s>>>(nchans, dt, f_top, df, d_dms, ndm, d_delay,
                                               d_max_delay, d_overflow);
     ++g_launch_count;
