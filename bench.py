@@ -126,12 +126,16 @@ def cpu_baseline(w: W.Workload, seconds_hint: str = "") -> dict:
 
 def ncu_traffic_bytes(config: str):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (or None)."""
-    p = ROOT / "profiles" / "traffic.json"
-    if p.exists():
-        try:
-            return json.loads(p.read_text()).get(config)
-        except (ValueError, OSError):
-            return None
+    p = ROOT / "profiles" / "traffic.csv"
+    if not p.exists():
+        return None
+    for line in p.read_text().splitlines():
+        f = line.split(",")
+        if len(f) >= 2 and f[0] == config:
+            try:
+                return float(f[1])
+            except ValueError:
+                return None
     return None
 
 
