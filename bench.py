@@ -24,6 +24,7 @@ import numpy as np
 
 ROOT = Path(__file__).resolve().parent
 sys.path.insert(0, str(ROOT))
+from paper_1112_0065_b200 import replicas  # noqa: E402
 from paper_1112_0065_b200 import workloads as W  # noqa: E402
 
 SM_COUNT_NOMINAL = 148
@@ -164,7 +165,7 @@ def run_ours(args) -> None:
         kw = dict(pulse_sweep=dd.dedisp_get_delay_table(p2), pulses=pp)
         dd.dedisp_destroy(p2)
     # each rank gets its own seeded beam(s): beam index offset by rank
-    beams = [W.generate(w, md, beam=b + rank * w.nbeams, **kw) for b in range(w.nbeams)]
+    beams = [W.generate(w, md, beam=b, **kw) for b in replicas.beam_indices(rank, w.nbeams)]
     host_in = torch.from_numpy(np.stack(beams)).pin_memory()
     nb, nch, stride = host_in.shape
     assert stride == dd.dedisp_get_in_row_stride_bytes(plan, w.nsamps_out, w.nbits)
@@ -208,14 +209,12 @@ def run_ours(args) -> None:
     launches = dd.dedisp_get_launch_count() - launches0
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
     if world > 1:
         dist.barrier()
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_ms = float(total_ms.item())
+    total_ms = replicas.max_over_ranks(sum(step_ms), dev)
     ms_per_step = total_ms / args.steps
     units_step = w.dm_trial_samples() * world
-    value = units_step / (ms_per_step * 1e-3)
+    value = replicas.job_throughput(w.dm_trial_samples(), world, ms_per_step * 1e-3)
 
     # ---- end to end through the public host-buffer call (H2D + kernels + D2H inside the timing)
     host_out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=out.dtype).pin_memory()
@@ -227,10 +226,8 @@ def run_ours(args) -> None:
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
-    e2e_s = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_value = units_step / float(e2e_s.item())
+    e2e_s = replicas.max_over_ranks((time.perf_counter() - t0) / e2e_steps, dev)
+    e2e_value = replicas.job_throughput(w.dm_trial_samples(), world, e2e_s)
     same = bool(torch.equal(host_out.to(dev), out))
     kernel_used = dd.dedisp_get_last_kernel(plan)
     dd.dedisp_destroy(plan)
