@@ -113,7 +113,7 @@ def cpu_baseline(w: W.Workload, seconds_hint: str = "") -> dict:
     import oracle
     delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
     x = W.generate(w.scaled(nbeams=1), md)
-    stride = max(1, w.ndm // 240)
+    stride = max(1, (w.ndm * w.nsamps_out) // (1200 * 65536))   # ~ one HTRU gulp of work
     sub = np.ascontiguousarray(delay[:, ::stride])
     t0 = time.perf_counter()
     _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)

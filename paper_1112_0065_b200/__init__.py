@@ -9,10 +9,12 @@ library is not built or no CUDA device is usable, calls raise.
 from __future__ import annotations
 
 import ctypes
+import os
 from pathlib import Path
 
 _PKG = Path(__file__).resolve().parent
-LIB_PATH = _PKG / "libdedisp_b200.so"
+# DEDISP_B200_LIB selects a tuning variant built by build.build(defs=..., out=...)
+LIB_PATH = Path(os.environ.get("DEDISP_B200_LIB") or (_PKG / "libdedisp_b200.so"))
 
 DEDISP_OK = 0
 DEDISP_ERR_INVALID_ARG = 1

@@ -35,20 +35,23 @@ def stale() -> bool:
     return any(d.stat().st_mtime > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not stale():
+def build(force: bool = False, verbose: bool = False, defs: list[str] | None = None,
+          out: Path | None = None) -> Path:
+    """defs/out: tuning variants for A/B runs (e.g. defs=["BS_NW=20"], out=Path("x.so"))."""
+    target = Path(out) if out else LIB
+    if not force and not defs and not out and not stale():
         return LIB
-    tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
-    cmd = [_nvcc(), *NVCC_FLAGS, f"-I{INCLUDE}", f"-I{CSRC}", "-o", str(tmp)] \
-        + [str(CSRC / s) for s in SOURCES]
+    tmp = target.with_suffix(f".tmp{os.getpid()}.so")
+    cmd = [_nvcc(), *NVCC_FLAGS, *[f"-D{d}" for d in (defs or [])], f"-I{INCLUDE}", f"-I{CSRC}",
+           "-o", str(tmp)] + [str(CSRC / s) for s in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed building libdedisp_b200.so")
-    (PKG / "build_ptxas.log").write_text(r.stdout + r.stderr)
-    os.replace(tmp, LIB)
-    return LIB
+    (target.parent / (target.stem + "_ptxas.log")).write_text(r.stdout + r.stderr)
+    os.replace(tmp, target)
+    return target
 
 
 if __name__ == "__main__":

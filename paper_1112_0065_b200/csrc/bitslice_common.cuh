@@ -13,17 +13,33 @@
 #pragma once
 #include <stdint.h>
 
+// tuning knobs (overridable with -D for A/B runs; defaults are the measured best)
+#ifndef BS_NW
+#define BS_NW 15
+#endif
+#ifndef BS_W
+#define BS_W 4
+#endif
+#ifndef BS_TREE_K
+#define BS_TREE_K 4
+#endif
+#ifndef BS_NSTAGE
+#define BS_NSTAGE 3
+#endif
+
 namespace bs {
-constexpr int NW = 16;                  // consumer warps per CTA
-constexpr int W = 4;                    // 32-sample words per thread per tile
-constexpr int TILE_WORDS = NW * W;      // 64 words
-constexpr int TILE_SAMPS = TILE_WORDS * 32;   // 2048 output samples per tile
+constexpr int NW = BS_NW;               // consumer warps per CTA
+constexpr int W = BS_W;                 // 32-sample words per thread per tile
+constexpr int TILE_WORDS = NW * W;      // 60 words
+constexpr int TILE_SAMPS = TILE_WORDS * 32;   // 1920 output samples per tile
 constexpr int LANES = 32;               // trial DMs per tile (one per lane)
-constexpr int CH = 16;                  // channels per pipeline stage
-constexpr int NSTAGE = 4;               // TMA ring depth
+constexpr int TREE_K = BS_TREE_K;       // adder tree depth: 2^(K+1) channels per tree
+constexpr int CH = 1 << (TREE_K + 1);   // channels per pipeline stage (one tree)
+constexpr int NSTAGE = BS_NSTAGE;       // TMA ring depth
 constexpr int NTHREADS = (NW + 1) * 32; // + 1 producer warp
 constexpr int WIN_SMALL = 96;           // window words per (channel, plane): small DM steps
 constexpr int WIN_LARGE = 224;          // large DM steps
+static_assert(TILE_WORDS % 4 == 0, "tile starts must stay 16-byte aligned for the TMA bulk copies");
 }  // namespace bs
 
 struct BitsliceParams {

@@ -136,8 +136,6 @@ struct Tree<0, C0, WIN> {
     }
 };
 
-constexpr int TREE_K = 3;   // 2^(K+1) = 16 = CH channels per tree
-static_assert((1 << (TREE_K + 1)) == CH, "one tree per pipeline stage");
 
 template <int WIN, int NP, bool F32>
 __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const BitsliceParams P, int vec_ok)
@@ -175,10 +173,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const Bitslic
                 const uint32_t fb = full0 + 8 * stage;
                 if (lane == 0) mbar_expect_tx(fb, S::BYTES);
                 __syncwarp();
-                // lane -> (channel, plane) of the chunk: CH * 2 = 32 copies
-                const int c = chunk * CH + (lane >> 1), pidx = lane & 1;
-                const uint32_t *src = pl + ((size_t)c * 2 + pidx) * P.row_pitch + P.ws[grow + c];
-                bulk_g2s(sb + lane * (WIN * 4), src, WIN * 4, fb);
+                // one copy per (channel, plane) of the chunk: CH * 2 copies spread over the lanes
+#pragma unroll
+                for (int i = lane; i < CH * 2; i += 32) {
+                    const int c = chunk * CH + (i >> 1), pidx = i & 1;
+                    const uint32_t *src = pl + ((size_t)c * 2 + pidx) * P.row_pitch + P.ws[grow + c];
+                    bulk_g2s(sb + i * (WIN * 4), src, WIN * 4, fb);
+                }
                 if (lane == 0)
                     bulk_g2s(sb + S::DATA_BYTES, P.rel + (grow + (size_t)chunk * CH) * LANES,
                              S::REL_BYTES, fb);
