@@ -5,15 +5,16 @@
 // Data layout in HBM for the tiled kernel ("planes"): the packed filterbank is
 // re-laid once per execute as bit planes,
 //     planes[beam][c][p][word],   word w of plane p holds bit p of samples 32w .. 32w+31
-//                                 of channel c (sample 32w+i in bit i),
+//                                 of channel c (sample 32w+i in bit i),   p < nbits
 // rows padded with zeros to `row_pitch` words (a multiple of 4 => every window the
 // TMA bulk copies fetch is 16-byte aligned), channels padded with all-zero rows to a
-// multiple of CH.  A (DM x time) tile of 32 trial DMs (one per lane) x TILE_WORDS
+// multiple of CH_PAD.  A (DM x time) tile of 32 trial DMs (one per lane) x TILE_WORDS
 // words then needs, per channel and plane, one contiguous window of WIN words.
 #pragma once
 #include <stdint.h>
 
-// tuning knobs (overridable with -D for A/B runs; defaults are the measured best)
+// tuning knobs of the 2-bit kernel (overridable with -D for A/B runs; defaults are
+// the measured best, profiles/r1_*.md)
 #ifndef BS_NW
 #define BS_NW 15
 #endif
@@ -28,22 +29,32 @@
 #endif
 
 namespace bs {
-constexpr int NW = BS_NW;               // consumer warps per CTA
-constexpr int W = BS_W;                 // 32-sample words per thread per tile
-constexpr int TILE_WORDS = NW * W;      // 60 words
-constexpr int TILE_SAMPS = TILE_WORDS * 32;   // 1920 output samples per tile
-constexpr int LANES = 32;               // trial DMs per tile (one per lane)
-constexpr int TREE_K = BS_TREE_K;       // adder tree depth: 2^(K+1) channels per tree
-constexpr int CH = 1 << (TREE_K + 1);   // channels per pipeline stage (one tree)
-constexpr int NSTAGE = BS_NSTAGE;       // TMA ring depth
-constexpr int NTHREADS = (NW + 1) * 32; // + 1 producer warp
-constexpr int WIN_SMALL = 96;           // window words per (channel, plane): small DM steps
-constexpr int WIN_LARGE = 224;          // large DM steps
-static_assert(TILE_WORDS % 4 == 0, "tile starts must stay 16-byte aligned for the TMA bulk copies");
+constexpr int LANES = 32;    // trial DMs per tile (one per lane)
+constexpr int CH_PAD = 32;   // channels are padded to a multiple of this (>= every Cfg::CH)
+
+// NB  input bit planes (= sample width)     NW  consumer warps per CTA
+// W   32-sample words per thread per tile   K   adder-tree depth: 2^(K+1) channels per stage
+// NP  accumulator bit planes (sums < 2^NP)  WIN_S / WIN_L  window words per (channel, plane)
+template <int NB_, int NW_, int W_, int K_, int NSTAGE_, int NP_, int WIN_S_, int WIN_L_>
+struct Cfg {
+    static constexpr int NB = NB_, NW = NW_, W = W_, K = K_, NSTAGE = NSTAGE_, NP = NP_;
+    static constexpr int WIN_S = WIN_S_, WIN_L = WIN_L_;
+    static constexpr int TILE_WORDS = NW * W;
+    static constexpr int TILE_SAMPS = TILE_WORDS * 32;
+    static constexpr int CH = 1 << (K + 1);          // channels per pipeline stage (one tree)
+    static constexpr int NTHREADS = (NW + 1) * 32;   // + 1 producer warp
+    static_assert(TILE_WORDS % 4 == 0, "tile starts must stay 16-byte aligned for the TMA bulk copies");
+    static_assert(CH_PAD % CH == 0, "channel padding must cover whole stages");
+    static_assert(NB + K + 1 <= NP, "tree carries must fit the accumulator");
+};
+// 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
+using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
+// 8-bit samples: 14 x 2 words = 896-sample tiles, 8-channel trees, sums < 2^20
+using Cfg8 = Cfg<8, 14, 2, 2, 3, 20, 64, 128>;
 }  // namespace bs
 
 struct BitsliceParams {
-    const uint32_t *planes;    // [nbeams][nchans_pad][NPL][row_pitch]
+    const uint32_t *planes;    // [nbeams][nchans_pad][NB][row_pitch]
     const int32_t *ws;         // [ngroups][nchans_pad] window start word (multiple of 4)
     const uint32_t *rel;       // [ngroups][nchans_pad][32] (byte offset in window << 16) | bit shift
     const int32_t *order;      // [ngroups*32] output row of each lane, -1 = padding lane
@@ -56,4 +67,5 @@ struct BitsliceParams {
     int ngroups;
     int ntiles;                // time tiles per (beam, group)
     int nbeams;
+    int vec_ok;                // output rows are 16-byte aligned: 128-bit stores allowed
 };

@@ -70,78 +70,134 @@ __device__ __forceinline__ uint32_t full_add(uint32_t &acc, uint32_t x, uint32_t
     return carry;
 }
 
-template <int WIN>
+template <class C, int WIN>
 struct Stage {
-    static constexpr int CPITCH = 2 * WIN * 4;          // bytes per channel: plane 0 then plane 1
-    static constexpr int DATA_BYTES = CH * CPITCH;
-    static constexpr int REL_BYTES = CH * LANES * 4;
+    static constexpr int CPITCH = C::NB * WIN * 4;      // bytes per channel: plane 0, plane 1, ...
+    static constexpr int DATA_BYTES = C::CH * CPITCH;
+    static constexpr int REL_BYTES = C::CH * LANES * 4;
     static constexpr int BYTES = DATA_BYTES + REL_BYTES;
+    static constexpr int SMEM = C::NSTAGE * BYTES + 2 * C::NSTAGE * 8;
 };
 
-// Load the W+1 words of both planes of channel C that this thread's 4 output words
+// Load the W+1 words of every plane of channel CI that this thread's W output words
 // need, and align them to the output time axis (one funnel shift per plane-word).
-template <int C, int WIN>
+template <class C, int CI, int WIN>
 __device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *relp,
-                                             uint32_t (&a)[W], uint32_t (&b)[W])
+                                             uint32_t (&x)[C::NB][C::W])
 {
-    const uint32_t r = relp[C * LANES];
-    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + C * (2 * WIN);
-    uint32_t w0[W + 1], w1[W + 1];
+    const uint32_t r = relp[CI * LANES];
+    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (C::NB * WIN);
 #pragma unroll
-    for (int j = 0; j <= W; ++j) {
-        w0[j] = wp[j];
-        w1[j] = wp[WIN + j];
-    }
+    for (int p = 0; p < C::NB; ++p) {
+        uint32_t w[C::W + 1];
 #pragma unroll
-    for (int j = 0; j < W; ++j) {
-        a[j] = __funnelshift_r(w0[j], w0[j + 1], r);   // shift amount = r & 31
-        b[j] = __funnelshift_r(w1[j], w1[j + 1], r);
+        for (int j = 0; j <= C::W; ++j) w[j] = wp[p * WIN + j];
+#pragma unroll
+        for (int j = 0; j < C::W; ++j) x[p][j] = __funnelshift_r(w[j], w[j + 1], r);   // shift = r & 31
     }
 }
 
-// Tree<K> adds 2^(K+1) channels (C0 ...) into the counter planes 0..K+1 and hands
-// back one carry word of weight 2^(K+1) (u) and one of weight 2^(K+2) (v).
-template <int K, int C0, int WIN>
+// Tree<K> adds 2^(K+1) channels (C0 ...) into counter planes 0 .. K+NB-1 and hands
+// back NB carry words e[i] of weight 2^(K+1+i): carry-save all the way, no ripple.
+template <class C, int K, int C0, int WIN>
 struct Tree {
-    template <int NP>
-    static __device__ __forceinline__ void run(uint32_t (&A)[NP][W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&u)[W],
-                                               uint32_t (&v)[W])
+    static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
+                                               const uint32_t *relp, uint32_t (&e)[C::NB][C::W])
     {
-        uint32_t u1[W], v1[W], u2[W], v2[W];
-        Tree<K - 1, C0, WIN>::run(A, tb, relp, u1, v1);
-        Tree<K - 1, C0 + (1 << K), WIN>::run(A, tb, relp, u2, v2);
+        uint32_t e1[C::NB][C::W], e2[C::NB][C::W];
+        Tree<C, K - 1, C0, WIN>::run(A, tb, relp, e1);
+        Tree<C, K - 1, C0 + (1 << K), WIN>::run(A, tb, relp, e2);
 #pragma unroll
-        for (int j = 0; j < W; ++j) {
-            u[j] = full_add(A[K][j], u1[j], u2[j]);
-            v[j] = full_add(A[K + 1][j], v1[j], v2[j]);
-        }
+        for (int i = 0; i < C::NB; ++i)
+#pragma unroll
+            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[K + i][j], e1[i][j], e2[i][j]);
     }
 };
-template <int C0, int WIN>
-struct Tree<0, C0, WIN> {
-    template <int NP>
-    static __device__ __forceinline__ void run(uint32_t (&A)[NP][W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&u)[W],
-                                               uint32_t (&v)[W])
+template <class C, int C0, int WIN>
+struct Tree<C, 0, C0, WIN> {
+    static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
+                                               const uint32_t *relp, uint32_t (&e)[C::NB][C::W])
     {
-        uint32_t a0[W], b0[W], a1[W], b1[W];
-        load_aligned<C0, WIN>(tb, relp, a0, b0);
-        load_aligned<C0 + 1, WIN>(tb, relp, a1, b1);
+        uint32_t x0[C::NB][C::W], x1[C::NB][C::W];
+        load_aligned<C, C0, WIN>(tb, relp, x0);
+        load_aligned<C, C0 + 1, WIN>(tb, relp, x1);
 #pragma unroll
-        for (int j = 0; j < W; ++j) {
-            u[j] = full_add(A[0][j], a0[j], a1[j]);   // bit 0 of both channels
-            v[j] = full_add(A[1][j], b0[j], b1[j]);   // bit 1 of both channels
-        }
+        for (int i = 0; i < C::NB; ++i)   // bit i of both channels
+#pragma unroll
+            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[i][j], x0[i][j], x1[i][j]);
     }
 };
 
-
-template <int WIN, int NP, bool F32>
-__global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const BitsliceParams P, int vec_ok)
+// Transpose step of the un-slice: rows a (index i, i & s == 0) and b (index i + s)
+// exchange the bit blocks (i, j | s) <-> (i + s, j).  m selects columns with j & s == 0.
+__device__ __forceinline__ void swap_block(uint32_t &a, uint32_t &b, int s, uint32_t m)
 {
+    const uint32_t bs = b << s, as = a >> s;
+    const uint32_t na = (a & m) | (bs & ~m);
+    b = (b & ~m) | (as & m);
+    a = na;
+}
+
+template <bool F32>
+__device__ __forceinline__ uint32_t cvt_out(uint32_t v)
+{
+    // exact for v < 2^23: 2^23 + v is representable, subtracting 2^23 leaves float(v)
+    return F32 ? __float_as_uint(__uint_as_float(v | 0x4B000000u) - 8388608.0f) : v;
+}
+
+// Un-slice one word (32 samples) of the counter and store it.  NP <= 16: the planes
+// are transposed as two 16x16 bit blocks side by side (M[i] = out[i] | out[i+16] << 16);
+// NP > 16: a full 32x32 transpose.
+template <int NP, int W, bool F32>
+__device__ __forceinline__ void unslice_store(uint32_t (&A)[NP][W], int j, uint8_t *orow, long long t0,
+                                              long long nsamps_out, bool fast)
+{
+    constexpr int R = (NP <= 16) ? 16 : 32;
+    uint32_t M[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) M[i] = (i < NP) ? A[i][j] : 0u;
+    if (R == 32) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) swap_block(M[i], M[i + 16], 16, 0x0000FFFFu);
+    }
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if ((i & 8) == 0) swap_block(M[i], M[i + 8], 8, 0x00FF00FFu);
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if ((i & 4) == 0) swap_block(M[i], M[i + 4], 4, 0x0F0F0F0Fu);
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if ((i & 2) == 0) swap_block(M[i], M[i + 2], 2, 0x33333333u);
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if ((i & 1) == 0) swap_block(M[i], M[i + 1], 1, 0x55555555u);
+    uint32_t o[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        uint32_t v;
+        if (R == 32) v = M[i];
+        else v = (i < 16) ? (M[i] & 0xFFFFu) : (M[i - 16] >> 16);
+        o[i] = cvt_out<F32>(v);
+    }
+    if (fast) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            *reinterpret_cast<uint4 *>(orow + (size_t)(t0 + 4 * q) * 4) =
+                make_uint4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+            if (t0 + i < nsamps_out) *reinterpret_cast<uint32_t *>(orow + (size_t)(t0 + i) * 4) = o[i];
+    }
+}
+
+template <class C, int WIN, bool F32>
+__global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const BitsliceParams P)
+{
+    constexpr int NW = C::NW, W = C::W, NP = C::NP, NB = C::NB, CH = C::CH, NSTAGE = C::NSTAGE;
     extern __shared__ __align__(128) uint8_t smem[];
-    using S = Stage<WIN>;
+    using S = Stage<C, WIN>;
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + NSTAGE * S::BYTES);
     const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NSTAGE);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -165,7 +221,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const Bitslic
             const int tile = (int)(item % P.ntiles);
             const int g = (int)((item / P.ntiles) % P.ngroups);
             const int beam = (int)(item / ((long long)P.ntiles * P.ngroups));
-            const uint32_t *pl = P.planes + (size_t)beam * P.beam_pitch_words + (size_t)tile * TILE_WORDS;
+            const uint32_t *pl = P.planes + (size_t)beam * P.beam_pitch_words + (size_t)tile * C::TILE_WORDS;
             const size_t grow = (size_t)g * P.nchans_pad;
             for (int chunk = 0; chunk < nchunks; ++chunk) {
                 mbar_wait(empty0 + 8 * stage, phase ^ 1);
@@ -173,11 +229,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const Bitslic
                 const uint32_t fb = full0 + 8 * stage;
                 if (lane == 0) mbar_expect_tx(fb, S::BYTES);
                 __syncwarp();
-                // one copy per (channel, plane) of the chunk: CH * 2 copies spread over the lanes
+                // one copy per (channel, plane) of the chunk, spread over the lanes
 #pragma unroll
-                for (int i = lane; i < CH * 2; i += 32) {
-                    const int c = chunk * CH + (i >> 1), pidx = i & 1;
-                    const uint32_t *src = pl + ((size_t)c * 2 + pidx) * P.row_pitch + P.ws[grow + c];
+                for (int i = lane; i < CH * NB; i += 32) {
+                    const int c = chunk * CH + i / NB, pidx = i % NB;
+                    const uint32_t *src = pl + ((size_t)c * NB + pidx) * P.row_pitch + P.ws[grow + c];
                     bulk_g2s(sb + i * (WIN * 4), src, WIN * 4, fb);
                 }
                 if (lane == 0)
@@ -202,22 +258,22 @@ __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const Bitslic
             const uint8_t *sb = smem + stage * S::BYTES;
             const uint8_t *tb = sb + warp * (W * 4);
             const uint32_t *relp = reinterpret_cast<const uint32_t *>(sb + S::DATA_BYTES) + lane;
-            uint32_t u[W], v[W];
-            Tree<TREE_K, 0, WIN>::run(A, tb, relp, u, v);
-            // fold the two carry words (weights 2^(K+1), 2^(K+2)) into the upper planes
+            uint32_t e[NB][W];
+            Tree<C, C::K, 0, WIN>::run(A, tb, relp, e);
+            // add the NB carry words (weights 2^(K+1) ...) into the upper planes: ripple carry
 #pragma unroll
             for (int j = 0; j < W; ++j) {
-                uint32_t c = u[j];
-                uint32_t t = A[TREE_K + 1][j] & c;
-                A[TREE_K + 1][j] ^= c;
-                c = full_add(A[TREE_K + 2][j], t, v[j]);
+                uint32_t c = A[C::K + 1][j] & e[0][j];
+                A[C::K + 1][j] ^= e[0][j];
 #pragma unroll
-                for (int p = TREE_K + 3; p < NP - 1; ++p) {
-                    t = A[p][j] & c;
+                for (int i = 1; i < NB; ++i) c = full_add(A[C::K + 1 + i][j], e[i][j], c);
+#pragma unroll
+                for (int p = C::K + 1 + NB; p < NP - 1; ++p) {
+                    const uint32_t t = A[p][j] & c;
                     A[p][j] ^= c;
                     c = t;
                 }
-                A[NP - 1][j] ^= c;
+                if (C::K + 1 + NB < NP) A[NP - 1][j] ^= c;
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty0 + 8 * stage);
@@ -233,72 +289,42 @@ __global__ void __launch_bounds__(NTHREADS, 1) bitslice_dedisperse(const Bitslic
                         (size_t)(d < 0 ? 0 : d) * (size_t)P.nsamps_out * 4;
 #pragma unroll
         for (int j = 0; j < W; ++j) {
-            const long long t0 = (long long)tile * TILE_SAMPS + (warp * W + j) * 32;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                uint32_t lo = 0, hi = 0;
-#pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    const uint32_t n = (A[p][j] >> (4 * q)) & 0xFu;
-                    // spread the 4 bits of n to bit (p & 7) of the 4 bytes
-                    const int pp = p & 7;
-                    const uint32_t s = (n * (0x00204081u << pp)) & (0x01010101u << pp);
-                    if (p < 8) lo |= s; else hi |= s;
-                }
-                uint32_t o[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    o[k] = __byte_perm(lo, hi, 0x40 + 0x11 * k) & 0xFFFFu;
-                    if (F32) o[k] = __float_as_uint(__uint_as_float(o[k] | 0x4B000000u) - 8388608.0f);
-                }
-                const long long t = t0 + 4 * q;
-                if (d >= 0) {
-                    if (vec_ok && t + 3 < P.nsamps_out) {
-                        *reinterpret_cast<uint4 *>(orow + (size_t)t * 4) = make_uint4(o[0], o[1], o[2], o[3]);
-                    } else {
-#pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            if (t + k < P.nsamps_out)
-                                *reinterpret_cast<uint32_t *>(orow + (size_t)(t + k) * 4) = o[k];
-                    }
-                }
-            }
+            const long long t0 = (long long)tile * C::TILE_SAMPS + (warp * W + j) * 32;
+            if (d >= 0 && t0 < P.nsamps_out)
+                unslice_store<NP, W, F32>(A, j, orow, t0, P.nsamps_out,
+                                          P.vec_ok && t0 + 32 <= P.nsamps_out);
 #pragma unroll
             for (int p = 0; p < NP; ++p) A[p][j] = 0;
         }
     }
 }
 
-template <int WIN, int NP, bool F32>
-cudaError_t launch_one(const BitsliceParams &P, int vec_ok, int grid, cudaStream_t s)
+template <class C, int WIN, bool F32>
+cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s)
 {
-    constexpr int SMEM = NSTAGE * Stage<WIN>::BYTES + 2 * NSTAGE * 8;
+    constexpr int SMEM = Stage<C, WIN>::SMEM;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(bitslice_dedisperse<WIN, NP, F32>,
+        cudaError_t e = cudaFuncSetAttribute(bitslice_dedisperse<C, WIN, F32>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    bitslice_dedisperse<WIN, NP, F32><<<grid, NTHREADS, SMEM, s>>>(P, vec_ok);
+    bitslice_dedisperse<C, WIN, F32><<<grid, C::NTHREADS, SMEM, s>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }
 
-}  // namespace
-
-dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
-                               const uint8_t *in, size_t row_stride, size_t in_beam_stride,
-                               int nbits, void *out, size_t out_beam_stride, int out_f32,
-                               cudaStream_t s)
+template <class C>
+dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, long long nsamps_out,
+                          const uint8_t *in, size_t row_stride, size_t in_beam_stride, void *out,
+                          size_t out_beam_stride, int out_f32, cudaStream_t s)
 {
-    if (nbits != 2) return DEDISP_ERR_INVALID_ARG;
-    const BitsliceGeom &G = plan->geom[0];
-    if (!G.usable) return DEDISP_ERR_INVALID_ARG;
-    const long long ntiles = (nsamps_out + TILE_SAMPS - 1) / TILE_SAMPS;
-    const long long pitch = (((long long)(plan->max_delay >> 5) + ntiles * TILE_WORDS + G.win_words + 4) + 3) & ~3ll;
-    if (ntiles > 0x7fffffff / TILE_WORDS || pitch > 0x7fffffff) return DEDISP_ERR_INVALID_ARG;
-    const size_t beam_pitch = (size_t)G.nchans_pad * 2 * (size_t)pitch;
+    const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
+    const long long pitch =
+        (((long long)(plan->max_delay >> 5) + ntiles * C::TILE_WORDS + G.win_words + 4) + 3) & ~3ll;
+    if (ntiles > 0x7fffffff / C::TILE_WORDS || pitch > 0x7fffffff) return DEDISP_ERR_INVALID_ARG;
+    const size_t beam_pitch = (size_t)G.nchans_pad * C::NB * (size_t)pitch;
     const size_t need = beam_pitch * (size_t)nbeams * 4;
     if (plan->planes_bytes < need) {
         cudaFree(plan->d_planes);
@@ -314,16 +340,16 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device));
 
     if (plan->timing) cudaEventRecord(plan->ev[0], s);
-    DEDISP_CUDA_TRY(plan, launch_planes2(in, in_beam_stride, row_stride, plan->nchans, nbeams,
-                                         plan->d_planes, (int)pitch, G.nchans_pad, s));
+    DEDISP_CUDA_TRY(plan, launch_planes(C::NB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
+                                        plan->d_planes, (int)pitch, G.nchans_pad, s));
     if (plan->timing) {
         cudaEventRecord(plan->ev[1], s);
         cudaEventRecord(plan->ev[2], s);
     }
     BitsliceParams P;
     P.planes = plan->d_planes;
-    P.ws = plan->d_ws[0];
-    P.rel = plan->d_rel[0];
+    P.ws = plan->d_ws;
+    P.rel = plan->d_rel;
     P.order = plan->d_order;
     P.out = (uint8_t *)out;
     P.out_beam_stride = out_beam_stride;
@@ -334,17 +360,15 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     P.ngroups = G.ngroups;
     P.ntiles = (int)ntiles;
     P.nbeams = nbeams;
+    P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
+               (nbeams == 1 || out_beam_stride % 16 == 0);
     const long long nitems = (long long)nbeams * G.ngroups * ntiles;
     const int grid = (int)(nitems < sms ? nitems : sms);
-    const int vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
-                       (nbeams == 1 || out_beam_stride % 16 == 0);
     cudaError_t e;
-    if (G.win_words == WIN_SMALL)
-        e = out_f32 ? launch_one<WIN_SMALL, 12, true>(P, vec_ok, grid, s)
-                    : launch_one<WIN_SMALL, 12, false>(P, vec_ok, grid, s);
+    if (G.win_words == C::WIN_S)
+        e = out_f32 ? launch_one<C, C::WIN_S, true>(P, grid, s) : launch_one<C, C::WIN_S, false>(P, grid, s);
     else
-        e = out_f32 ? launch_one<WIN_LARGE, 12, true>(P, vec_ok, grid, s)
-                    : launch_one<WIN_LARGE, 12, false>(P, vec_ok, grid, s);
+        e = out_f32 ? launch_one<C, C::WIN_L, true>(P, grid, s) : launch_one<C, C::WIN_L, false>(P, grid, s);
     DEDISP_CUDA_TRY(plan, e);
     if (plan->timing) {
         cudaEventRecord(plan->ev[3], s);
@@ -352,4 +376,20 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
         plan->timing_has_prepass = true;
     }
     return DEDISP_OK;
+}
+
+}  // namespace
+
+dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
+                               const uint8_t *in, size_t row_stride, size_t in_beam_stride,
+                               int nbits, void *out, size_t out_beam_stride, int out_f32,
+                               cudaStream_t s)
+{
+    const BitsliceGeom &G = plan->geom[nbits == 2 ? 0 : 1];
+    if (!G.usable) return DEDISP_ERR_INVALID_ARG;
+    if (nbits == 2)
+        return execute_cfg<Cfg2>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                 out_beam_stride, out_f32, s);
+    return execute_cfg<Cfg8>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                             out_beam_stride, out_f32, s);
 }

@@ -105,14 +105,69 @@ planes2_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row
     }
 }
 
-cudaError_t launch_planes2(const uint8_t *in, size_t in_beam_stride, size_t row_stride, int nchans,
-                           int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
-                           cudaStream_t s)
+// 8-bit samples: thread i of a row turns input bytes [32i, 32i+32) (32 samples) into
+// one word of each of the 8 bit planes.  Three aligned 16-byte vectors cover the bytes.
+__global__ void __launch_bounds__(128)
+planes8_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride,
+               int nchans, const uint8_t *valid_begin, const uint8_t *valid_end,
+               uint32_t *__restrict__ planes, int row_pitch, int nchans_pad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 32-sample word
+    const int c = blockIdx.y, b = blockIdx.z;
+    if (i >= row_pitch || c >= nchans_pad) return;
+    uint32_t pw[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+    const long long nvalid = (long long)row_stride - 32ll * i;
+    if (c < nchans && nvalid > 0) {
+        const uint8_t *a = in + (size_t)b * in_beam_stride + (size_t)c * row_stride + 32u * (size_t)i;
+        const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)15;
+        const int m = (int)((uintptr_t)a & 15);
+        uint32_t v[12];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            uint4 q = make_uint4(0, 0, 0, 0);
+            const uintptr_t ak = a0 + 16u * k;
+            if ((k < 2 || m) && ak + 16 > (uintptr_t)valid_begin && ak < (uintptr_t)valid_end)
+                q = __ldg(reinterpret_cast<const uint4 *>(ak));
+            v[4 * k] = q.x; v[4 * k + 1] = q.y; v[4 * k + 2] = q.z; v[4 * k + 3] = q.w;
+        }
+        const int q4 = m >> 2, sh = (m & 3) * 8;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            uint32_t x0 = v[k], x1 = v[k + 1];
+            if (q4 == 1) { x0 = v[k + 1]; x1 = v[k + 2]; }
+            if (q4 == 2) { x0 = v[k + 2]; x1 = v[k + 3]; }
+            if (q4 == 3) { x0 = v[k + 3]; x1 = v[k + 4]; }
+            uint32_t r = __funnelshift_r(x0, x1, sh);     // samples 4k .. 4k+3, one per byte
+            const long long nb = nvalid - 4 * k;
+            if (nb <= 0) r = 0;
+            else if (nb < 4) r &= (1u << (8 * (int)nb)) - 1u;
+            // bit p of the 4 bytes -> a nibble: the multiply gathers bits 0,8,16,24 into 24..27
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+                const uint32_t nib = (((r >> p) & 0x01010101u) * 0x01020408u) >> 24;
+                pw[p] |= nib << (4 * k);
+            }
+        }
+    }
+    uint32_t *row0 = planes + (((size_t)b * nchans_pad + c) * 8) * (size_t)row_pitch;
+#pragma unroll
+    for (int p = 0; p < 8; ++p) row0[(size_t)p * row_pitch + i] = pw[p];
+}
+
+cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
+                          int nchans, int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
+                          cudaStream_t s)
 {
     const uint8_t *vend = in + (size_t)(nbeams - 1) * in_beam_stride + (size_t)nchans * row_stride;
-    dim3 block(128), grid((row_pitch / 2 + 127) / 128, nchans_pad, nbeams);
-    planes2_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
-                                          row_pitch, nchans_pad);
+    if (nbits == 2) {
+        dim3 block(128), grid((row_pitch / 2 + 127) / 128, nchans_pad, nbeams);
+        planes2_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
+                                              row_pitch, nchans_pad);
+    } else {
+        dim3 block(128), grid((row_pitch + 127) / 128, nchans_pad, nbeams);
+        planes8_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
+                                              row_pitch, nchans_pad);
+    }
     ++g_launch_count;
     return cudaGetLastError();
 }
@@ -120,47 +175,56 @@ cudaError_t launch_planes2(const uint8_t *in, size_t in_beam_stride, size_t row_
 // ---- host side of set_dm_list ------------------------------------------------
 void bitslice_release(dedisp_plan p)
 {
-    for (int k = 0; k < 2; ++k) {
-        cudaFree(p->d_rel[k]);
-        cudaFree(p->d_ws[k]);
-        p->d_rel[k] = nullptr;
-        p->d_ws[k] = nullptr;
-        p->geom[k] = BitsliceGeom();
-    }
+    cudaFree(p->d_rel);
+    cudaFree(p->d_ws);
     cudaFree(p->d_order);
+    p->d_rel = nullptr;
+    p->d_ws = nullptr;
     p->d_order = nullptr;
+    p->geom[0] = BitsliceGeom();
+    p->geom[1] = BitsliceGeom();
+}
+
+template <class C>
+static void fill_geom(BitsliceGeom &G, int nbits, int nchans_pad, int ndm_pad, int max_off, long long maxsum)
+{
+    G = BitsliceGeom();
+    G.nbits = nbits;
+    G.nchans_pad = nchans_pad;
+    G.ndm_pad = ndm_pad;
+    G.ngroups = ndm_pad / 32;
+    G.nplanes_acc = C::NP;
+    // a thread reads words off + warp*W + j, j = 0..W  =>  off_max + TILE_WORDS + 1 words
+    const int need = max_off + C::TILE_WORDS + 1;
+    if (need <= C::WIN_S) G.win_words = C::WIN_S;
+    else if (need <= C::WIN_L) G.win_words = C::WIN_L;
+    else return;   // DM steps too coarse for a tile window: the DIRECT kernel serves the plan
+    G.usable = maxsum < (1ll << C::NP);
 }
 
 dedisp_status bitslice_prepare(dedisp_plan p)
 {
-    // Only the 2-bit geometry exists so far; 8-bit plans run the DIRECT kernel.
-    BitsliceGeom &G = p->geom[0];
-    G = BitsliceGeom();
-    G.nbits = 2;
-    if ((long long)p->nchans * 3 >= 4096) return DEDISP_OK;   // 12 accumulator planes
     const int ndm = p->ndm;
-    G.ndm_pad = (ndm + 31) / 32 * 32;
-    G.ngroups = G.ndm_pad / 32;
-    G.nchans_pad = (p->nchans + bs::CH - 1) / bs::CH * bs::CH;
-    G.nplanes_acc = 12;
+    const int ndm_pad = (ndm + 31) / 32 * 32, ngroups = ndm_pad / 32;
+    const int nchans_pad = (p->nchans + bs::CH_PAD - 1) / bs::CH_PAD * bs::CH_PAD;
     // trial DMs sorted ascending (stable) -> lanes of a group have nearby, monotone delays
-    std::vector<int32_t> sorted(G.ndm_pad, -1);
+    std::vector<int32_t> sorted(ndm_pad, -1);
     std::iota(sorted.begin(), sorted.begin() + ndm, 0);
     std::stable_sort(sorted.begin(), sorted.begin() + ndm,
                      [&](int a, int b) { return p->dms[a] < p->dms[b]; });
     int *d_max = nullptr;
-    const size_t nrows = (size_t)G.ngroups * G.nchans_pad;
-    cudaError_t e = cudaMalloc(&p->d_order, sizeof(int32_t) * G.ndm_pad);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws[0], sizeof(int32_t) * nrows);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_rel[0], sizeof(uint32_t) * nrows * 32);
+    const size_t nrows = (size_t)ngroups * nchans_pad;
+    cudaError_t e = cudaMalloc(&p->d_order, sizeof(int32_t) * ndm_pad);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws, sizeof(int32_t) * nrows);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_rel, sizeof(uint32_t) * nrows * 32);
     if (e == cudaSuccess) e = cudaMalloc(&d_max, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(d_max, 0, sizeof(int));
     if (e == cudaSuccess)
-        e = cudaMemcpy(p->d_order, sorted.data(), sizeof(int32_t) * G.ndm_pad, cudaMemcpyHostToDevice);
+        e = cudaMemcpy(p->d_order, sorted.data(), sizeof(int32_t) * ndm_pad, cudaMemcpyHostToDevice);
     int max_off = 0;
     if (e == cudaSuccess) {
-        bitslice_tables_kernel<<<G.ngroups, 256>>>(p->d_delay, p->nchans, ndm, p->d_order,
-                                                   G.nchans_pad, p->d_ws[0], p->d_rel[0], d_max);
+        bitslice_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, p->d_order, nchans_pad,
+                                                 p->d_ws, p->d_rel, d_max);
         ++g_launch_count;
         e = cudaGetLastError();
     }
@@ -170,11 +234,7 @@ dedisp_status bitslice_prepare(dedisp_plan p)
         p->last_cuda_error = (int)e;
         return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
     }
-    // a thread reads words off + warp*W + j, j = 0..W  =>  off_max + TILE_WORDS + 1 words
-    const int need = max_off + bs::TILE_WORDS + 1;
-    if (need <= bs::WIN_SMALL) G.win_words = bs::WIN_SMALL;
-    else if (need <= bs::WIN_LARGE) G.win_words = bs::WIN_LARGE;
-    else return DEDISP_OK;   // DM steps too coarse for a tile window: DIRECT kernel serves the plan
-    G.usable = true;
+    fill_geom<bs::Cfg2>(p->geom[0], 2, nchans_pad, ndm_pad, max_off, 3ll * p->nchans);
+    fill_geom<bs::Cfg8>(p->geom[1], 8, nchans_pad, ndm_pad, max_off, 255ll * p->nchans);
     return DEDISP_OK;
 }

@@ -32,8 +32,8 @@ struct dedisp_plan_s {
     int last_cuda_error = 0;
     // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
     BitsliceGeom geom[2];         // [0]: 2-bit, [1]: 8-bit
-    uint32_t *d_rel[2] = {nullptr, nullptr};   // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
-    int32_t *d_ws[2] = {nullptr, nullptr};     // [ngroups][nchans_pad] window start word
+    uint32_t *d_rel = nullptr;    // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
+    int32_t *d_ws = nullptr;      // [ngroups][nchans_pad] window start word
     int32_t *d_order = nullptr;   // [ndm_pad] trial index of each sorted lane, -1 = padding
     uint32_t *d_planes = nullptr; // bit-plane copy of the input
     size_t planes_bytes = 0;
@@ -73,9 +73,9 @@ cudaError_t launch_direct(const int32_t *d_delay, int nchans, int ndm, long long
                           cudaStream_t s);
 
 // bitslice_prepare.cu / bitslice_kernel.cu
-cudaError_t launch_planes2(const uint8_t *in, size_t in_beam_stride, size_t row_stride, int nchans,
-                           int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
-                           cudaStream_t s);
+cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
+                          int nchans, int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
+                          cudaStream_t s);
 dedisp_status bitslice_prepare(dedisp_plan plan);   // called at the end of set_dm_list
 void bitslice_release(dedisp_plan plan);
 // returns DEDISP_OK, or DEDISP_ERR_INVALID_ARG when the plan cannot use this kernel
