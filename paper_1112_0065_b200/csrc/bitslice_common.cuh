@@ -28,6 +28,20 @@
 #define BS_NSTAGE 3
 #endif
 
+// ... and of the 8-bit kernel
+#ifndef BS8_NW
+#define BS8_NW 14
+#endif
+#ifndef BS8_W
+#define BS8_W 2
+#endif
+#ifndef BS8_TREE_K
+#define BS8_TREE_K 2
+#endif
+#ifndef BS8_NSTAGE
+#define BS8_NSTAGE 3
+#endif
+
 namespace bs {
 constexpr int LANES = 32;    // trial DMs per tile (one per lane)
 constexpr int CH_PAD = 32;   // channels are padded to a multiple of this (>= every Cfg::CH)
@@ -50,7 +64,7 @@ struct Cfg {
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
 using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
 // 8-bit samples: 14 x 2 words = 896-sample tiles, 8-channel trees, sums < 2^20
-using Cfg8 = Cfg<8, 14, 2, 2, 3, 20, 64, 128>;
+using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, 64, 128>;
 }  // namespace bs
 
 struct BitsliceParams {
