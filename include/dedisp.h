@@ -139,6 +139,39 @@ int dedisp_get_last_kernel(dedisp_plan plan);
 dedisp_status dedisp_set_timing(dedisp_plan plan, int enable);
 dedisp_status dedisp_get_last_kernel_ms(dedisp_plan plan, float *prepass_ms, float *main_ms);
 
+/* ---- downstream of dedispersion ---- */
+
+/* Largest boxcar width dedisp_matched_filter accepts. */
+#define DEDISP_MF_MAX_WIDTH 8192
+
+/* Baseline removal by running mean, then boxcar matched filters, over nrows
+ * independent time series of nsamps samples (Sec. 2.3 "compute a running
+ * mean for the data with a given window size ... and then subtracting this off the
+ * original data ... exploit a parallel prefix sum ... subtracting the points at plus
+ * and minus the window radius"; "convolving the time series with boxcar
+ * functions of increasing sizes (e.g., 2, 4, 8 etc. samples) ... in the same manner
+ * using the parallel prefix sum").  With N = 2*radius+1 and a(t) = clip(t-radius, 0,
+ * nsamps-N) (the window keeps its length and stops at the ends of the series):
+ *     y[t]   = x[t] - (1/N) * sum_{k=a(t)}^{a(t)+N-1} x[k]
+ *     z_w[t] = (1/sqrt(w)) * sum_{k=0}^{w-1} y[t+k]   for 0 <= t <= nsamps-w, else 0
+ * (the 1/sqrt(w) keeps the white-noise variance equal for all widths).
+ *   x_dev   DEVICE, [nrows][nsamps] tight, uint32 or float32 holding exact integers
+ *           <= x_max (the output of dedisp_execute[_batch], any number of beams, is
+ *           such an array with nrows = nbeams*ndm); 4-byte aligned.
+ *   x_max   caller's upper bound on x (0 = 2^24-1; values >= 2^24 are rejected with
+ *           DEDISP_ERR_OVERFLOW).  It selects 32- or 64-bit exact integer arithmetic.
+ *   widths_host  HOST array of nwidths boxcar widths, 1 <= w <= min(nsamps,
+ *           DEDISP_MF_MAX_WIDTH), 1 <= nwidths <= 16; copied during the call.
+ *   z_dev   DEVICE float32 [nwidths][nrows][nsamps] tight, written completely.
+ * All sums are exact integers; each output is fl32(numerator) * fl32(1/(N sqrt(w))),
+ * i.e. within 1.5 ulp (float32) of the real value.  Only enqueues work on
+ * cuda_stream.  Errors: INVALID_ARG (null pointer, nrows/nsamps < 1, radius < 0,
+ * 2*radius+1 > nsamps, bad width or count), UNSUPPORTED_DTYPE, OVERFLOW, CUDA. */
+dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
+                                    long long nsamps, int radius, const int *widths_host,
+                                    int nwidths, unsigned int x_max, float *z_dev,
+                                    void *cuda_stream);
+
 /* Number of kernel launches this library has issued in this process (all plans). */
 unsigned long long dedisp_get_launch_count(void);
 

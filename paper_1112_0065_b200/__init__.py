@@ -52,7 +52,9 @@ ABI = {
     "dedisp_get_last_cuda_error": (_i, [_vp]),
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
     "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
+    "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
 }
+DEDISP_MF_MAX_WIDTH = 8192
 
 _lib = None
 
@@ -193,3 +195,12 @@ def dedisp_get_last_kernel_ms(plan: int) -> tuple[float, float]:
     _check(plan, lib().dedisp_get_last_kernel_ms(plan, ctypes.byref(a), ctypes.byref(b)),
            "dedisp_get_last_kernel_ms")
     return a.value, b.value
+
+
+def dedisp_matched_filter(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: int, widths,
+                          x_max: int, z_ptr, stream: int = 0) -> None:
+    """Baseline removal + boxcar matched filters (include/dedisp.h)."""
+    w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
+    st = lib().dedisp_matched_filter(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths),
+                                     x_max, _ptr(z_ptr), stream or None)
+    _check(None, st, "dedisp_matched_filter")

@@ -30,10 +30,10 @@
 
 // ... and of the 8-bit kernel
 #ifndef BS8_NW
-#define BS8_NW 14
+#define BS8_NW 7
 #endif
 #ifndef BS8_W
-#define BS8_W 2
+#define BS8_W 4
 #endif
 #ifndef BS8_TREE_K
 #define BS8_TREE_K 2
@@ -63,7 +63,9 @@ struct Cfg {
 };
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
 using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
-// 8-bit samples: 14 x 2 words = 896-sample tiles, 8-channel trees, sums < 2^20
+// 8-bit samples: 7 x 4 words = 896-sample tiles, 8-channel trees, sums < 2^20
+// (sweep on B200, wide8: (NW,W,K,NSTAGE) = (14,2,2,3) 81.6 ms, (7,4,2,3) 75.0, (6,4,2,3) 85.8,
+//  (12,2,3,3) 91.5, (10,2,3,3) 101.9)
 using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, 64, 128>;
 }  // namespace bs
 

@@ -190,5 +190,30 @@ def random_small(seed: int, nchans: int, nsamps_in: int, nbits: int) -> np.ndarr
     return np.stack([pack2(lev[c]) for c in range(nchans)])
 
 
+def dedispersed_like(seed: int, nrows: int, nsamps: int, mean: float = 1536.0, sigma: float = 30.1,
+                     x_max: int = 3072, wiggle: float = 40.0, npulses: int = 3) -> np.ndarray:
+    """Seeded stand-in for dedispersed time series (input of the matched-filter row f1):
+    uint32 [nrows, nsamps] = Gaussian noise (mean, sigma: the HTRU-gulp output statistics)
+    + a slow baseline wiggle (two sinusoids with periods of ~nsamps/3 and ~nsamps/11, the
+    "red noise" of PAPER.md:52) + npulses boxcar pulses per row (width 1..64, height
+    3..8 sigma/sqrt(width)), rounded and clipped to [0, x_max]."""
+    out = np.empty((nrows, nsamps), dtype=np.uint32)
+    t = np.arange(nsamps, dtype=np.float64)
+    for r in range(nrows):
+        g = _rng(seed, (3 << 48) | r)
+        v = mean + sigma * g.standard_normal(nsamps)
+        ph = g.random(2) * 2 * np.pi
+        v += wiggle * np.sin(2 * np.pi * 3 * t / nsamps + ph[0]) + 0.5 * wiggle * np.sin(2 * np.pi * 11 * t / nsamps + ph[1])
+        u = g.random((npulses, 3))
+        for k in range(npulses):
+            wd = 1 + int(64 * u[k, 0])
+            if wd >= nsamps:
+                continue
+            t0 = int(u[k, 1] * (nsamps - wd))
+            v[t0:t0 + wd] += (3.0 + 5.0 * u[k, 2]) * sigma / np.sqrt(wd)
+        out[r] = np.clip(np.floor(v + 0.5), 0, x_max).astype(np.uint32)
+    return out
+
+
 def sha256(a: np.ndarray) -> str:
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
