@@ -288,6 +288,101 @@ def run_ours(args) -> None:
         dist.destroy_process_group()
 
 
+def run_matched_filter(args) -> None:
+    """--op matched_filter: row f1 on the dedispersed output of --config,
+    one GPU.  A step = one dedisp_matched_filter call over all DM trials (x resident in HBM);
+    HBM-bound: algorithmic bytes = x read once + nwidths float32 series written."""
+    import torch
+    import paper_1112_0065_b200 as dd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    torch.cuda.set_device(0)
+    w = W.CONFIGS[args.config].scaled(nbeams=1)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream()
+    plan = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+    dd.dedisp_set_dm_list(plan, list(w.dms()))
+    md = dd.dedisp_get_max_delay(plan)
+    host_in = torch.from_numpy(W.generate(w, md)).pin_memory()
+    x = torch.empty((w.ndm, w.nsamps_out), dtype=torch.int32, device=dev)
+    dd.dedisp_execute(plan, w.nsamps_out, host_in.to(dev), w.nbits, x, dd.DEDISP_OUT_U32, stream.cuda_stream)
+    dd.dedisp_destroy(plan)
+    widths = [1, 2, 4, 8, 16, 32, 64]
+    radius = min(int(round(1.0 / w.dt)), (w.nsamps_out - 1) // 2)   # 2 s window (DESIGN.md R21)
+    x_max = w.nchans * ((1 << w.nbits) - 1)
+    z = torch.empty((len(widths), w.ndm, w.nsamps_out), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        dd.dedisp_matched_filter(x, dd.DEDISP_OUT_U32, w.ndm, w.nsamps_out, radius, widths, x_max, z,
+                                 stream.cuda_stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = dd.dedisp_get_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    launches = dd.dedisp_get_launch_count() - launches0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = statistics.mean(step_ms)
+    units = w.ndm * w.nsamps_out * len(widths)
+    # end to end: host x -> device, filter, z -> host
+    hx = x.cpu().pin_memory()
+    hz = torch.empty(z.shape, dtype=torch.float32).pin_memory()
+    e2e_steps = 2
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        x.copy_(hx, non_blocking=True)
+        step()
+        hz.copy_(z, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    alg_bytes = x.numel() * 4 + z.numel() * 4
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import matched_filter as MF
+        rows = x[:: max(1, w.ndm // 48)].cpu().numpy().view(np.uint32)
+        t0 = time.perf_counter()
+        MF.matched_filter(rows, radius, widths)
+        dt = time.perf_counter() - t0
+        cpu = {"value": rows.size * len(widths) / dt, "unit": "filtered samples/s", "cores": 1, "kind": "oracle",
+               "sample": f"{rows.shape[0]} of {w.ndm} rows x {w.nsamps_out} samples x {len(widths)} widths, {dt:.2f} s"}
+    res = {"metric": "matched-filter output samples/sec", "value": units / (ms * 1e-3), "unit": "filtered samples/s",
+           "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32/int64 -> f32",
+           "data": "synthetic",
+           "config": {"workload": f"matched_filter on dedispersed {w.name}", "nrows": w.ndm,
+                      "nsamps": w.nsamps_out, "radius": radius, "widths": widths, "x_max": x_max,
+                      "l2": "256 MiB flush buffer zeroed between timed iterations"},
+           "roofline": {"bound": "hbm", "achieved": alg_bytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
+                        "traffic": ncu_traffic_bytes("matched_filter_" + w.name),
+                        "kernel": "matched_filter_kernel", "kernel_ms": ms,
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
+           "cpu_baseline": cpu,
+           "e2e": {"value": units / e2e_s, "unit": "filtered samples/s", "h2d_bytes_per_step": x.numel() * 4,
+                   "d2h_bytes_per_step": z.numel() * 4, "steps": e2e_steps},
+           "gpu_launches": launches, "clocks": clocks,
+           "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
+    print(json.dumps(res), flush=True)
+
+
 def run_reference(args) -> None:
     """The oracle, as it stands, on the host cores: the base contract's reference arm."""
     rank = int(os.environ.get("RANK", "0"))
@@ -333,10 +428,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter"],
+                    help="dedisperse = the hot path (default, the metric BASELINE.json names); "
+                         "matched_filter = row f1 downstream of it")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.op == "matched_filter":
+        run_matched_filter(args)
     else:
         run_ours(args)
 

@@ -165,7 +165,8 @@ dedisp_status dedisp_get_last_kernel_ms(dedisp_plan plan, float *prepass_ms, flo
  *   z_dev   DEVICE float32 [nwidths][nrows][nsamps] tight, written completely.
  * All sums are exact integers; each output is fl32(numerator) * fl32(1/(N sqrt(w))),
  * i.e. within 1.5 ulp (float32) of the real value.  Only enqueues work on
- * cuda_stream.  Errors: INVALID_ARG (null pointer, nrows/nsamps < 1, radius < 0,
+ * cuda_stream.  Errors: INVALID_ARG (null or misaligned pointer, nrows/nsamps < 1,
+ * nsamps > 2^30, nrows*ceil(nsamps/16384) > 2^31-1, radius < 0,
  * 2*radius+1 > nsamps, bad width or count), UNSUPPORTED_DTYPE, OVERFLOW, CUDA. */
 dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
                                     long long nsamps, int radius, const int *widths_host,

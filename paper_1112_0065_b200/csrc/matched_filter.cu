@@ -37,21 +37,12 @@ struct MFParams {
     int radius;
     int nw;
     int wmax;
-    int ring;                    // ring entries, power of two >= E + wmax + 1
+    int ring;                    // ring entries, multiple of 8, >= E + wmax + 1
     int seg;                     // samples per segment (multiple of E)
     int nseg;
     int w[MAXW];
     float scale[MAXW];           // fl32(1 / (N sqrt(w)))
 };
-
-__device__ __forceinline__ int pad(int i) { return i + (i >> 5); }
-
-template <bool XF32>
-__device__ __forceinline__ uint32_t load_x(const void *x, long long idx)
-{
-    if (XF32) return (uint32_t)__ldg(reinterpret_cast<const float *>(x) + idx);
-    return __ldg(reinterpret_cast<const uint32_t *>(x) + idx);
-}
 
 // inclusive block scan of one value per thread; returns the thread's inclusive prefix and
 // the block total.  sc: NT/32 words of shared scratch.
@@ -78,59 +69,133 @@ __device__ __forceinline__ ACC block_scan(ACC v, ACC *sc, ACC &total)
     return v + base;
 }
 
+template <bool XF32>
+__device__ __forceinline__ uint32_t cvt_x(uint32_t raw)
+{
+    return XF32 ? (uint32_t)__uint_as_float(raw) : raw;
+}
+
+// float32 of a signed accumulator; the 64-bit conversion runs on the slow XU pipe, so
+// numerators that fit 32 bits (almost all) take the fast conversion -- same rounding.
+__device__ __forceinline__ float acc_to_float(uint32_t d) { return (float)(int)d; }
+__device__ __forceinline__ float acc_to_float(unsigned long long d)
+{
+    const int l = (int)(uint32_t)d, h = (int)(uint32_t)(d >> 32);
+    if (h == (l >> 31)) return (float)l;
+    return (float)(long long)d;
+}
+
+template <class ACC> struct Vec8;
+template <> struct Vec8<uint32_t> {
+    static __device__ __forceinline__ void store(uint32_t *p, const uint32_t (&v)[V])
+    {
+        reinterpret_cast<uint4 *>(p)[0] = make_uint4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<uint4 *>(p)[1] = make_uint4(v[4], v[5], v[6], v[7]);
+    }
+};
+template <> struct Vec8<unsigned long long> {
+    static __device__ __forceinline__ void store(unsigned long long *p, const unsigned long long (&v)[V])
+    {
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            reinterpret_cast<ulonglong2 *>(p)[q] = make_ulonglong2(v[2 * q], v[2 * q + 1]);
+    }
+};
+
 template <class ACC, bool XF32>
 __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
 {
-    typedef typename std::conditional<sizeof(ACC) == 8, long long, int>::type SACC;
     extern __shared__ __align__(16) uint8_t smem_raw[];
-    uint32_t *sX = reinterpret_cast<uint32_t *>(smem_raw);          // [pad(E)]
-    uint32_t *sD = sX + (E + E / 32);                               // [pad(E)]  x[t+R] - x[t-R-1]
-    ACC *sc = reinterpret_cast<ACC *>(sD + (E + E / 32));           // [NT/32]
-    ACC *ring = sc + NT / 32;                                       // [ring + ring/32]
-    const int rmask = P.ring - 1;
+    uint32_t *sX = reinterpret_cast<uint32_t *>(smem_raw);          // [E]  x[t]
+    uint32_t *sD = sX + E;                                          // [E]  x[t+R] - x[t-R-1]
+    ACC *sc = reinterpret_cast<ACC *>(sD + E);                      // [NT/32]
+    ACC *ring = sc + NT / 32;                                       // [ring] slot i holds P[i+1]
+    const int RING = P.ring;                                        // multiple of 8, >= E + wmax + 1
 
     const long long row = blockIdx.x / P.nseg;
     const int seg = (int)(blockIdx.x % P.nseg);
     const long long n = P.n;
-    const long long R = P.radius, N = 2 * R + 1;
+    const int R = P.radius;
+    const long long N = 2ll * R + 1;
     const long long lo = (long long)seg * P.seg;
-    const long long hi = (lo + P.seg < n) ? lo + P.seg : n;
-    const long long xrow = row * n;
+    const int seglen = (int)((lo + P.seg < n) ? P.seg : n - lo);
+    const int nrem = (int)(n - lo);                  // samples from lo to the end of the row
+    const uint32_t *xr = reinterpret_cast<const uint32_t *>(P.x) + row * n + lo;   // sample lo of this row
     const int j = threadIdx.x;
 
-    // window sum of the sample before the segment: a0 = clip(lo-1-R, 0, n-N)
+    // ---- window sum of the sample before the segment: window start a0 = clip(lo-1-R, 0, n-N) ----
     long long a0 = lo - 1 - R;
     if (a0 < 0) a0 = 0;
     if (a0 > n - N) a0 = n - N;
     ACC part = 0;
-    for (long long k = j; k < N; k += NT) part += (ACC)load_x<XF32>(P.x, xrow + a0 + k);
+    {
+        const uint32_t *wb = xr + (a0 - lo);
+        int head = (int)((4 - (((uintptr_t)wb >> 2) & 3)) & 3);      // scalars up to 16-byte alignment
+        if (head > N) head = (int)N;
+        if (j < head) part += (ACC)cvt_x<XF32>(__ldg(wb + j));
+        const int nvec = (int)((N - head) >> 2);
+        const uint4 *vb = reinterpret_cast<const uint4 *>(wb + head);
+        for (int v = j; v < nvec; v += NT) {
+            const uint4 q = __ldg(vb + v);
+            part += (ACC)cvt_x<XF32>(q.x) + (ACC)cvt_x<XF32>(q.y) + (ACC)cvt_x<XF32>(q.z) +
+                    (ACC)cvt_x<XF32>(q.w);
+        }
+        const int tail = head + 4 * nvec + j;
+        if (tail < N) part += (ACC)cvt_x<XF32>(__ldg(wb + tail));
+    }
     ACC carryW;
     block_scan<ACC>(part, sc, carryW);
     ACC carryP = 0;                         // P[lo] = 0: only differences are used
-    if (j == 0) ring[pad((int)(lo & rmask))] = 0;
+    // ring slots: wslot = slot of P[lo+tb+1] (first value written this step),
+    //             rslot = slot of P[lo+tb-wmax] (first value read this step)
+    int wslot = (int)(lo % RING);
+    int rslot = wslot - 1 - P.wmax;
+    if (rslot < 0) rslot += RING;
+    if (j == 0) ring[wslot == 0 ? RING - 1 : wslot - 1] = 0;
+    // d[t] = x[t+R] - x[t-R-1] while the window slides: R+1 <= t <= n-R-1, as offsets from lo
+    const long long dlo_ll = (long long)R + 1 - lo;
+    const int dlo = dlo_ll < -(1 << 30) ? -(1 << 30) : (int)dlo_ll;
+    const int dhi = nrem - R - 1;
+    const size_t plane = (size_t)P.nrows * (size_t)n;
+    float *const zrow = P.z + (size_t)row * (size_t)n + (size_t)lo;
 
-    for (long long h = lo; h < hi + P.wmax; h += E) {
-        // ---- the three input streams, coalesced ----
+    for (int tb = 0; tb < seglen + P.wmax; tb += E) {
+        // ---- the three input streams, coalesced (the two trailing ones hit L2) ----
+        if (tb + E <= nrem && tb >= dlo && tb + E - 1 <= dhi) {
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-            const int i = j + k * NT;
-            const long long t = h + i;
-            uint32_t xt = 0, d = 0;
-            if (t < n) {
-                xt = load_x<XF32>(P.x, xrow + t);
-                if (t >= R + 1 && t <= n - R - 1)
-                    d = load_x<XF32>(P.x, xrow + t + R) - load_x<XF32>(P.x, xrow + t - R - 1);
+            for (int k = 0; k < V; ++k) {
+                const int i = j + k * NT;
+                const uint32_t *q = xr + tb + i;
+                sX[i] = cvt_x<XF32>(__ldg(q));
+                sD[i] = cvt_x<XF32>(__ldg(q + R)) - cvt_x<XF32>(__ldg(q - R - 1));
             }
-            sX[pad(i)] = xt;
-            sD[pad(i)] = d;
+        } else {
+#pragma unroll
+            for (int k = 0; k < V; ++k) {
+                const int i = j + k * NT;
+                const int o = tb + i;
+                uint32_t xt = 0, d = 0;
+                if (o < nrem) {
+                    xt = cvt_x<XF32>(__ldg(xr + o));
+                    if (o >= dlo && o <= dhi)
+                        d = cvt_x<XF32>(__ldg(xr + o + R)) - cvt_x<XF32>(__ldg(xr + o - R - 1));
+                }
+                sX[i] = xt;
+                sD[i] = d;
+            }
         }
         __syncthreads();
-        // ---- running window sum: scan of d ----
+        // ---- running window sum: scan of d (8 consecutive samples per thread) ----
+        uint32_t dv[V], xv[V];
+        *reinterpret_cast<uint4 *>(&dv[0]) = reinterpret_cast<const uint4 *>(sD + j * V)[0];
+        *reinterpret_cast<uint4 *>(&dv[4]) = reinterpret_cast<const uint4 *>(sD + j * V)[1];
+        *reinterpret_cast<uint4 *>(&xv[0]) = reinterpret_cast<const uint4 *>(sX + j * V)[0];
+        *reinterpret_cast<uint4 *>(&xv[4]) = reinterpret_cast<const uint4 *>(sX + j * V)[1];
         ACC wv[V];
         ACC run = 0;
 #pragma unroll
         for (int k = 0; k < V; ++k) {
-            run += (ACC)(SACC)(int)sD[pad(j * V + k)];   // d is a signed difference
+            run += (ACC)(long long)(int)dv[k];   // d is a signed difference
             wv[k] = run;
         }
         ACC tot;
@@ -142,9 +207,8 @@ __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
         run = 0;
 #pragma unroll
         for (int k = 0; k < V; ++k) {
-            const long long t = h + j * V + k;
-            ACC ny = (ACC)N * (ACC)sX[pad(j * V + k)] - (wbase + wv[k]);
-            if (t >= n) ny = 0;
+            ACC ny = (ACC)N * (ACC)xv[k] - (wbase + wv[k]);
+            if (tb + j * V + k >= nrem) ny = 0;
             run += ny;
             pv[k] = run;
         }
@@ -152,25 +216,59 @@ __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
         const ACC pbase = carryP + (inc - run);
         carryP += tot;
 #pragma unroll
-        for (int k = 0; k < V; ++k)   // P[t+1]
-            ring[pad((int)((h + j * V + k + 1) & rmask))] = pbase + pv[k];
+        for (int k = 0; k < V; ++k) pv[k] += pbase;
+        {
+            int ws = wslot + j * V;               // 8 consecutive slots, never across the wrap
+            if (ws >= RING) ws -= RING;
+            Vec8<ACC>::store(ring + ws, pv);
+        }
         __syncthreads();
-        // ---- outputs of the step that lags wmax behind ----
-#pragma unroll 2
+        // ---- outputs of the step that lags wmax behind: o = tb - wmax + j + k*NT ----
+        const int ob = tb - P.wmax + j;
+        int rs[V];
+        ACC p0[V];
+#pragma unroll
         for (int k = 0; k < V; ++k) {
-            const long long t = h - P.wmax + j + k * NT;
-            if (t < lo || t >= hi) continue;
-            const ACC p0 = ring[pad((int)(t & rmask))];
-            for (int iw = 0; iw < P.nw; ++iw) {
+            int sl = rslot + j + k * NT;
+            if (sl >= RING) sl -= RING;
+            rs[k] = sl;
+            p0[k] = ring[sl];
+        }
+        const bool interior = (tb - P.wmax >= 0) && (tb - P.wmax + E <= seglen) &&
+                              (tb + E - 1 <= nrem);      // every output valid, every boxcar complete
+        float *zp = zrow + ob;
+        if (interior) {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
-                float z = 0.f;
-                if (t + w <= n) {
-                    const ACC dz = ring[pad((int)((t + w) & rmask))] - p0;
-                    z = (float)(SACC)dz * P.scale[iw];
+                const float scl = P.scale[iw];
+#pragma unroll
+                for (int k = 0; k < V; ++k) {
+                    int sl = rs[k] + w;
+                    if (sl >= RING) sl -= RING;
+                    __stcs(zp + k * NT, acc_to_float((ACC)(ring[sl] - p0[k])) * scl);
                 }
-                P.z[((size_t)iw * (size_t)P.nrows + (size_t)row) * (size_t)n + (size_t)t] = z;
+            }
+        } else {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
+                const int w = P.w[iw];
+                const float scl = P.scale[iw];
+                const int lim = nrem - w;                 // t + w <= n  <=>  o <= lim
+#pragma unroll
+                for (int k = 0; k < V; ++k) {
+                    const int o = ob + k * NT;
+                    if (o >= 0 && o < seglen) {
+                        int sl = rs[k] + w;
+                        if (sl >= RING) sl -= RING;
+                        const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
+                        __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
+                    }
+                }
             }
         }
+        wslot += E;
+        if (wslot >= RING) wslot -= RING;
+        rslot += E;
+        if (rslot >= RING) rslot -= RING;
         __syncthreads();
     }
 }
@@ -185,7 +283,8 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     if (!x_dev || !z_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0)
         return DEDISP_ERR_INVALID_ARG;
     if (x_dtype != DEDISP_OUT_U32 && x_dtype != DEDISP_OUT_F32) return DEDISP_ERR_UNSUPPORTED_DTYPE;
-    if (nwidths < 1 || nwidths > MAXW) return DEDISP_ERR_INVALID_ARG;
+    if (nwidths < 1 || nwidths > MAXW || nsamps > (1ll << 30)) return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)x_dev & 3u) || ((uintptr_t)z_dev & 3u)) return DEDISP_ERR_INVALID_ARG;
     const long long N = 2ll * radius + 1;
     if (N > nsamps) return DEDISP_ERR_INVALID_ARG;
     if (x_max == 0) x_max = (1u << 24) - 1;
@@ -206,8 +305,7 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
         if (w > P.wmax) P.wmax = w;
     }
     for (int i = nwidths; i < MAXW; ++i) { P.w[i] = 1; P.scale[i] = 0.f; }
-    int ring = 1;
-    while (ring < E + P.wmax + 1) ring <<= 1;
+    const int ring = (E + P.wmax + 1 + 7) & ~7;
     P.ring = ring;
     // segments: about 8 steps each, so that the grid is many waves deep
     long long seg = 8ll * E;
@@ -221,7 +319,7 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     if (bound >= 9.0e18L) return DEDISP_ERR_OVERFLOW;
     const bool wide = bound >= 2147483648.0L;
     const size_t accb = wide ? 8 : 4;
-    const size_t smem = 2 * (size_t)(E + E / 32) * 4 + (NT / 32) * accb + (size_t)(ring + ring / 32 + 1) * accb;
+    const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (size_t)ring * accb;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
