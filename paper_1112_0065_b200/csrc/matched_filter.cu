@@ -13,7 +13,8 @@
 //   P[t+1]  = P[t] + NY[t]                               (prefix sum of NY, kept in a ring)
 //   z_w[t]  = float(P[t+w] - P[t]) * fl32(1 / (N sqrt(w)))
 // Differences of modular prefix sums are exact as long as the true value fits the
-// word, so 32-bit words serve whenever wmax*N*x_max < 2^31 and 64-bit words otherwise.
+// word, so 32-bit words serve whenever wmax*N*x_max < 2^31 (or, guarded by a per-step
+// check of the data, whenever N*x_max < 2^31) and 64-bit words otherwise.
 // A work item is (row, segment of SEG samples); a CTA walks its segment in steps of
 // E = NT*V samples: coalesced loads of the three input streams (x[t], x[t+R],
 // x[t-R-1]; the two trailing streams hit L2), two block scans, then the outputs of
@@ -40,6 +41,8 @@ struct MFParams {
     int ring;                    // ring entries, multiple of 8, >= E + wmax + 1
     int seg;                     // samples per segment (multiple of E)
     int nseg;
+    int guard_lim;               // guarded 32-bit mode: |NY| <= guard_lim => every boxcar fits int32
+    int guard_hist;              // mask of the step flags the outputs of one step depend on
     int w[MAXW];
     float scale[MAXW];           // fl32(1 / (N sqrt(w)))
 };
@@ -102,9 +105,16 @@ template <> struct Vec8<unsigned long long> {
     }
 };
 
-template <class ACC, bool XF32>
-__global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
+// GUARD (32-bit words only, host has checked N*x_max < 2^31 so that NY is exact in int32):
+// the worst-case boxcar wmax*N*x_max does not fit 32 bits, but real series stay far below
+// it.  Every step flags |NY| > (2^31-1)/wmax block-wide; outputs that depend on a flagged
+// step are summed sample by sample in 64 bits from NY[t] = P[t+1]-P[t] (exact, slow, never
+// taken on noise-like data), all others use the 32-bit differences, which are then exact.
+template <class ACC, bool XF32, bool GUARD>
+__global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
 {
+    static_assert(!GUARD || sizeof(ACC) == 4, "the guard belongs to the 32-bit path");
+    int slowbits = 0;
     extern __shared__ __align__(16) uint8_t smem_raw[];
     uint32_t *sX = reinterpret_cast<uint32_t *>(smem_raw);          // [E]  x[t]
     uint32_t *sD = sX + E;                                          // [E]  x[t+R] - x[t-R-1]
@@ -205,10 +215,12 @@ __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
         // ---- NY = N*x - Wsum and its prefix sum ----
         ACC pv[V];
         run = 0;
+        int bad = 0;
 #pragma unroll
         for (int k = 0; k < V; ++k) {
             ACC ny = (ACC)N * (ACC)xv[k] - (wbase + wv[k]);
             if (tb + j * V + k >= nrem) ny = 0;
+            if (GUARD) bad |= (abs((int)ny) > P.guard_lim);
             run += ny;
             pv[k] = run;
         }
@@ -222,7 +234,8 @@ __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
             if (ws >= RING) ws -= RING;
             Vec8<ACC>::store(ring + ws, pv);
         }
-        __syncthreads();
+        if (GUARD) slowbits = (slowbits << 1) | (__syncthreads_or(bad) ? 1 : 0);
+        else __syncthreads();
         // ---- outputs of the step that lags wmax behind: o = tb - wmax + j + k*NT ----
         const int ob = tb - P.wmax + j;
         int rs[V];
@@ -237,7 +250,31 @@ __global__ void __launch_bounds__(NT) matched_filter_kernel(const MFParams P)
         const bool interior = (tb - P.wmax >= 0) && (tb - P.wmax + E <= seglen) &&
                               (tb + E - 1 <= nrem);      // every output valid, every boxcar complete
         float *zp = zrow + ob;
-        if (interior) {
+        if (GUARD && (slowbits & P.guard_hist)) {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
+                const int w = P.w[iw];
+                const float scl = P.scale[iw];
+                const int lim = nrem - w;
+#pragma unroll 1
+                for (int k = 0; k < V; ++k) {
+                    const int o = ob + k * NT;
+                    if (o < 0 || o >= seglen) continue;
+                    long long zz = 0;
+                    if (o <= lim) {
+                        int sl = rslot + j + k * NT;      // recomputed: no dynamic register-array index
+                        if (sl >= RING) sl -= RING;
+                        uint32_t prev = (uint32_t)ring[sl];
+                        for (int q = 0; q < w; ++q) {
+                            if (++sl >= RING) sl = 0;
+                            const uint32_t cur = (uint32_t)ring[sl];
+                            zz += (long long)(int)(cur - prev);
+                            prev = cur;
+                        }
+                    }
+                    __stcs(zp + k * NT, (float)zz * scl);
+                }
+            }
+        } else if (interior) {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
@@ -317,25 +354,34 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     // |boxcar numerator| <= wmax * N * x_max must fit the signed accumulator
     const long double bound = (long double)P.wmax * (long double)N * (long double)x_max;
     if (bound >= 9.0e18L) return DEDISP_ERR_OVERFLOW;
-    const bool wide = bound >= 2147483648.0L;
+    // 32-bit words when every boxcar provably fits; guarded 32-bit words when at least NY does
+    // (N*x_max < 2^31); 64-bit words otherwise
+    const bool fits32 = bound < 2147483648.0L;
+    const bool guard = !fits32 && (long double)N * (long double)x_max < 2147483648.0L;
+    const bool wide = !fits32 && !guard;
+    P.guard_lim = (int)(2147483647ll / P.wmax);
+    P.guard_hist = (1 << ((P.wmax + E - 1) / E + 1)) - 1;
     const size_t accb = wide ? 8 : 4;
     const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (size_t)ring * accb;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
-#define MF_LAUNCH(ACC, F)                                                                        \
+#define MF_LAUNCH(ACC, F, G)                                                                     \
     do {                                                                                         \
-        e = cudaFuncSetAttribute(matched_filter_kernel<ACC, F>,                                  \
+        e = cudaFuncSetAttribute(matched_filter_kernel<ACC, F, G>,                               \
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
-        if (e == cudaSuccess) matched_filter_kernel<ACC, F><<<grid, block, smem, s>>>(P);        \
+        if (e == cudaSuccess) matched_filter_kernel<ACC, F, G><<<grid, block, smem, s>>>(P);     \
     } while (0)
     const bool f32 = (x_dtype == DEDISP_OUT_F32);
     if (wide) {
-        if (f32) MF_LAUNCH(unsigned long long, true);
-        else MF_LAUNCH(unsigned long long, false);
+        if (f32) MF_LAUNCH(unsigned long long, true, false);
+        else MF_LAUNCH(unsigned long long, false, false);
+    } else if (guard) {
+        if (f32) MF_LAUNCH(uint32_t, true, true);
+        else MF_LAUNCH(uint32_t, false, true);
     } else {
-        if (f32) MF_LAUNCH(uint32_t, true);
-        else MF_LAUNCH(uint32_t, false);
+        if (f32) MF_LAUNCH(uint32_t, true, false);
+        else MF_LAUNCH(uint32_t, false, false);
     }
 #undef MF_LAUNCH
     if (e == cudaSuccess) e = cudaGetLastError();

@@ -74,6 +74,24 @@ def test_two_second_window_htru():
     check(gpu_mf(x, 15625, widths, 3072), MF.matched_filter(x, 15625, widths))
 
 
+def test_guarded_32bit_path_spikes_force_exact_fallback():
+    """N*x_max < 2^31 <= wmax*N*x_max: the guarded 32-bit kernel.  Rows 0-1 are noise (fast
+    path); rows 2-3 carry runs of x_max over a zero floor whose boxcar numerators exceed 2^31,
+    so the flagged steps must take the exact sample-by-sample fallback."""
+    n, R = 40000, 15625
+    x = W.dedispersed_like(28, 4, n)
+    x[2:] = 0
+    x[2, 20000:20064] = 3072                    # 64 * 31251 * 3072 = 6.1e9 > 2^31
+    x[2, 36860:36870] = 3072                    # run straddling a step boundary region
+    x[3, ::4096] = 3072
+    x[3, 2040:2120] = 3072                      # across the first step boundary (E = 2048)
+    widths = [1, 2, 4, 8, 16, 32, 64]
+    want = MF.matched_filter(x, R, widths)
+    assert np.abs(want[-1, 2] * (2 * R + 1) * 8).max() > 2 ** 31      # the bound really is crossed
+    check(gpu_mf(x, R, widths, 3072), want)
+    check(gpu_mf(x, R, widths, 3072, f32_in=True), want)
+
+
 def test_edges_and_degenerate_cases():
     x = W.dedispersed_like(25, 2, 301, npulses=1)
     check(gpu_mf(x, 150, [1, 301], 3072), MF.matched_filter(x, 150, [1, 301]))   # N == n, w == n
