@@ -114,12 +114,15 @@ template <class ACC, bool XF32, bool GUARD>
 __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
 {
     static_assert(!GUARD || sizeof(ACC) == 4, "the guard belongs to the 32-bit path");
+    // 32-bit rings are stored twice (slot i and i+RING) so that reads at slot+w never wrap;
+    // 64-bit rings are not (the doubled footprint costs more occupancy than the wrap test)
+    constexpr bool MIRROR = sizeof(ACC) == 4;
     int slowbits = 0;
     extern __shared__ __align__(16) uint8_t smem_raw[];
     uint32_t *sX = reinterpret_cast<uint32_t *>(smem_raw);          // [E]  x[t]
     uint32_t *sD = sX + E;                                          // [E]  x[t+R] - x[t-R-1]
     ACC *sc = reinterpret_cast<ACC *>(sD + E);                      // [NT/32]
-    ACC *ring = sc + NT / 32;                                       // [ring] slot i holds P[i+1]
+    ACC *ring = sc + NT / 32;                                       // [2*ring] slot i (and i+ring) holds P[i+1]
     const int RING = P.ring;                                        // multiple of 8, >= E + wmax + 1
 
     const long long row = blockIdx.x / P.nseg;
@@ -161,7 +164,11 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
     int wslot = (int)(lo % RING);
     int rslot = wslot - 1 - P.wmax;
     if (rslot < 0) rslot += RING;
-    if (j == 0) ring[wslot == 0 ? RING - 1 : wslot - 1] = 0;
+    if (j == 0) {
+        const int s0 = wslot == 0 ? RING - 1 : wslot - 1;
+        ring[s0] = 0;
+        if (MIRROR) ring[s0 + RING] = 0;
+    }
     // d[t] = x[t+R] - x[t-R-1] while the window slides: R+1 <= t <= n-R-1, as offsets from lo
     const long long dlo_ll = (long long)R + 1 - lo;
     const int dlo = dlo_ll < -(1 << 30) ? -(1 << 30) : (int)dlo_ll;
@@ -233,6 +240,7 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
             int ws = wslot + j * V;               // 8 consecutive slots, never across the wrap
             if (ws >= RING) ws -= RING;
             Vec8<ACC>::store(ring + ws, pv);
+            if (MIRROR) Vec8<ACC>::store(ring + ws + RING, pv);
         }
         if (GUARD) slowbits = (slowbits << 1) | (__syncthreads_or(bad) ? 1 : 0);
         else __syncthreads();
@@ -281,7 +289,7 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     int sl = rs[k] + w;
-                    if (sl >= RING) sl -= RING;
+                    if (!MIRROR && sl >= RING) sl -= RING;
                     __stcs(zp + k * NT, acc_to_float((ACC)(ring[sl] - p0[k])) * scl);
                 }
             }
@@ -295,7 +303,7 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
                     const int o = ob + k * NT;
                     if (o >= 0 && o < seglen) {
                         int sl = rs[k] + w;
-                        if (sl >= RING) sl -= RING;
+                        if (!MIRROR && sl >= RING) sl -= RING;
                         const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
                         __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
                     }
@@ -362,7 +370,7 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     P.guard_lim = (int)(2147483647ll / P.wmax);
     P.guard_hist = (1 << ((P.wmax + E - 1) / E + 1)) - 1;
     const size_t accb = wide ? 8 : 4;
-    const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (size_t)ring * accb;
+    const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (wide ? 1 : 2) * (size_t)ring * accb;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
