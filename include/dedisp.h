@@ -173,6 +173,50 @@ dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
                                     int nwidths, unsigned int x_max, float *z_dev,
                                     void *cuda_stream);
 
+/* ---- peak finding ---- */
+
+/* One detected event: a maximal run of consecutive samples of one series above threshold. */
+typedef struct {
+    int series;   /* row of z the run lies in */
+    int t_start;  /* first sample of the run */
+    int length;   /* samples in the run */
+    int t_peak;   /* FIRST position of the maximum of z over the run */
+    float peak;   /* that maximum */
+} dedisp_event;
+
+/* Bytes of device scratch dedisp_find_events needs for this shape (0 = shape rejected):
+ * a bit mask of the sigma-cut (1 bit per sample) plus per-chunk and per-series counters. */
+size_t dedisp_find_events_workspace_bytes(long long nseries, long long nsamps);
+
+/* Sigma-cut, then contiguous regions gathered into events (Sec. 2.3 "first
+ * performing a sigma-cut and then gathering contiguous regions together into individual
+ * events ... 'transform' and 'reduce_by_key'"):
+ *     above[s][t] = z[s][t] > nsigma * sigma[s]      (float32 product, strict >; NaN is never above)
+ *     event       = maximal run of consecutive t with above[s][t], series by series
+ *   z_dev      DEVICE float32 [nseries][nsamps] tight (e.g. the output of dedisp_matched_filter
+ *              viewed as nwidths*nrows series); 4-byte aligned.
+ *   sigma_dev  DEVICE float32 [nseries]: noise level of each series (dedisp_series_rms offers
+ *              an estimate; the paper names none).
+ *   workspace_dev  DEVICE scratch, 8-byte aligned, >= dedisp_find_events_workspace_bytes();
+ *              owned by the caller, free to reuse after the call's work has completed.
+ *   events_dev DEVICE array of max_events records (may be NULL when max_events = 0), written
+ *              in ascending (series, t_start) order; events beyond max_events are dropped.
+ *   count_dev  DEVICE long long, 8-byte aligned: total number of events found (may exceed
+ *              max_events).
+ * Only enqueues work on cuda_stream (4 kernels; z is read once, plus the samples inside runs).
+ * Errors: INVALID_ARG (null/misaligned pointer, nseries/nsamps < 1, nsamps > 2^30,
+ * nseries > 2^31-1, workspace too small, max_events < 0), CUDA. */
+dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long long nsamps,
+                                 const float *sigma_dev, float nsigma, void *workspace_dev,
+                                 size_t workspace_bytes, dedisp_event *events_dev,
+                                 long long max_events, long long *count_dev, void *cuda_stream);
+
+/* rms_dev[s] = float32( sqrt( (1/nsamps) * sum_t z[s][t]^2 ) ), accumulated in float64: the
+ * noise estimate of a baseline-removed (zero-mean) series, offered as sigma for the
+ * sigma-cut (the paper does not say how sigma is obtained).  DEVICE pointers, 4-byte aligned. */
+dedisp_status dedisp_series_rms(const float *z_dev, long long nseries, long long nsamps,
+                                float *rms_dev, void *cuda_stream);
+
 /* Number of kernel launches this library has issued in this process (all plans). */
 unsigned long long dedisp_get_launch_count(void);
 

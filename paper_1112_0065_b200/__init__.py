@@ -53,8 +53,12 @@ ABI = {
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
     "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
     "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
+    "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
+    "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
+    "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
 }
 DEDISP_MF_MAX_WIDTH = 8192
+DEDISP_EVENT_BYTES = 20      # struct dedisp_event {int series, t_start, length, t_peak; float peak;}
 
 _lib = None
 
@@ -204,3 +208,23 @@ def dedisp_matched_filter(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: 
     st = lib().dedisp_matched_filter(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths),
                                      x_max, _ptr(z_ptr), stream or None)
     _check(None, st, "dedisp_matched_filter")
+
+
+def dedisp_find_events_workspace_bytes(nseries: int, nsamps: int) -> int:
+    return int(lib().dedisp_find_events_workspace_bytes(nseries, nsamps))
+
+
+def dedisp_find_events(z_ptr, nseries: int, nsamps: int, sigma_ptr, nsigma: float, workspace_ptr,
+                       workspace_bytes: int, events_ptr, max_events: int, count_ptr,
+                       stream: int = 0) -> None:
+    """Sigma-cut + grouping of contiguous regions into events (include/dedisp.h)."""
+    st = lib().dedisp_find_events(_ptr(z_ptr), nseries, nsamps, _ptr(sigma_ptr), nsigma,
+                                  _ptr(workspace_ptr), workspace_bytes,
+                                  _ptr(events_ptr) if events_ptr is not None else None, max_events,
+                                  _ptr(count_ptr), stream or None)
+    _check(None, st, "dedisp_find_events")
+
+
+def dedisp_series_rms(z_ptr, nseries: int, nsamps: int, rms_ptr, stream: int = 0) -> None:
+    _check(None, lib().dedisp_series_rms(_ptr(z_ptr), nseries, nsamps, _ptr(rms_ptr), stream or None),
+           "dedisp_series_rms")

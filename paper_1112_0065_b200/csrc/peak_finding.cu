@@ -1,0 +1,312 @@
+// peak_finding.cu -- sigma-cut + grouping of contiguous regions into events
+// (Sec. 2.3: "first performing a sigma-cut and
+// then gathering contiguous regions together into individual events ... 'transform' and
+// 'reduce_by_key'"), and the per-series RMS offered as the sigma estimate.
+//
+//   m[s][t] = z[s][t] > nsigma * sigma[s]          (float32 product, strict >, NaN never above)
+//   event   = maximal run of consecutive t of one series with m true
+//           -> (series, t_start, length, t_peak = first position of the maximum, peak)
+//   events listed in ascending (series, t_start) order, at most max_events of them.
+//
+// B200 design: z (the large array) is read ONCE, coalesced, by the transform kernel, which
+// leaves a bit mask (1 bit per sample: 3 % of the bytes) and the number of run starts per
+// 1024-sample chunk.  Two small scans turn the counts into output offsets, so the list
+// comes out sorted and deterministic without atomics or a sort.  The grouping kernel then
+// works on the bit mask only and re-reads z just inside the runs (sparse).
+#include "dedisp_internal.h"
+
+namespace {
+
+constexpr int CHUNK_WORDS = 32;                  // one warp: 32 mask words
+constexpr int CHUNK = CHUNK_WORDS * 32;          // = 1024 samples per chunk
+constexpr int WARPS = 8;                         // chunks per CTA in the transform kernel
+
+struct PFLayout {
+    long long nwords;        // mask words per series (multiple of CHUNK_WORDS)
+    long long nchunks;       // chunks per series
+    size_t off_counts, off_chunk_off, off_series_tot, off_series_base, total;
+};
+
+PFLayout make_layout(long long nseries, long long nsamps)
+{
+    PFLayout L;
+    L.nchunks = (nsamps + CHUNK - 1) / CHUNK;
+    L.nwords = L.nchunks * CHUNK_WORDS;
+    size_t o = (size_t)nseries * (size_t)L.nwords * 4;          // mask
+    L.off_counts = o;
+    o += (size_t)nseries * (size_t)L.nchunks * 4;
+    L.off_chunk_off = o;
+    o += (size_t)nseries * (size_t)L.nchunks * 4;
+    L.off_series_tot = o;
+    o += (size_t)nseries * 4;
+    o = (o + 7) & ~(size_t)7;
+    L.off_series_base = o;
+    o += (size_t)nseries * 8;
+    L.total = o;
+    return L;
+}
+
+// run starts of a mask word: set bits whose predecessor (previous bit, or the top bit of the
+// previous word for bit 0) is clear
+__device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
+{
+    return m & ~((m << 1) | (prev_word >> 31));
+}
+
+// ---- transform: one warp per (series, chunk) ----
+__global__ void __launch_bounds__(WARPS * 32)
+sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+                 const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
+                 uint32_t *__restrict__ counts)
+{
+    const int lane = threadIdx.x & 31;
+    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (item >= nseries * nchunks) return;
+    const long long s = item / nchunks, c = item % nchunks;
+    const float thr = __fmul_rn(nsigma, __ldg(sigma + s));
+    const float *zr = z + s * n;
+    const long long t0 = c * CHUNK;
+    uint32_t mine = 0;
+    if (t0 + CHUNK <= n) {
+#pragma unroll 8
+        for (int w = 0; w < CHUNK_WORDS; ++w) {
+            const uint32_t b = __ballot_sync(0xffffffffu, __ldcs(zr + t0 + w * 32 + lane) > thr);
+            if (lane == w) mine = b;
+        }
+    } else {
+        for (int w = 0; w < CHUNK_WORDS; ++w) {
+            const long long t = t0 + w * 32 + lane;
+            const uint32_t b = __ballot_sync(0xffffffffu, t < n && __ldcs(zr + t) > thr);
+            if (lane == w) mine = b;
+        }
+    }
+    // top bit of the word before: previous lane, or the sample before the chunk
+    uint32_t prev = __shfl_up_sync(0xffffffffu, mine, 1);
+    if (lane == 0) prev = (t0 > 0 && __ldg(zr + t0 - 1) > thr) ? 0x80000000u : 0u;
+    int cnt = __popc(run_starts(mine, prev));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    mask[(s * nchunks + c) * CHUNK_WORDS + lane] = mine;
+    if (lane == 0) counts[s * nchunks + c] = (uint32_t)cnt;
+}
+
+// ---- scan 1: one warp per series: exclusive offsets of its chunks + series total ----
+__global__ void __launch_bounds__(256)
+chunk_scan_kernel(const uint32_t *__restrict__ counts, long long nseries, long long nchunks,
+                  uint32_t *__restrict__ chunk_off, uint32_t *__restrict__ series_tot)
+{
+    const int lane = threadIdx.x & 31;
+    const long long s = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (s >= nseries) return;
+    uint32_t carry = 0;
+    for (long long c0 = 0; c0 < nchunks; c0 += 32) {
+        const long long c = c0 + lane;
+        const uint32_t v = c < nchunks ? counts[s * nchunks + c] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (c < nchunks) chunk_off[s * nchunks + c] = carry + inc - v;
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) series_tot[s] = carry;
+}
+
+// ---- scan 2: one CTA: exclusive 64-bit offsets of the series + grand total ----
+__global__ void __launch_bounds__(1024)
+series_scan_kernel(const uint32_t *__restrict__ series_tot, long long nseries,
+                   unsigned long long *__restrict__ series_base, long long *__restrict__ count_out)
+{
+    __shared__ unsigned long long sc[32];
+    __shared__ unsigned long long carry_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (long long s0 = 0; s0 < nseries; s0 += 1024) {
+        const long long s = s0 + threadIdx.x;
+        const unsigned long long v = s < nseries ? series_tot[s] : 0ull;
+        unsigned long long inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) sc[warp] = inc;
+        __syncthreads();
+        unsigned long long base = carry_s, tot = 0;
+        for (int k = 0; k < 32; ++k) {
+            if (k < warp) base += sc[k];
+            tot += sc[k];
+        }
+        if (s < nseries) series_base[s] = base + inc - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *count_out = (long long)carry_s;
+}
+
+// ---- reduce by key: one warp per (series, chunk), lane = mask word ----
+__global__ void __launch_bounds__(WARPS * 32)
+group_events_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+                    const uint32_t *__restrict__ mask, const uint32_t *__restrict__ chunk_off,
+                    const unsigned long long *__restrict__ series_base,
+                    dedisp_event *__restrict__ events, long long max_events)
+{
+    const int lane = threadIdx.x & 31;
+    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (item >= nseries * nchunks) return;
+    const long long s = item / nchunks, c = item % nchunks;
+    const long long nwords = nchunks * CHUNK_WORDS;
+    const uint32_t *mrow = mask + s * nwords;
+    const long long wi = c * CHUNK_WORDS + lane;
+    const uint32_t m = mrow[wi];
+    uint32_t prev = __shfl_up_sync(0xffffffffu, m, 1);
+    if (lane == 0) prev = c > 0 ? mrow[wi - 1] : 0u;
+    uint32_t st = run_starts(m, prev);
+    if (__ballot_sync(0xffffffffu, st != 0) == 0) return;     // nothing starts in this chunk
+    const int cnt = __popc(st);
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+    }
+    unsigned long long slot = series_base[s] + chunk_off[s * nchunks + c] + (unsigned)(inc - cnt);
+    const float *zr = z + s * n;
+    while (st) {
+        const int b = __ffs(st) - 1;
+        st &= st - 1;
+        const long long t_start = wi * 32 + b;
+        // length of the run of ones from bit b; it may continue through the next words
+        const uint32_t inv = ~(m >> b);
+        long long len = inv ? __ffs(inv) - 1 : 32;
+        if (len >= 32 - b) {
+            len = 32 - b;
+            for (long long w2 = wi + 1; w2 < nwords; ++w2) {
+                const uint32_t mw = mrow[w2];
+                if (mw == 0xffffffffu) {
+                    len += 32;
+                    continue;
+                }
+                len += __ffs(~mw) - 1;
+                break;
+            }
+        }
+        if ((long long)slot < max_events) {
+            float peak = zr[t_start];
+            long long tp = t_start;
+            for (long long t = t_start + 1; t < t_start + len; ++t) {
+                const float v = zr[t];
+                if (v > peak) {
+                    peak = v;
+                    tp = t;
+                }
+            }
+            dedisp_event e;
+            e.series = (int)s;
+            e.t_start = (int)t_start;
+            e.length = (int)len;
+            e.t_peak = (int)tp;
+            e.peak = peak;
+            events[slot] = e;
+        }
+        ++slot;
+    }
+}
+
+// ---- sigma estimate: sqrt(mean z^2) per series, float64 accumulation in a fixed order ----
+__global__ void __launch_bounds__(256)
+series_rms_kernel(const float *__restrict__ z, long long n, float *__restrict__ rms)
+{
+    __shared__ double sc[8];
+    const float *zr = z + (long long)blockIdx.x * n;
+    double acc = 0.0;
+    const bool vec = (((uintptr_t)zr & 15u) == 0);
+    const long long nv = vec ? (n >> 2) : 0;
+    const float4 *z4 = reinterpret_cast<const float4 *>(zr);
+    for (long long i = threadIdx.x; i < nv; i += 256) {
+        const float4 q = __ldcs(z4 + i);
+        acc += (double)q.x * (double)q.x + (double)q.y * (double)q.y + (double)q.z * (double)q.z +
+               (double)q.w * (double)q.w;
+    }
+    for (long long i = 4 * nv + threadIdx.x; i < n; i += 256) {
+        const double v = (double)__ldcs(zr + i);
+        acc += v * v;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sc[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < 8; ++k) t += sc[k];
+        rms[blockIdx.x] = (float)sqrt(t / (double)n);
+    }
+}
+
+bool pf_sizes_ok(long long nseries, long long nsamps)
+{
+    if (nseries < 1 || nsamps < 1 || nsamps > (1ll << 30) || nseries > 0x7fffffffll) return false;
+    const long long nchunks = (nsamps + CHUNK - 1) / CHUNK;
+    return nseries * nchunks <= 0x7fffffffll * (long long)WARPS / 2;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t dedisp_find_events_workspace_bytes(long long nseries, long long nsamps)
+{
+    if (!pf_sizes_ok(nseries, nsamps)) return 0;
+    return make_layout(nseries, nsamps).total;
+}
+
+dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long long nsamps,
+                                 const float *sigma_dev, float nsigma, void *workspace_dev,
+                                 size_t workspace_bytes, dedisp_event *events_dev,
+                                 long long max_events, long long *count_dev, void *cuda_stream)
+{
+    if (!z_dev || !sigma_dev || !workspace_dev || !count_dev || max_events < 0 ||
+        (max_events > 0 && !events_dev))
+        return DEDISP_ERR_INVALID_ARG;
+    if (!pf_sizes_ok(nseries, nsamps)) return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)z_dev & 3u) || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)events_dev & 3u) ||
+        ((uintptr_t)count_dev & 7u))
+        return DEDISP_ERR_INVALID_ARG;
+    const PFLayout L = make_layout(nseries, nsamps);
+    if (workspace_bytes < L.total) return DEDISP_ERR_INVALID_ARG;
+    uint8_t *ws = (uint8_t *)workspace_dev;
+    uint32_t *mask = (uint32_t *)ws;
+    uint32_t *counts = (uint32_t *)(ws + L.off_counts);
+    uint32_t *chunk_off = (uint32_t *)(ws + L.off_chunk_off);
+    uint32_t *series_tot = (uint32_t *)(ws + L.off_series_tot);
+    unsigned long long *series_base = (unsigned long long *)(ws + L.off_series_base);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const long long items = nseries * L.nchunks;
+    const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
+    sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
+                                                 mask, counts);
+    chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
+                                                                    chunk_off, series_tot);
+    series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
+    group_events_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, mask, chunk_off,
+                                                    series_base, events_dev, max_events);
+    g_launch_count += 4;
+    return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
+}
+
+dedisp_status dedisp_series_rms(const float *z_dev, long long nseries, long long nsamps,
+                                float *rms_dev, void *cuda_stream)
+{
+    if (!z_dev || !rms_dev || nseries < 1 || nsamps < 1 || nseries > 0x7fffffffll)
+        return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)z_dev & 3u) || ((uintptr_t)rms_dev & 3u)) return DEDISP_ERR_INVALID_ARG;
+    series_rms_kernel<<<(unsigned)nseries, 256, 0, (cudaStream_t)cuda_stream>>>(z_dev, nsamps, rms_dev);
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
+}
+
+}  // extern "C"

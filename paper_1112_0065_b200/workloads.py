@@ -215,5 +215,24 @@ def dedispersed_like(seed: int, nrows: int, nsamps: int, mean: float = 1536.0, s
     return out
 
 
+def filtered_like(seed: int, nseries: int, nsamps: int, sigma: float = 30.1, npulses: int = 4,
+                  max_width: int = 3000) -> np.ndarray:
+    """Seeded stand-in for matched-filter output (input of the peak-finding row f2):
+    float32 [nseries, nsamps] = zero-mean Gaussian noise of the given sigma + npulses flat-topped
+    pulses per series (width 1..max_width, log-uniform, so that runs cross 32-sample words and
+    1024-sample chunks; height 6..12 sigma with a small seeded ripple so maxima are unique)."""
+    out = np.empty((nseries, nsamps), dtype=np.float32)
+    for r in range(nseries):
+        g = _rng(seed, (5 << 48) | r)
+        v = sigma * g.standard_normal(nsamps)
+        u = g.random((npulses, 3))
+        for k in range(npulses):
+            wd = min(nsamps, int(np.exp(u[k, 0] * np.log(max_width))))
+            t0 = int(u[k, 1] * (nsamps - wd + 1))
+            v[t0:t0 + wd] += (6.0 + 6.0 * u[k, 2]) * sigma
+        out[r] = v.astype(np.float32)
+    return out
+
+
 def sha256(a: np.ndarray) -> str:
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
