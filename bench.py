@@ -320,6 +320,8 @@ def run_matched_filter(args) -> None:
         dd.dedisp_matched_filter(x, dd.DEDISP_OUT_U32, w.ndm, w.nsamps_out, radius, widths, x_max, z,
                                  stream.cuda_stream)
 
+    if args.op == "find_events":
+        return _bench_find_events(args, dd, torch, w, widths, z, step, flush, stream)
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -383,6 +385,87 @@ def run_matched_filter(args) -> None:
     print(json.dumps(res), flush=True)
 
 
+def _bench_find_events(args, dd, torch, w, widths, z, make_z, flush, stream) -> None:
+    """--op find_events: row f2 on the matched-filter output of --config.  A step =
+    dedisp_series_rms (the sigma estimate) + dedisp_find_events at 6 sigma over all
+    nwidths*ndm filtered series; HBM-bound: z is read twice (once per call), the bit mask
+    (1/32 of z) is written and read once."""
+    make_z()
+    dev = z.device
+    ns, n = z.shape[0] * z.shape[1], z.shape[2]
+    nsigma, cap = 6.0, 1 << 20
+    wsb = dd.dedisp_find_events_workspace_bytes(ns, n)
+    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+    rms = torch.empty(ns, dtype=torch.float32, device=dev)
+    ev = torch.empty((cap, 5), dtype=torch.int32, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def step():
+        dd.dedisp_series_rms(z, ns, n, rms, stream.cuda_stream)
+        dd.dedisp_find_events(z, ns, n, rms, nsigma, ws, wsb, ev, cap, cnt, stream.cuda_stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = dd.dedisp_get_launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(args.steps)]
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    launches = dd.dedisp_get_launch_count() - launches0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    ms = statistics.mean(step_ms)
+    found = int(cnt.item())
+    # end to end: z from pinned host memory, events + count back to the host
+    hz = z.cpu().pin_memory()
+    hev = torch.empty((cap, 5), dtype=torch.int32).pin_memory()
+    t0 = time.perf_counter()
+    z.copy_(hz, non_blocking=True)
+    step()
+    k = min(int(cnt.item()), cap)
+    hev[:k].copy_(ev[:k], non_blocking=True)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    alg_bytes = 2 * z.numel() * 4 + 2 * (z.numel() // 8)
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import peak_finding as PF
+        rows = z.reshape(ns, n)[:: max(1, ns // 48)].cpu().numpy()
+        t0 = time.perf_counter()
+        PF.find_events(rows, PF.series_rms(rows).astype(np.float32), nsigma)
+        dt = time.perf_counter() - t0
+        cpu = {"value": rows.size / dt, "unit": "searched samples/s", "cores": 1, "kind": "oracle",
+               "sample": f"{rows.shape[0]} of {ns} series x {n} samples (rms + find_events), {dt:.2f} s"}
+    res = {"metric": "peak-finding input samples/sec", "value": ns * n / (ms * 1e-3), "unit": "searched samples/s",
+           "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 compare / f64 sum",
+           "data": "synthetic",
+           "config": {"workload": f"series_rms + find_events on matched-filtered {w.name}", "nseries": ns,
+                      "nsamps": n, "nsigma": nsigma, "events_found": found, "widths": widths,
+                      "l2": "256 MiB flush buffer zeroed between timed iterations"},
+           "roofline": {"bound": "hbm", "achieved": alg_bytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
+                        "traffic": ncu_traffic_bytes("find_events_" + w.name),
+                        "kernel": "series_rms_kernel + sigma_cut_kernel (+ 3 small kernels)", "kernel_ms": ms,
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
+           "cpu_baseline": cpu,
+           "e2e": {"value": ns * n / e2e_s, "unit": "searched samples/s", "h2d_bytes_per_step": z.numel() * 4,
+                   "d2h_bytes_per_step": k * 20 + 8, "steps": 1},
+           "gpu_launches": launches, "clocks": clocks,
+           "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
+    print(json.dumps(res), flush=True)
+
+
 def run_reference(args) -> None:
     """The oracle, as it stands, on the host cores: the base contract's reference arm."""
     rank = int(os.environ.get("RANK", "0"))
@@ -428,14 +511,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter"],
+    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events"],
                     help="dedisperse = the hot path (default, the metric BASELINE.json names); "
-                         "matched_filter = row f1 downstream of it")
+                         "matched_filter = row f1 downstream of it; find_events = row f2 downstream of f1")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
-    elif args.op == "matched_filter":
+    elif args.op in ("matched_filter", "find_events"):
         run_matched_filter(args)
     else:
         run_ours(args)

@@ -57,7 +57,7 @@ __device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
 __global__ void __launch_bounds__(WARPS * 32)
 sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
                  const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
-                 uint32_t *__restrict__ counts)
+                 uint32_t *__restrict__ counts, int vec_ok)
 {
     const int lane = threadIdx.x & 31;
     const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
@@ -67,7 +67,24 @@ sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, lo
     const float *zr = z + s * n;
     const long long t0 = c * CHUNK;
     uint32_t mine = 0;
-    if (t0 + CHUNK <= n) {
+    if (vec_ok && t0 + CHUNK <= n) {
+        // 128-bit loads: lane l of pass i holds samples 128 i + 4 l .. + 3 -> a nibble of word
+        // 4 i + l/8; three OR-shuffles assemble the word in its 8-lane group, one more hands word
+        // L to lane L
+        const float4 *z4 = reinterpret_cast<const float4 *>(zr + t0);
+#pragma unroll
+        for (int i = 0; i < CHUNK / 128; ++i) {
+            const float4 q = __ldcs(z4 + i * 32 + lane);
+            uint32_t v = (q.x > thr ? 1u : 0u) | (q.y > thr ? 2u : 0u) | (q.z > thr ? 4u : 0u) |
+                         (q.w > thr ? 8u : 0u);
+            v <<= 4 * (lane & 7);
+            v |= __shfl_xor_sync(0xffffffffu, v, 1);
+            v |= __shfl_xor_sync(0xffffffffu, v, 2);
+            v |= __shfl_xor_sync(0xffffffffu, v, 4);
+            v = __shfl_sync(0xffffffffu, v, 8 * (lane & 3));
+            if ((lane >> 2) == i) mine = v;
+        }
+    } else if (t0 + CHUNK <= n) {
 #pragma unroll 8
         for (int w = 0; w < CHUNK_WORDS; ++w) {
             const uint32_t b = __ballot_sync(0xffffffffu, __ldcs(zr + t0 + w * 32 + lane) > thr);
@@ -114,50 +131,49 @@ chunk_scan_kernel(const uint32_t *__restrict__ counts, long long nseries, long l
     if (lane == 0) series_tot[s] = carry;
 }
 
-// ---- scan 2: one CTA: exclusive 64-bit offsets of the series + grand total ----
+// ---- scan 2: one CTA: exclusive 64-bit offsets of the series + grand total; each thread owns
+// a run of consecutive series, one block scan in between ----
 __global__ void __launch_bounds__(1024)
 series_scan_kernel(const uint32_t *__restrict__ series_tot, long long nseries,
                    unsigned long long *__restrict__ series_base, long long *__restrict__ count_out)
 {
     __shared__ unsigned long long sc[32];
-    __shared__ unsigned long long carry_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (long long s0 = 0; s0 < nseries; s0 += 1024) {
-        const long long s = s0 + threadIdx.x;
-        const unsigned long long v = s < nseries ? series_tot[s] : 0ull;
-        unsigned long long inc = v;
+    const long long per = (nseries + 1023) / 1024;
+    const long long s0 = (long long)threadIdx.x * per;
+    const long long s1 = s0 + per < nseries ? s0 + per : nseries;
+    unsigned long long v = 0;
+    for (long long q = s0; q < s1; ++q) v += series_tot[q];
+    unsigned long long inc = v;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const unsigned long long u = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += u;
-        }
-        if (lane == 31) sc[warp] = inc;
-        __syncthreads();
-        unsigned long long base = carry_s, tot = 0;
-        for (int k = 0; k < 32; ++k) {
-            if (k < warp) base += sc[k];
-            tot += sc[k];
-        }
-        if (s < nseries) series_base[s] = base + inc - v;
-        __syncthreads();
-        if (threadIdx.x == 0) carry_s += tot;
-        __syncthreads();
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
     }
-    if (threadIdx.x == 0) *count_out = (long long)carry_s;
+    if (lane == 31) sc[warp] = inc;
+    __syncthreads();
+    unsigned long long base = 0, tot = 0;
+    for (int k = 0; k < 32; ++k) {
+        if (k < warp) base += sc[k];
+        tot += sc[k];
+    }
+    unsigned long long run = base + inc - v;
+    for (long long q = s0; q < s1; ++q) {
+        series_base[q] = run;
+        run += series_tot[q];
+    }
+    if (threadIdx.x == 0) *count_out = (long long)tot;
 }
 
-// ---- reduce by key: one warp per (series, chunk), lane = mask word ----
-__global__ void __launch_bounds__(WARPS * 32)
-group_events_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
-                    const uint32_t *__restrict__ mask, const uint32_t *__restrict__ chunk_off,
-                    const unsigned long long *__restrict__ series_base,
-                    dedisp_event *__restrict__ events, long long max_events)
+// ---- reduce by key: a warp takes 32 (series, chunk) items at a time, skips those in which no
+// run starts (their count is 0) and handles the others one by one, lane = mask word ----
+__device__ __forceinline__ void group_chunk(const float *__restrict__ z, long long n, long long nchunks,
+                                            const uint32_t *__restrict__ mask,
+                                            const uint32_t *__restrict__ chunk_off,
+                                            const unsigned long long *__restrict__ series_base,
+                                            dedisp_event *__restrict__ events, long long max_events,
+                                            long long item, int lane)
 {
-    const int lane = threadIdx.x & 31;
-    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    if (item >= nseries * nchunks) return;
     const long long s = item / nchunks, c = item % nchunks;
     const long long nwords = nchunks * CHUNK_WORDS;
     const uint32_t *mrow = mask + s * nwords;
@@ -166,7 +182,6 @@ group_events_kernel(const float *__restrict__ z, long long nseries, long long n,
     uint32_t prev = __shfl_up_sync(0xffffffffu, m, 1);
     if (lane == 0) prev = c > 0 ? mrow[wi - 1] : 0u;
     uint32_t st = run_starts(m, prev);
-    if (__ballot_sync(0xffffffffu, st != 0) == 0) return;     // nothing starts in this chunk
     const int cnt = __popc(st);
     int inc = cnt;
 #pragma unroll
@@ -214,6 +229,28 @@ group_events_kernel(const float *__restrict__ z, long long nseries, long long n,
             events[slot] = e;
         }
         ++slot;
+    }
+}
+
+__global__ void __launch_bounds__(WARPS * 32)
+group_events_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+                    const uint32_t *__restrict__ mask, const uint32_t *__restrict__ counts,
+                    const uint32_t *__restrict__ chunk_off,
+                    const unsigned long long *__restrict__ series_base,
+                    dedisp_event *__restrict__ events, long long max_events)
+{
+    const int lane = threadIdx.x & 31;
+    const long long nitems = nseries * nchunks;
+    const long long stride = (long long)gridDim.x * WARPS * 32;
+    for (long long base = ((long long)blockIdx.x * WARPS + (threadIdx.x >> 5)) * 32; base < nitems;
+         base += stride) {
+        const long long it = base + lane;
+        uint32_t has = __ballot_sync(0xffffffffu, it < nitems && counts[it] != 0u);
+        while (has) {
+            const int src = __ffs(has) - 1;
+            has &= has - 1;
+            group_chunk(z, n, nchunks, mask, chunk_off, series_base, events, max_events, base + src, lane);
+        }
     }
 }
 
@@ -287,13 +324,18 @@ dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long lon
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const long long items = nseries * L.nchunks;
     const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
+    const int vec_ok = (((uintptr_t)z_dev & 15u) == 0) && (nsamps % 4 == 0);
     sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
-                                                 mask, counts);
+                                                 mask, counts, vec_ok);
     chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
                                                                     chunk_off, series_tot);
     series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
-    group_events_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, mask, chunk_off,
-                                                    series_base, events_dev, max_events);
+    int sms = 148, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long gwant = (items + WARPS * 32 - 1) / (WARPS * 32);
+    const unsigned ggrid = (unsigned)(gwant < 8ll * sms ? gwant : 8ll * sms);
+    group_events_kernel<<<ggrid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, mask, counts,
+                                                     chunk_off, series_base, events_dev, max_events);
     g_launch_count += 4;
     return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
 }
