@@ -217,6 +217,27 @@ dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long lon
 dedisp_status dedisp_series_rms(const float *z_dev, long long nseries, long long nsamps,
                                 float *rms_dev, void *cuda_stream);
 
+/* ---- multibeam coincidence RFI mask ---- */
+
+/* PAPER.md:38-40 Sec. 2.1: "a signal exceeding 3 sigma in 4 or more beams ... a transform of the
+ * multibeam time series, where for each sample the 13 beams are checked against the thresholds
+ * and the result is written as a boolean RFI mask":
+ *     above[b][s][t] = x[b][s][t] > fl32( mean[b][s] + fl32( nsigma * sigma[b][s] ) )
+ *     mask[s][t]     = ( number of beams b with above[b][s][t] ) >= min_beams      (1 or 0)
+ *   x_dev     DEVICE, nbeams blocks of [nseries][nsamps] (tight inside a beam), beam b at
+ *             x_dev + b*beam_stride_bytes (a multiple of 4, >= nseries*nsamps*4); uint32 or float32
+ *             holding values < 2^24 (uint32) -- e.g. the DM-0 trial of every beam of a batched
+ *             dedisp_execute_batch output: nseries = 1, beam_stride_bytes = ndm*nsamps*4.
+ *   mean_dev, sigma_dev  DEVICE float32 [nbeams][nseries]: level and noise of every series (the
+ *             paper leaves their estimate open).
+ *   mask_dev  DEVICE uint8 [nseries][nsamps], written completely.
+ * Strict >, thresholds formed in float32, NaN never above.  nseries <= 65535.  Only enqueues
+ * work on cuda_stream.  Errors: INVALID_ARG, UNSUPPORTED_DTYPE, CUDA. */
+dedisp_status dedisp_rfi_mask(const void *x_dev, dedisp_out_dtype x_dtype, int nbeams,
+                              long long nseries, long long nsamps, size_t beam_stride_bytes,
+                              const float *mean_dev, const float *sigma_dev, float nsigma,
+                              int min_beams, unsigned char *mask_dev, void *cuda_stream);
+
 /* Number of kernel launches this library has issued in this process (all plans). */
 unsigned long long dedisp_get_launch_count(void);
 

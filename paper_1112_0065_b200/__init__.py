@@ -56,6 +56,7 @@ ABI = {
     "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
     "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
+    "dedisp_rfi_mask": (_i, [_vp, _i, _i, _ll, _ll, _sz, _vp, _vp, ctypes.c_float, _i, _vp, _vp]),
 }
 DEDISP_MF_MAX_WIDTH = 8192
 DEDISP_EVENT_BYTES = 20      # struct dedisp_event {int series, t_start, length, t_peak; float peak;}
@@ -228,3 +229,12 @@ def dedisp_find_events(z_ptr, nseries: int, nsamps: int, sigma_ptr, nsigma: floa
 def dedisp_series_rms(z_ptr, nseries: int, nsamps: int, rms_ptr, stream: int = 0) -> None:
     _check(None, lib().dedisp_series_rms(_ptr(z_ptr), nseries, nsamps, _ptr(rms_ptr), stream or None),
            "dedisp_series_rms")
+
+
+def dedisp_rfi_mask(x_ptr, x_dtype: int, nbeams: int, nseries: int, nsamps: int, beam_stride_bytes: int,
+                    mean_ptr, sigma_ptr, nsigma: float, min_beams: int, mask_ptr, stream: int = 0) -> None:
+    """Multibeam coincidence RFI mask (include/dedisp.h)."""
+    st = lib().dedisp_rfi_mask(_ptr(x_ptr), x_dtype, nbeams, nseries, nsamps, beam_stride_bytes,
+                               _ptr(mean_ptr), _ptr(sigma_ptr), nsigma, min_beams, _ptr(mask_ptr),
+                               stream or None)
+    _check(None, st, "dedisp_rfi_mask")
