@@ -77,12 +77,17 @@ int64_t oracle_row_stride_bytes(int64_t nsamps, int nbits)
 }
 
 /* Sample t of a packed row.  2-bit: LSB-first, 4 per byte (reading R10);
- * 8-bit: unsigned byte (reading R11). */
+ * 8-bit: unsigned byte (reading R11); 1- and 4-bit (row f4, reading R36): the same
+ * LSB-first rule, 8 / 2 samples per byte: bits [t*nbits, (t+1)*nbits) of the row read
+ * as a little-endian bit string. */
 static inline uint32_t oracle_get_sample(const uint8_t *row, int64_t t, int nbits)
 {
     if (nbits == 8) return row[t];
-    return (row[t >> 2] >> (2 * (t & 3))) & 3u;
+    int64_t bit = t * nbits;
+    return (row[bit >> 3] >> (bit & 7)) & ((1u << nbits) - 1u);
 }
+
+static int oracle_nbits_ok(int nbits) { return nbits == 1 || nbits == 2 || nbits == 4 || nbits == 8; }
 
 /* O1 -- the literal triple loop on the packed bytes.
  *   in  : nchans rows of row_stride bytes, each holding nsamps_out+max_delay samples
@@ -93,7 +98,7 @@ int oracle_dedisperse_literal(int nchans, int ndm, int64_t nsamps_out,
                               int64_t row_stride, int nbits, uint32_t *out)
 {
     if (nchans < 1 || ndm < 1 || nsamps_out < 1 || !delay || !in || !out) return -1;
-    if (nbits != 2 && nbits != 8) return -1;
+    if (!oracle_nbits_ok(nbits)) return -1;
     for (int d = 0; d < ndm; ++d)
         for (int64_t t = 0; t < nsamps_out; ++t) {
             uint32_t acc = 0;
@@ -117,7 +122,7 @@ int oracle_dedisperse(int nchans, int ndm, int64_t nsamps_out,
                       uint32_t *out, int d_begin, int d_end, int nthreads)
 {
     if (nchans < 1 || ndm < 1 || nsamps_out < 1 || !delay || !in || !out) return -1;
-    if (nbits != 2 && nbits != 8) return -1;
+    if (!oracle_nbits_ok(nbits)) return -1;
     if (d_begin < 0 || d_end > ndm || d_begin > d_end || max_delay < 0) return -1;
     int64_t nsamps_in = nsamps_out + max_delay;
     uint8_t *u8 = NULL;
@@ -132,7 +137,7 @@ int oracle_dedisperse(int nchans, int ndm, int64_t nsamps_out,
         for (int c = 0; c < nchans; ++c)
             for (int64_t t = 0; t < nsamps_in; ++t)
                 u8[(size_t)c * nsamps_in + t] =
-                    (uint8_t)oracle_get_sample(in + (size_t)c * row_stride, t, 2);
+                    (uint8_t)oracle_get_sample(in + (size_t)c * row_stride, t, nbits);
         rows = u8;
         rstride = nsamps_in;
     }

@@ -101,6 +101,31 @@ def unpack2(row: np.ndarray, nsamps: int) -> np.ndarray:
     return ((row[:, None] >> sh[None, :]) & 3).reshape(-1)[:nsamps].astype(np.uint8)
 
 
+def pack_bits(levels: np.ndarray, nbits: int) -> np.ndarray:
+    """Pack levels (1-D, values < 2**nbits, nbits in 1/2/4/8) LSB-first into bytes, zero padded:
+    sample t occupies bits [t*nbits, (t+1)*nbits) of the row read as a little-endian bit string."""
+    if nbits == 8:
+        return levels.astype(np.uint8)
+    per = 8 // nbits
+    n = levels.shape[0]
+    nb = (n + per - 1) // per
+    buf = np.zeros(nb * per, dtype=np.uint8)
+    buf[:n] = levels
+    q = buf.reshape(nb, per)
+    out = np.zeros(nb, dtype=np.uint8)
+    for k in range(per):
+        out |= (q[:, k] << (k * nbits)).astype(np.uint8)
+    return out
+
+
+def unpack_bits(row: np.ndarray, nbits: int, nsamps: int) -> np.ndarray:
+    """Inverse of :func:`pack_bits` through numpy.unpackbits (a layout statement for tests)."""
+    if nbits == 8:
+        return row[:nsamps].astype(np.uint8)
+    bits = np.unpackbits(row, bitorder="little")[: nsamps * nbits].reshape(nsamps, nbits)
+    return (bits << np.arange(nbits, dtype=np.uint8)).sum(axis=1).astype(np.uint8)
+
+
 def _rng(seed: int, stream: int) -> np.random.Generator:
     return np.random.Generator(np.random.Philox(key=np.array([seed, stream], dtype=np.uint64)))
 
@@ -186,8 +211,10 @@ def random_small(seed: int, nchans: int, nsamps_in: int, nbits: int) -> np.ndarr
     g = _rng(seed, 7)
     if nbits == 8:
         return g.integers(0, 256, size=(nchans, nsamps_in), dtype=np.uint8)
-    lev = (g.random((nchans, nsamps_in)) * 4).astype(np.uint8)
-    return np.stack([pack2(lev[c]) for c in range(nchans)])
+    lev = (g.random((nchans, nsamps_in)) * (1 << nbits)).astype(np.uint8)
+    if nbits == 2:
+        return np.stack([pack2(lev[c]) for c in range(nchans)])
+    return np.stack([pack_bits(lev[c], nbits) for c in range(nchans)])
 
 
 def dedispersed_like(seed: int, nrows: int, nsamps: int, mean: float = 1536.0, sigma: float = 30.1,

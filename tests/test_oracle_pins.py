@@ -40,7 +40,9 @@ def _slice_sum(delay, u8, nsamps_out):
 def _unpack(packed, nbits, nsamps):
     if nbits == 8:
         return packed[:, :nsamps]
-    return np.stack([W.unpack2(r, nsamps) for r in packed])
+    if nbits == 2:
+        return np.stack([W.unpack2(r, nsamps) for r in packed])
+    return np.stack([W.unpack_bits(r, nbits, nsamps) for r in packed])
 
 
 def _read_delay_pins(golden_dir):
@@ -268,7 +270,21 @@ def test_prefix_sum_conservation(tiny):
         assert o[k].sum() == want
 
 
-@pytest.mark.parametrize("nbits", [2, 8])
+def test_sub_byte_layouts_against_unpackbits():
+    """Row f4 (reading R36): 1-, 2- and 4-bit samples are LSB-first; numpy.unpackbits
+    (bitorder='little') is the independent statement of that layout."""
+    for nbits, hexrow, want in ((1, "b1 03", [1, 0, 0, 0, 1, 1, 0, 1, 1, 1, 0, 0, 0, 0, 0, 0]),
+                                (4, "a3 0f 70", [3, 10, 15, 0, 0, 7]),
+                                (2, "e4", [0, 1, 2, 3])):
+        row = np.frombuffer(bytes.fromhex(hexrow.replace(" ", "")), dtype=np.uint8)
+        assert W.unpack_bits(row, nbits, len(want)).tolist() == want
+        assert W.pack_bits(np.array(want, np.uint8), nbits).tolist() == row.tolist()
+        delay = np.zeros((1, 1), np.int32)
+        out = oracle.dedisperse_literal(delay, row[None].copy(), nbits, len(want))
+        assert out[0].tolist() == want          # one channel, DM 0: the output is the samples
+
+
+@pytest.mark.parametrize("nbits", [1, 2, 4, 8])
 @pytest.mark.parametrize("seed", [1, 2, 3])
 def test_brute_force_random_small_shapes(seed, nbits):
     g = np.random.default_rng(seed)
