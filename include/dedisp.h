@@ -23,6 +23,8 @@
  *        nsamps_in = nsamps_out + max_delay samples, time contiguous.
  *        2-bit: 4 samples per byte, LSB first: sample t of a row is
  *               (row[t>>2] >> (2*(t&3))) & 3.   8-bit: one unsigned byte per sample.
+ *        1- and 4-bit (input-format variants): the same rule,
+ *               sample t = bits [t*nbits, (t+1)*nbits) of the row as a little-endian bit string.
  *        Row stride is TIGHT: dedisp_get_in_row_stride_bytes() =
  *        ceil(nsamps_in*nbits/8) bytes; no alignment is required of the base
  *        pointer or of the rows.  Bits past the last sample of a row are never read
@@ -55,7 +57,7 @@ typedef enum {
     DEDISP_OK = 0,
     DEDISP_ERR_INVALID_ARG = 1,       /* null pointer, non-positive size, bad geometry */
     DEDISP_ERR_NO_DM_LIST = 2,        /* execute/getter before dedisp_set_dm_list */
-    DEDISP_ERR_UNSUPPORTED_NBITS = 3, /* in_nbits not in {2, 8} */
+    DEDISP_ERR_UNSUPPORTED_NBITS = 3, /* in_nbits not in {1, 2, 4, 8} */
     DEDISP_ERR_UNSUPPORTED_DTYPE = 4, /* out_dtype not U32/F32 */
     DEDISP_ERR_OVERFLOW = 5,          /* nchans*(2^nbits-1) >= 2^24, or a delay beyond int32 */
     DEDISP_ERR_ALLOC = 6,             /* host or device allocation failed */

@@ -67,6 +67,12 @@ using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
 // (sweep on B200, wide8: (NW,W,K,NSTAGE) = (14,2,2,3) 81.6 ms, (7,4,2,3) 75.0, (6,4,2,3) 85.8,
 //  (12,2,3,3) 91.5, (10,2,3,3) 101.9)
 using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, 64, 128>;
+// 1-bit samples (row f4): the packed row IS the bit plane; sums <= 4096 need 13 planes
+using Cfg1 = Cfg<1, 15, 4, 4, 3, 13, 96, 224>;
+// 4-bit samples (row f4): 10 x 4 words = 1280-sample tiles, 8-channel trees, sums < 2^16
+using Cfg4 = Cfg<4, 10, 4, 2, 3, 16, 96, 224>;
+
+constexpr int geom_index(int nbits) { return nbits == 1 ? 0 : nbits == 2 ? 1 : nbits == 4 ? 2 : 3; }
 }  // namespace bs
 
 struct BitsliceParams {

@@ -385,10 +385,16 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
                                int nbits, void *out, size_t out_beam_stride, int out_f32,
                                cudaStream_t s)
 {
-    const BitsliceGeom &G = plan->geom[nbits == 2 ? 0 : 1];
+    const BitsliceGeom &G = plan->geom[geom_index(nbits)];
     if (!G.usable) return DEDISP_ERR_INVALID_ARG;
     if (nbits == 2)
         return execute_cfg<Cfg2>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                 out_beam_stride, out_f32, s);
+    if (nbits == 1)
+        return execute_cfg<Cfg1>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                 out_beam_stride, out_f32, s);
+    if (nbits == 4)
+        return execute_cfg<Cfg4>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
                                  out_beam_stride, out_f32, s);
     return execute_cfg<Cfg8>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
                              out_beam_stride, out_f32, s);

@@ -154,6 +154,84 @@ planes8_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row
     for (int p = 0; p < 8; ++p) row0[(size_t)p * row_pitch + i] = pw[p];
 }
 
+// ---- 1-bit and 4-bit samples (row f4) ----
+// Bytes [16 i, 16 i + 16) of a tight row as four byte-aligned words (zero past the row end):
+// the same two aligned 128-bit loads + funnel shifts as planes2_kernel.
+__device__ __forceinline__ void load16_aligned(const uint8_t *a, long long nvalid,
+                                               const uint8_t *valid_begin, const uint8_t *valid_end,
+                                               uint32_t (&r)[4])
+{
+    const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)15;
+    const int m = (int)((uintptr_t)a & 15);
+    uint4 lo = make_uint4(0, 0, 0, 0), hi = make_uint4(0, 0, 0, 0);
+    if (a0 + 16 > (uintptr_t)valid_begin && a0 < (uintptr_t)valid_end)
+        lo = __ldg(reinterpret_cast<const uint4 *>(a0));
+    if (m && a0 + 16 < (uintptr_t)valid_end) hi = __ldg(reinterpret_cast<const uint4 *>(a0 + 16));
+    const uint32_t v[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+    const int q = m >> 2, sh = (m & 3) * 8;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        uint32_t x0 = v[k], x1 = v[k + 1];
+        if (q == 1) { x0 = v[k + 1]; x1 = v[k + 2]; }
+        if (q == 2) { x0 = v[k + 2]; x1 = v[k + 3]; }
+        if (q == 3) { x0 = v[k + 3]; x1 = v[k + 4 < 8 ? k + 4 : 7]; }
+        r[k] = __funnelshift_r(x0, x1, sh);
+        const long long nb = nvalid - 4 * k;
+        if (nb <= 0) r[k] = 0;
+        else if (nb < 4) r[k] &= (1u << (8 * (int)nb)) - 1u;
+    }
+}
+
+// bits 0, 4, 8, ..., 28 of x -> bits 0..7
+__device__ __forceinline__ uint32_t every_fourth_bit_to_low8(uint32_t x)
+{
+    x &= 0x11111111u;
+    x = (x | (x >> 3)) & 0x03030303u;
+    x = (x | (x >> 6)) & 0x000f000fu;
+    x = (x | (x >> 12)) & 0x000000ffu;
+    return x;
+}
+
+// 1-bit: the LSB-first packed row IS bit plane 0; thread i copies 16 bytes = 4 words (128 samples).
+__global__ void __launch_bounds__(128)
+planes1_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride,
+               int nchans, const uint8_t *valid_begin, const uint8_t *valid_end,
+               uint32_t *__restrict__ planes, int row_pitch, int nchans_pad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 128-sample block
+    const int c = blockIdx.y, b = blockIdx.z;
+    if (4 * i >= row_pitch || c >= nchans_pad) return;
+    uint32_t r[4] = {0u, 0u, 0u, 0u};
+    const long long nvalid = (long long)row_stride - 16ll * i;
+    if (c < nchans && nvalid > 0)
+        load16_aligned(in + (size_t)b * in_beam_stride + (size_t)c * row_stride + 16u * (size_t)i, nvalid,
+                       valid_begin, valid_end, r);
+    uint32_t *row0 = planes + ((size_t)b * nchans_pad + c) * (size_t)row_pitch;
+    *reinterpret_cast<uint4 *>(row0 + 4 * i) = make_uint4(r[0], r[1], r[2], r[3]);
+}
+
+// 4-bit: thread i turns 16 bytes = 32 samples into one word of each of the 4 planes.
+__global__ void __launch_bounds__(128)
+planes4_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride,
+               int nchans, const uint8_t *valid_begin, const uint8_t *valid_end,
+               uint32_t *__restrict__ planes, int row_pitch, int nchans_pad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 32-sample word
+    const int c = blockIdx.y, b = blockIdx.z;
+    if (i >= row_pitch || c >= nchans_pad) return;
+    uint32_t r[4] = {0u, 0u, 0u, 0u};
+    const long long nvalid = (long long)row_stride - 16ll * i;
+    if (c < nchans && nvalid > 0)
+        load16_aligned(in + (size_t)b * in_beam_stride + (size_t)c * row_stride + 16u * (size_t)i, nvalid,
+                       valid_begin, valid_end, r);
+    uint32_t *row0 = planes + (((size_t)b * nchans_pad + c) * 4) * (size_t)row_pitch;
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+        row0[(size_t)p * row_pitch + i] =
+            every_fourth_bit_to_low8(r[0] >> p) | (every_fourth_bit_to_low8(r[1] >> p) << 8) |
+            (every_fourth_bit_to_low8(r[2] >> p) << 16) | (every_fourth_bit_to_low8(r[3] >> p) << 24);
+}
+
 cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
                           int nchans, int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
                           cudaStream_t s)
@@ -162,6 +240,14 @@ cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, s
     if (nbits == 2) {
         dim3 block(128), grid((row_pitch / 2 + 127) / 128, nchans_pad, nbeams);
         planes2_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
+                                              row_pitch, nchans_pad);
+    } else if (nbits == 1) {
+        dim3 block(128), grid((row_pitch / 4 + 127) / 128, nchans_pad, nbeams);
+        planes1_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
+                                              row_pitch, nchans_pad);
+    } else if (nbits == 4) {
+        dim3 block(128), grid((row_pitch + 127) / 128, nchans_pad, nbeams);
+        planes4_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans, in, vend, planes,
                                               row_pitch, nchans_pad);
     } else {
         dim3 block(128), grid((row_pitch + 127) / 128, nchans_pad, nbeams);
@@ -181,8 +267,7 @@ void bitslice_release(dedisp_plan p)
     p->d_rel = nullptr;
     p->d_ws = nullptr;
     p->d_order = nullptr;
-    p->geom[0] = BitsliceGeom();
-    p->geom[1] = BitsliceGeom();
+    for (int i = 0; i < 4; ++i) p->geom[i] = BitsliceGeom();
 }
 
 template <class C>
@@ -234,7 +319,9 @@ dedisp_status bitslice_prepare(dedisp_plan p)
         p->last_cuda_error = (int)e;
         return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
     }
-    fill_geom<bs::Cfg2>(p->geom[0], 2, nchans_pad, ndm_pad, max_off, 3ll * p->nchans);
-    fill_geom<bs::Cfg8>(p->geom[1], 8, nchans_pad, ndm_pad, max_off, 255ll * p->nchans);
+    fill_geom<bs::Cfg1>(p->geom[0], 1, nchans_pad, ndm_pad, max_off, 1ll * p->nchans);
+    fill_geom<bs::Cfg2>(p->geom[1], 2, nchans_pad, ndm_pad, max_off, 3ll * p->nchans);
+    fill_geom<bs::Cfg4>(p->geom[2], 4, nchans_pad, ndm_pad, max_off, 15ll * p->nchans);
+    fill_geom<bs::Cfg8>(p->geom[3], 8, nchans_pad, ndm_pad, max_off, 255ll * p->nchans);
     return DEDISP_OK;
 }

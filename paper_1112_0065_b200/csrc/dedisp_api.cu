@@ -13,15 +13,16 @@ unsigned long long g_launch_count = 0;
 namespace {
 
 bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+bool nbits_ok(int b) { return b == 1 || b == 2 || b == 4 || b == 8; }
 
 dedisp_status check_exec_args(dedisp_plan plan, int nbeams, long long nsamps_out, const void *in,
                               int nbits, void *out, dedisp_out_dtype dt)
 {
     if (!plan || !in || !out || nbeams < 1 || nsamps_out < 1) return DEDISP_ERR_INVALID_ARG;
     if (plan->ndm < 1 || !plan->d_delay) return DEDISP_ERR_NO_DM_LIST;
-    if (nbits != 2 && nbits != 8) return DEDISP_ERR_UNSUPPORTED_NBITS;
+    if (!nbits_ok(nbits)) return DEDISP_ERR_UNSUPPORTED_NBITS;
     if (dt != DEDISP_OUT_U32 && dt != DEDISP_OUT_F32) return DEDISP_ERR_UNSUPPORTED_DTYPE;
-    const long long maxv = (nbits == 2) ? 3 : 255;
+    const long long maxv = (1ll << nbits) - 1;
     if ((long long)plan->nchans * maxv >= (1ll << 24)) return DEDISP_ERR_OVERFLOW;
     if (((uintptr_t)out & 3u) != 0) return DEDISP_ERR_INVALID_ARG;
     return DEDISP_OK;
@@ -163,7 +164,7 @@ dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps
 {
     if (!plan || !in_host || !out_host || nbeams < 1 || nsamps_out < 1) return DEDISP_ERR_INVALID_ARG;
     if (plan->ndm < 1) return DEDISP_ERR_NO_DM_LIST;
-    if (in_nbits != 2 && in_nbits != 8) return DEDISP_ERR_UNSUPPORTED_NBITS;
+    if (!nbits_ok(in_nbits)) return DEDISP_ERR_UNSUPPORTED_NBITS;
     const size_t row = dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits);
     const size_t in_beam = row * (size_t)plan->nchans;
     const size_t out_beam = (size_t)plan->ndm * (size_t)nsamps_out * 4;
@@ -214,7 +215,7 @@ int dedisp_get_ndm(dedisp_plan plan) { return plan ? plan->ndm : 0; }
 
 size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, int in_nbits)
 {
-    if (!plan || plan->ndm < 1 || nsamps_out < 1 || (in_nbits != 2 && in_nbits != 8)) return 0;
+    if (!plan || plan->ndm < 1 || nsamps_out < 1 || !nbits_ok(in_nbits)) return 0;
     const unsigned long long n = (unsigned long long)nsamps_out + (unsigned long long)plan->max_delay;
     return (size_t)((n * (unsigned)in_nbits + 7) / 8);
 }
@@ -269,7 +270,7 @@ const char *dedisp_get_error_string(dedisp_status s)
         case DEDISP_OK: return "ok";
         case DEDISP_ERR_INVALID_ARG: return "invalid argument";
         case DEDISP_ERR_NO_DM_LIST: return "no DM list set";
-        case DEDISP_ERR_UNSUPPORTED_NBITS: return "unsupported in_nbits (2 or 8)";
+        case DEDISP_ERR_UNSUPPORTED_NBITS: return "unsupported in_nbits (1, 2, 4 or 8)";
         case DEDISP_ERR_UNSUPPORTED_DTYPE: return "unsupported output dtype";
         case DEDISP_ERR_OVERFLOW: return "sum or delay out of range";
         case DEDISP_ERR_ALLOC: return "allocation failed";

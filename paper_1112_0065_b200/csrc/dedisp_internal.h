@@ -31,7 +31,7 @@ struct dedisp_plan_s {
     int last_kernel = 0;
     int last_cuda_error = 0;
     // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
-    BitsliceGeom geom[2];         // [0]: 2-bit, [1]: 8-bit
+    BitsliceGeom geom[4];         // [log2(nbits)]: 1-, 2-, 4-, 8-bit samples
     uint32_t *d_rel = nullptr;    // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
     int32_t *d_ws = nullptr;      // [ngroups][nchans_pad] window start word
     int32_t *d_order = nullptr;   // [ndm_pad] trial index of each sorted lane, -1 = padding

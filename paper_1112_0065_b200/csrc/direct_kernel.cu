@@ -21,10 +21,12 @@ direct_kernel(const int32_t *__restrict__ delay, int nchans, int ndm, long long 
     for (int c = 0; c < nchans; ++c) {
         const long long ti = t + __ldg(&delay[(size_t)c * ndm + d]);
         const uint8_t *row = inb + (size_t)c * row_stride;
-        if (NBITS == 8)
+        if (NBITS == 8) {
             acc += row[ti];
-        else
-            acc += (row[ti >> 2] >> (2 * (ti & 3))) & 3u;
+        } else {   // LSB-first sub-byte samples: bits [ti*NBITS, (ti+1)*NBITS) of the row
+            const long long bit = ti * NBITS;
+            acc += (row[bit >> 3] >> (int)(bit & 7)) & ((1u << NBITS) - 1u);
+        }
     }
     uint8_t *ob = out + (size_t)b * out_beam_stride;
     const size_t idx = (size_t)d * (size_t)nsamps_out + (size_t)t;
@@ -51,6 +53,10 @@ cudaError_t launch_direct(const int32_t *d_delay, int nchans, int ndm, long long
                                                 in_beam_stride, o, out_beam_stride)
         if (nbits == 2 && !out_f32) LAUNCH(2, false);
         else if (nbits == 2) LAUNCH(2, true);
+        else if (nbits == 1 && !out_f32) LAUNCH(1, false);
+        else if (nbits == 1) LAUNCH(1, true);
+        else if (nbits == 4 && !out_f32) LAUNCH(4, false);
+        else if (nbits == 4) LAUNCH(4, true);
         else if (!out_f32) LAUNCH(8, false);
         else LAUNCH(8, true);
 #undef LAUNCH

@@ -87,6 +87,11 @@ SHAPES = [  # nchans, ndm, nsamps_out, nbits, dm_hi, df
     (1, 1, 1, 2, 0.0, -1.0), (3, 1, 5, 2, 50.0, -20.0), (37, 5, 333, 2, 120.0, -7.0),
     (64, 33, 4097, 2, 90.0, -4.0), (130, 70, 2049, 2, 300.0, -2.5), (100, 31, 1000, 8, 150.0, -3.0),
     (257, 3, 77, 8, 40.0, -1.0), (1024, 40, 3000, 2, 1000.0, -0.390625), (5, 64, 8192, 8, 10.0, -50.0),
+    # row f4: 1- and 4-bit samples
+    (1, 1, 1, 1, 0.0, -1.0), (37, 5, 333, 1, 120.0, -7.0), (64, 33, 4097, 1, 90.0, -4.0),
+    (1024, 70, 5000, 1, 1000.0, -0.390625), (4096, 40, 2100, 1, 400.0, -0.09765625),
+    (3, 1, 5, 4, 50.0, -20.0), (130, 70, 2049, 4, 300.0, -2.5), (1024, 40, 3000, 4, 1000.0, -0.390625),
+    (4096, 33, 1300, 4, 400.0, -0.09765625),
 ]
 
 
@@ -209,7 +214,7 @@ def test_execute_errors():
     p = make_plan(8, 64e-6, 1500.0, -10.0, [0.0, 10.0])
     x = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
     o = torch.zeros(1 << 16, dtype=torch.int32, device="cuda")
-    cases = [((p, 100, x, 4, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_UNSUPPORTED_NBITS),
+    cases = [((p, 100, x, 3, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_UNSUPPORTED_NBITS),
              ((p, 100, x, 2, o, 5), dd.DEDISP_ERR_UNSUPPORTED_DTYPE),
              ((p, 0, x, 2, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_INVALID_ARG),
              ((p, 100, 0, 2, o, dd.DEDISP_OUT_U32), dd.DEDISP_ERR_INVALID_ARG),
@@ -233,3 +238,30 @@ def test_launch_counter_and_probe():
     dd.dedisp_destroy(p)
     r = dd.dedisp_probe_alu_rate(0)
     assert 1e12 < r < 1e15
+
+
+@pytest.mark.parametrize("nbits", [1, 4])
+def test_sub_byte_variants_use_the_tiled_kernel_and_extreme_values(nbits):
+    """Row f4: HTRU channelisation with 1- and 4-bit samples runs on the bit-sliced kernel (not the
+    DIRECT fallback); all-ones input gives nchans * (2^nbits - 1) everywhere."""
+    w = W.CONFIGS["htru_gulp"].scaled(ndm=96, dm_hi=1000.0 * 95 / 1199, nsamps_out=6000)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.random_small(77 + nbits, w.nchans, w.nsamps_out + md, nbits)
+    want = oracle.dedisperse(delay, x, nbits, w.nsamps_out)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    assert np.array_equal(gpu_dedisperse(p, x[None], nbits, w.nsamps_out)[0], want)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
+    assert np.array_equal(gpu_dedisperse(p, x[None], nbits, w.nsamps_out, "f32")[0], oracle.to_f32(want))
+    ones = np.full_like(x, 0xFF)
+    got = gpu_dedisperse(p, ones[None], nbits, w.nsamps_out)[0]
+    assert np.all(got == w.nchans * ((1 << nbits) - 1))
+    # two beams in one batched call, beam 1 = all ones
+    both = np.stack([x, ones])
+    got2 = gpu_dedisperse(p, both, nbits, w.nsamps_out)
+    assert np.array_equal(got2[0], want) and np.all(got2[1] == w.nchans * ((1 << nbits) - 1))
+    dd.dedisp_destroy(p)
+    with pytest.raises(dd.DedispError) as e:
+        p = make_plan(8, 64e-6, 1500.0, -1.0, [0.0])
+        dd.dedisp_execute(p, 8, torch.zeros(64, dtype=torch.uint8, device="cuda"), 3,
+                          torch.zeros(8, dtype=torch.int32, device="cuda"), dd.DEDISP_OUT_U32, 0)
+    assert e.value.status == dd.DEDISP_ERR_UNSUPPORTED_NBITS
