@@ -509,7 +509,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER)
+    ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER + W.EXTRA_CONFIGS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events"],
                     help="dedisperse = the hot path (default, the metric BASELINE.json names); "

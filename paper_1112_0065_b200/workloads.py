@@ -28,7 +28,7 @@ class Workload:
     f_top: float          # MHz, frequency of channel 0
     df: float             # MHz, channel spacing (negative)
     dt: float             # s
-    nbits: int            # 2 or 8
+    nbits: int            # 1, 2, 4 or 8
     ndm: int
     dm_lo: float
     dm_hi: float
@@ -36,7 +36,7 @@ class Workload:
     out_dtype: str        # "u32" | "f32"
     nbeams: int
     seed: int
-    kind: str             # "uniform2" | "gauss2" | "gauss2_pulses" | "gauss8"
+    kind: str             # "uniform2" | "gauss2" | "gauss2_pulses" | "gauss8" | "uniform"
     npulses: int = 0
 
     def dms(self) -> np.ndarray:
@@ -68,7 +68,14 @@ CONFIGS: dict[str, Workload] = {
     "beams13": Workload("beams13", 1024, 1581.8, -0.390625, 64e-6, 2, 1200, 0.0, 1000.0, 65536,
                         "u32", 13, 1100, "gauss2"),
 }
-CONFIG_ORDER = ["tiny", "htru_gulp", "htru_long_pulses", "wide8", "beams13"]
+CONFIG_ORDER = ["tiny", "htru_gulp", "htru_long_pulses", "wide8", "beams13"]   # BASELINE.json configs
+# input-format variants: the HTRU gulp shape with 1- and 4-bit samples,
+# levels uniform on [0, 2^nbits) -- not BASELINE configs, bench/profile lines only
+CONFIGS["htru_gulp_1bit"] = replace(CONFIGS["htru_gulp"], name="htru_gulp_1bit", nbits=1, seed=1201,
+                                    kind="uniform")
+CONFIGS["htru_gulp_4bit"] = replace(CONFIGS["htru_gulp"], name="htru_gulp_4bit", nbits=4, seed=1204,
+                                    kind="uniform")
+EXTRA_CONFIGS = ["htru_gulp_1bit", "htru_gulp_4bit"]
 
 
 def _phi(x: float) -> float:
@@ -168,7 +175,9 @@ def generate(w: Workload, max_delay: int, beam: int = 0,
         thr_k = np.array([[_phi(j - k) for j in (-1.0, 0.0, 1.0)] for k in range(kmax + 1)])
     for c in range(w.nchans):
         g = _rng(seed, (beam << 32) | c)
-        if w.kind == "uniform2":
+        if w.kind == "uniform":
+            out[c] = pack_bits((g.random(nsamps_in) * (1 << w.nbits)).astype(np.uint8), w.nbits)
+        elif w.kind == "uniform2":
             u = g.random(nsamps_in)
             lev = (u * 4).astype(np.uint8)
             out[c] = pack2(lev)
