@@ -240,6 +240,20 @@ dedisp_status dedisp_rfi_mask(const void *x_dev, dedisp_out_dtype x_dtype, int n
                               const float *mean_dev, const float *sigma_dev, float nsigma,
                               int min_beams, unsigned char *mask_dev, void *cuda_stream);
 
+/* ---- input-format variant: telescope-order stream ---- */
+
+/* Re-lay a time-major filterbank stream (for every time sample all channels next to
+ * each other, channel fastest: sample (t, c) = bits [(t*nchans + c)*nbits, +nbits) of the stream,
+ * LSB-first) as the channel-major tight rows dedisp_execute reads (layouts above):
+ *   in_dev   DEVICE, nsamps*nchans*nbits/8 bytes, 4-byte aligned; nchans*nbits must be a
+ *            multiple of 32 (whole 32-bit words per time sample).
+ *   out_dev  DEVICE, nchans rows of ceil(nsamps*nbits/8) bytes, written completely (unused high
+ *            bits of a row's last byte are zero).  Pass nsamps = nsamps_out + max_delay and the
+ *            result is a valid dedisp_execute input.
+ * Only enqueues work on cuda_stream.  Errors: INVALID_ARG, UNSUPPORTED_NBITS, CUDA. */
+dedisp_status dedisp_transpose_time_major(const void *in_dev, int nchans, long long nsamps, int nbits,
+                                          void *out_dev, void *cuda_stream);
+
 /* Number of kernel launches this library has issued in this process (all plans). */
 unsigned long long dedisp_get_launch_count(void);
 

@@ -56,6 +56,7 @@ ABI = {
     "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
     "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
+    "dedisp_transpose_time_major": (_i, [_vp, _i, _ll, _i, _vp, _vp]),
     "dedisp_rfi_mask": (_i, [_vp, _i, _i, _ll, _ll, _sz, _vp, _vp, ctypes.c_float, _i, _vp, _vp]),
 }
 DEDISP_MF_MAX_WIDTH = 8192
@@ -238,3 +239,9 @@ def dedisp_rfi_mask(x_ptr, x_dtype: int, nbeams: int, nseries: int, nsamps: int,
                                _ptr(mean_ptr), _ptr(sigma_ptr), nsigma, min_beams, _ptr(mask_ptr),
                                stream or None)
     _check(None, st, "dedisp_rfi_mask")
+
+
+def dedisp_transpose_time_major(in_ptr, nchans: int, nsamps: int, nbits: int, out_ptr, stream: int = 0) -> None:
+    """Telescope-order stream -> channel-major tight rows (include/dedisp.h; row f4)."""
+    st = lib().dedisp_transpose_time_major(_ptr(in_ptr), nchans, nsamps, nbits, _ptr(out_ptr), stream or None)
+    _check(None, st, "dedisp_transpose_time_major")
