@@ -36,10 +36,24 @@
 #define BS8_W 4
 #endif
 #ifndef BS8_TREE_K
-#define BS8_TREE_K 2
+#define BS8_TREE_K 3
 #endif
 #ifndef BS8_NSTAGE
 #define BS8_NSTAGE 3
+#endif
+
+// ... and of the 4-bit kernel
+#ifndef BS4_NW
+#define BS4_NW 11
+#endif
+#ifndef BS4_W
+#define BS4_W 4
+#endif
+#ifndef BS4_TREE_K
+#define BS4_TREE_K 3
+#endif
+#ifndef BS4_NSTAGE
+#define BS4_NSTAGE 3
 #endif
 
 namespace bs {
@@ -63,14 +77,16 @@ struct Cfg {
 };
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
 using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
-// 8-bit samples: 7 x 4 words = 896-sample tiles, 8-channel trees, sums < 2^20
+// 8-bit samples: 7 x 4 words = 896-sample tiles, 16-channel trees, sums < 2^20
 // (sweep on B200, wide8: (NW,W,K,NSTAGE) = (14,2,2,3) 81.6 ms, (7,4,2,3) 75.0, (6,4,2,3) 85.8,
-//  (12,2,3,3) 91.5, (10,2,3,3) 101.9)
+//  (12,2,3,3) 91.5, (10,2,3,3) 101.9, (7,4,3,3) 74.5, (6,4,3,3) 84.9)
 using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, 64, 128>;
 // 1-bit samples (row f4): the packed row IS the bit plane; sums <= 4096 need 13 planes
 using Cfg1 = Cfg<1, 15, 4, 4, 3, 13, 96, 224>;
-// 4-bit samples (row f4): 10 x 4 words = 1280-sample tiles, 8-channel trees, sums < 2^16
-using Cfg4 = Cfg<4, 10, 4, 2, 3, 16, 96, 224>;
+// 4-bit samples (row f4): 11 x 4 words = 1408-sample tiles, 16-channel trees, sums < 2^16
+// (sweep on B200, gulp at 4 bits: (NW,W,K,NSTAGE) = (10,4,2,3) 2.88 ms, (10,4,3,3) 2.62, (10,4,4,3) 2.53,
+//  (11,4,3,3) 2.43, (9,4,3,3) 2.79, (12,3,2,3) 2.88, (14,2,3,3) 3.27)
+using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224>;
 
 constexpr int geom_index(int nbits) { return nbits == 1 ? 0 : nbits == 2 ? 1 : nbits == 4 ? 2 : 3; }
 }  // namespace bs
