@@ -265,3 +265,33 @@ def test_sub_byte_variants_use_the_tiled_kernel_and_extreme_values(nbits):
         dd.dedisp_execute(p, 8, torch.zeros(64, dtype=torch.uint8, device="cuda"), 3,
                           torch.zeros(8, dtype=torch.int32, device="cuda"), dd.DEDISP_OUT_U32, 0)
     assert e.value.status == dd.DEDISP_ERR_UNSUPPORTED_NBITS
+
+
+def test_cuda_graph_capture_and_replay():
+    """execute only enqueues kernels (no allocation, no sync in the steady state), so a whole
+    dedispersion step can be captured in a CUDA graph and replayed on new input."""
+    w = W.CONFIGS["tiny"]
+    delay, md, packed = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = torch.from_numpy(packed[0]).cuda()
+    out = torch.zeros((w.ndm, w.nsamps_out), dtype=torch.int32, device="cuda")
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        dd.dedisp_execute(p, w.nsamps_out, x, w.nbits, out, dd.DEDISP_OUT_U32, side.cuda_stream)   # warm-up
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            dd.dedisp_execute(p, w.nsamps_out, x, w.nbits, out, dd.DEDISP_OUT_U32,
+                              torch.cuda.current_stream().cuda_stream)
+    want = oracle.dedisperse(delay, packed[0], w.nbits, w.nsamps_out)
+    for trial in range(2):
+        if trial == 1:      # new data in the same buffers
+            packed2 = W.generate(w.scaled(seed=w.seed + 5), md)
+            x.copy_(torch.from_numpy(packed2))
+            want = oracle.dedisperse(delay, packed2, w.nbits, w.nsamps_out)
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), want)
+    print("tiny kernel:", dd.dedisp_get_last_kernel(p))
+    dd.dedisp_destroy(p)
