@@ -108,15 +108,19 @@ def dist_setup(ngpus: int):
     return rank, world, local
 
 
-def cpu_baseline(w: W.Workload, seconds_hint: str = "") -> dict:
+def cpu_baseline(w: W.Workload, seconds_hint: str = "", tscrunch: int = 1) -> dict:
     """The oracle as it stands, on this box's host cores, on a bounded sample."""
     import oracle
-    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
-    x = W.generate(w.scaled(nbeams=1), md)
+    delay, md = oracle.delay_table(w.nchans, tscrunch * w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w.scaled(nbeams=1), tscrunch * (w.nsamps_out + md) - w.nsamps_out)
     stride = max(1, (w.ndm * w.nsamps_out) // (1200 * 65536))   # ~ one HTRU gulp of work
     sub = np.ascontiguousarray(delay[:, ::stride])
     t0 = time.perf_counter()
-    _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)
+    if tscrunch > 1:
+        from oracle import tscrunch as TS
+        _, used = TS.dedisperse_tscrunch_bytes(sub, x, w.nbits, tscrunch, w.nsamps_out, return_threads=True)
+    else:
+        _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)
     dt = time.perf_counter() - t0
     units = sub.shape[1] * w.nsamps_out
     return {"value": units / dt, "unit": "DM-trial-samples/s", "cores": used, "kind": "oracle",
@@ -152,7 +156,10 @@ def run_ours(args) -> None:
     props = torch.cuda.get_device_properties(dev)
     stream = torch.cuda.current_stream()
 
-    plan = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+    k = args.tscrunch   # row f4: blocks of k samples summed, trials dedispersed on the grid k*dt (reading R38)
+    if k > 1 and w.kind == "gauss2_pulses":
+        raise SystemExit("bench.py: --tscrunch is benched on the noise-only configs")
+    plan = dd.dedisp_plan_create(w.nchans, k * w.dt, w.f_top, w.df)
     t0 = time.perf_counter()
     dd.dedisp_set_dm_list(plan, list(w.dms()))
     set_dm_ms = (time.perf_counter() - t0) * 1e3
@@ -165,10 +172,11 @@ def run_ours(args) -> None:
         kw = dict(pulse_sweep=dd.dedisp_get_delay_table(p2), pulses=pp)
         dd.dedisp_destroy(p2)
     # each rank gets its own seeded beam(s): beam index offset by rank
-    beams = [W.generate(w, md, beam=b, **kw) for b in replicas.beam_indices(rank, w.nbeams)]
+    beams = [W.generate(w, k * (w.nsamps_out + md) - w.nsamps_out, beam=b, **kw)
+             for b in replicas.beam_indices(rank, w.nbeams)]
     host_in = torch.from_numpy(np.stack(beams)).pin_memory()
     nb, nch, stride = host_in.shape
-    assert stride == dd.dedisp_get_in_row_stride_bytes(plan, w.nsamps_out, w.nbits)
+    assert stride == dd.dedisp_get_in_row_stride_bytes_tscrunch(plan, k, w.nsamps_out, w.nbits)
     x = host_in.to(dev)
     f32 = w.out_dtype == "f32"
     code = dd.DEDISP_OUT_F32 if f32 else dd.DEDISP_OUT_U32
@@ -177,8 +185,16 @@ def run_ours(args) -> None:
     in_bs, out_bs = nch * stride, w.ndm * w.nsamps_out * 4
 
     def step():
-        dd.dedisp_execute_batch(plan, nb, w.nsamps_out, x, in_bs, w.nbits, out, out_bs, code,
-                                stream.cuda_stream)
+        dd.dedisp_execute_tscrunch(plan, k, nb, w.nsamps_out, x, in_bs, w.nbits, out, out_bs, code,
+                                   stream.cuda_stream)
+
+    def host_step():
+        if k == 1:
+            return dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+        x.copy_(host_in, non_blocking=True)
+        step()
+        host_out.copy_(out, non_blocking=True)
+        stream.synchronize()
 
     dd.dedisp_set_timing(plan, True)
     for _ in range(args.warmup):
@@ -220,12 +236,12 @@ def run_ours(args) -> None:
     host_out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=out.dtype).pin_memory()
     dd.dedisp_set_timing(plan, False)
     e2e_steps = max(2, min(args.steps, 5))
-    dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+    host_step()
     if world > 1:
         dist.barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+        host_step()
     e2e_s = replicas.max_over_ranks((time.perf_counter() - t0) / e2e_steps, dev)
     e2e_value = replicas.job_throughput(w.dm_trial_samples(), world, e2e_s)
     same = bool(torch.equal(host_out.to(dev), out))
@@ -240,7 +256,7 @@ def run_ours(args) -> None:
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = props.multi_processor_count * ADDS_PER_CLK_PER_SM * sm_max_mhz * 1e6   # adds/s
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0)) * 1e9
-    adds = w.adds()
+    adds = w.adds() * k          # every fine sample is added once
     in_bytes, out_bytes = nb * in_bs, nb * out_bs
     t_alu, t_hbm = adds / alu_peak, (in_bytes + out_bytes) / hbm_peak
     mm = statistics.mean(main_ms) * 1e-3
@@ -261,7 +277,7 @@ def run_ours(args) -> None:
         probe = {"error": str(e)}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(w)
+        cpu = cpu_baseline(w, tscrunch=k)
     for line in PAPER_CONTEXT:
         log(line)
     res = {
@@ -270,10 +286,10 @@ def run_ours(args) -> None:
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
         "data": "synthetic",
         "config": {"workload": w.name, "nchans": w.nchans, "ndm": w.ndm, "nsamps_out": w.nsamps_out,
-                   "nbits": w.nbits, "nbeams_per_gpu": w.nbeams, "out_dtype": w.out_dtype,
+                   "nbits": w.nbits, "tscrunch": k, "nbeams_per_gpu": w.nbeams, "out_dtype": w.out_dtype,
                    "max_delay": md, "l2": "256 MiB flush buffer zeroed between timed iterations",
                    "parallelism": f"replicas x{world} (one seeded beam set per GPU, no collective)"},
-        "real_time_factor": w.obs_seconds() / (ms_per_step * 1e-3),
+        "real_time_factor": k * w.obs_seconds() / (ms_per_step * 1e-3),
         "roofline": roofline, "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": in_bytes,
                 "d2h_bytes_per_step": out_bytes, "steps": e2e_steps, "matches_device_run": same},
@@ -466,6 +482,130 @@ def _bench_find_events(args, dd, torch, w, widths, z, make_z, flush, stream) -> 
     print(json.dumps(res), flush=True)
 
 
+def _time_steps(torch, step, flush, stream, warmup, steps):
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def run_small_op(args) -> None:
+    """--op rfi_mask: row f3 on 13 beams x 2^24 float32 samples (the multibeam
+    zero-DM series of ~18 min at 64 us), 3 sigma in >= 4 beams.
+    --op transpose: row f4 (telescope-order stream -> channel-major rows) on the packed input of
+    --config.  Both HBM-bound single kernels; a step = one call, inputs resident in HBM."""
+    import torch
+    import paper_1112_0065_b200 as dd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    cpu = None
+    if args.op == "rfi_mask":
+        nb, n = 13, 1 << 24
+        hx = torch.randn((nb, 1, n), generator=torch.Generator().manual_seed(1301)).pin_memory()
+        x = hx.to(dev)
+        mean, sigma = torch.zeros((nb, 1), device=dev), torch.ones((nb, 1), device=dev)
+        m = torch.empty((1, n), dtype=torch.uint8, device=dev)
+        hm = torch.empty((1, n), dtype=torch.uint8).pin_memory()
+
+        def step():
+            dd.dedisp_rfi_mask(x, dd.DEDISP_OUT_F32, nb, 1, n, n * 4, mean, sigma, 3.0, 4, m, stream.cuda_stream)
+
+        def e2e():
+            x.copy_(hx, non_blocking=True)
+            step()
+            hm.copy_(m, non_blocking=True)
+            torch.cuda.synchronize()
+        units, unit, alg = n, "masked samples/s", nb * n * 4 + n
+        h2d, d2h = nb * n * 4, n
+        cfg = {"workload": "rfi_mask, seeded unit Gaussian series", "nbeams": nb, "nseries": 1, "nsamps": n,
+               "nsigma": 3.0, "min_beams": 4}
+        kern, metric, dtype = "rfi_mask_kernel", "RFI-mask samples/sec", "f32 compare"
+        if not args.no_cpu_baseline:
+            from oracle import rfi_mask as RM
+            sub = hx[:, :, : 1 << 21].numpy()
+            t0 = time.perf_counter()
+            RM.coincidence_mask(sub, np.zeros((nb, 1)), np.ones((nb, 1)), 3.0, 4)
+            dt = time.perf_counter() - t0
+            cpu = {"value": sub.shape[2] / dt, "unit": unit, "cores": 1, "kind": "oracle",
+                   "sample": f"first {sub.shape[2]} of {n} samples x {nb} beams, {dt:.2f} s"}
+    else:
+        w = W.CONFIGS[args.config].scaled(nbeams=1)
+        plan = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+        dd.dedisp_set_dm_list(plan, list(w.dms()))
+        nin = w.nsamps_out + dd.dedisp_get_max_delay(plan)
+        dd.dedisp_destroy(plan)
+        nbytes = nin * w.nchans * w.nbits // 8
+        hs = torch.from_numpy(np.random.default_rng(w.seed).integers(0, 256, nbytes, dtype=np.uint8)).pin_memory()
+        sd = hs.to(dev)
+        stride = (nin * w.nbits + 7) // 8
+        out = torch.empty((w.nchans, stride), dtype=torch.uint8, device=dev)
+        ho = torch.empty((w.nchans, stride), dtype=torch.uint8).pin_memory()
+
+        def step():
+            dd.dedisp_transpose_time_major(sd, w.nchans, nin, w.nbits, out, stream.cuda_stream)
+
+        def e2e():
+            sd.copy_(hs, non_blocking=True)
+            step()
+            ho.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        units, unit, alg = nin * w.nchans, "transposed samples/s", nbytes + w.nchans * stride
+        h2d, d2h = nbytes, w.nchans * stride
+        cfg = {"workload": f"time-major stream of {w.name} -> channel-major rows", "nchans": w.nchans,
+               "nsamps_in": nin, "nbits": w.nbits}
+        kern, metric, dtype = "time_major_kernel", "transposed samples/sec", "u8 bit re-layout"
+        if not args.no_cpu_baseline:
+            from oracle import time_major as TM
+            k = min(nin, 1 << 16)
+            t0 = time.perf_counter()
+            TM.to_channel_major(hs.numpy(), w.nchans, k, w.nbits)
+            dt = time.perf_counter() - t0
+            cpu = {"value": k * w.nchans / dt, "unit": unit, "cores": 1, "kind": "oracle",
+                   "sample": f"first {k} of {nin} time samples x {w.nchans} channels, {dt:.2f} s"}
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = dd.dedisp_get_launch_count()
+    step_ms = _time_steps(torch, step, flush, stream, args.warmup, args.steps)
+    launches = dd.dedisp_get_launch_count() - launches0 - args.warmup
+    clocks = sampler.stop()
+    ms = statistics.mean(step_ms)
+    e2e()
+    t0 = time.perf_counter()
+    e2e()
+    e2e_s = time.perf_counter() - t0
+    res = {"metric": metric, "value": units / (ms * 1e-3), "unit": unit, "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+           "config": dict(cfg, l2="256 MiB flush buffer zeroed between timed iterations"),
+           "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": alg / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": ncu_traffic_bytes(args.op),
+                        "kernel": kern, "kernel_ms": ms,
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
+           "cpu_baseline": cpu,
+           "e2e": {"value": units / e2e_s, "unit": unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "steps": 1},
+           "gpu_launches": launches, "clocks": clocks,
+           "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
+    print(json.dumps(res), flush=True)
+
+
 def run_reference(args) -> None:
     """The oracle, as it stands, on the host cores: the base contract's reference arm."""
     rank = int(os.environ.get("RANK", "0"))
@@ -511,15 +651,20 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER + W.EXTRA_CONFIGS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events"],
+    ap.add_argument("--tscrunch", type=int, default=1,
+                    help="--op dedisperse only: sum blocks of K input samples and dedisperse on the grid K*dt "
+                         "(row f4; the input then holds K x as many samples per output sample)")
+    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events", "rfi_mask", "transpose"],
                     help="dedisperse = the hot path (default, the metric BASELINE.json names); "
-                         "matched_filter = row f1 downstream of it; find_events = row f2 downstream of f1")
+                         "matched_filter = row f1 downstream of it; find_events = row f2 downstream of f1; rfi_mask = row f3; transpose = row f4")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
     elif args.op in ("matched_filter", "find_events"):
         run_matched_filter(args)
+    elif args.op in ("rfi_mask", "transpose"):
+        run_small_op(args)
     else:
         run_ours(args)
 

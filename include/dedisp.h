@@ -103,6 +103,32 @@ dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamp
                                    void *out_dev, size_t out_beam_stride_bytes,
                                    dedisp_out_dtype out_dtype, void *cuda_stream);
 
+/* Dedispersion at reduced time resolution ("time scrunching", SURVEY.md Sec. 8(f) row f4;
+ * DESIGN.md reading R38 -- the paper only says that ~1200 trial DMs are searched).
+ * Every input row is first summed in non-overlapping blocks of `tscrunch` samples (block 0 starts
+ * at sample 0; raw sums, no division), and the block sums are dedispersed on the coarse grid:
+ *
+ *     s[c][u]   = sum_{j < tscrunch} in[c][tscrunch*u + j]
+ *     out[d][t] = sum_c s[c][ t + delay[c][d] ]
+ *
+ * `plan` describes the COARSE grid: create it with dt_s = tscrunch * (the input's sample time);
+ * delay[][] and max_delay are in coarse samples.  Each input row holds
+ * tscrunch * (nsamps_out + max_delay) samples of in_nbits bits in a tight row of
+ * dedisp_get_in_row_stride_bytes_tscrunch() bytes; out is [ndm][nsamps_out] as for dedisp_execute;
+ * beams as in dedisp_execute_batch.  Requires tscrunch >= 1 and tscrunch*(2^in_nbits - 1) <= 255
+ * (else DEDISP_ERR_INVALID_ARG) and nchans*tscrunch*(2^in_nbits - 1) < 2^24 (else
+ * DEDISP_ERR_OVERFLOW).  tscrunch = 1 is dedisp_execute_batch.  Factors 2, 4, 8, 16 with
+ * in_nbits*tscrunch <= 32 are summed inside the bit-plane pre-pass and run the bit-sliced kernel
+ * on 2..6 (or 8) planes; any other factor is summed to bytes and served by the DIRECT kernel.
+ * Only enqueues work on the stream. */
+dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams, long long nsamps_out,
+                                      const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
+                                      void *out_dev, size_t out_beam_stride_bytes,
+                                      dedisp_out_dtype out_dtype, void *cuda_stream);
+/* ceil(tscrunch * (nsamps_out + max_delay) * in_nbits / 8); 0 on error. */
+size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, long long nsamps_out,
+                                               int in_nbits);
+
 /* End-to-end convenience with HOST buffers (tight beam strides): copies the
  * packed input host->device, runs dedisp_execute_batch, copies the result back
  * and synchronises.  Device staging buffers are owned and reused by the plan.

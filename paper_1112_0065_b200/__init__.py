@@ -37,6 +37,8 @@ ABI = {
     "dedisp_set_dm_list": (_i, [_vp, ctypes.POINTER(_d), _i]),
     "dedisp_execute": (_i, [_vp, _ll, _vp, _i, _vp, _i, _vp]),
     "dedisp_execute_batch": (_i, [_vp, _i, _ll, _vp, _sz, _i, _vp, _sz, _i, _vp]),
+    "dedisp_execute_tscrunch": (_i, [_vp, _i, _i, _ll, _vp, _sz, _i, _vp, _sz, _i, _vp]),
+    "dedisp_get_in_row_stride_bytes_tscrunch": (_sz, [_vp, _i, _ll, _i]),
     "dedisp_execute_host": (_i, [_vp, _i, _ll, _vp, _i, _vp, _i]),
     "dedisp_destroy": (_i, [_vp]),
     "dedisp_get_max_delay": (_i, [_vp]),
@@ -128,6 +130,18 @@ def dedisp_execute_batch(plan: int, nbeams: int, nsamps_out: int, in_ptr, in_bea
     st = lib().dedisp_execute_batch(plan, nbeams, nsamps_out, _ptr(in_ptr), in_beam_stride, in_nbits,
                                     _ptr(out_ptr), out_beam_stride, out_dtype, stream or None)
     _check(plan, st, "dedisp_execute_batch")
+
+
+def dedisp_execute_tscrunch(plan: int, tscrunch: int, nbeams: int, nsamps_out: int, in_ptr, in_beam_stride: int,
+                            in_nbits: int, out_ptr, out_beam_stride: int, out_dtype: int,
+                            stream: int = 0) -> None:
+    st = lib().dedisp_execute_tscrunch(plan, tscrunch, nbeams, nsamps_out, _ptr(in_ptr), in_beam_stride,
+                                       in_nbits, _ptr(out_ptr), out_beam_stride, out_dtype, stream or None)
+    _check(plan, st, "dedisp_execute_tscrunch")
+
+
+def dedisp_get_in_row_stride_bytes_tscrunch(plan: int, tscrunch: int, nsamps_out: int, in_nbits: int) -> int:
+    return lib().dedisp_get_in_row_stride_bytes_tscrunch(plan, tscrunch, nsamps_out, in_nbits)
 
 
 def dedisp_execute_host(plan: int, nbeams: int, nsamps_out: int, in_host, in_nbits: int, out_host,

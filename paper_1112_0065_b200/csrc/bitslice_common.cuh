@@ -88,7 +88,41 @@ using Cfg1 = Cfg<1, 15, 4, 4, 3, 13, 96, 224>;
 //  (11,4,3,3) 2.43, (9,4,3,3) 2.79, (12,3,2,3) 2.88, (14,2,3,3) 3.27)
 using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224>;
 
-constexpr int geom_index(int nbits) { return nbits == 1 ? 0 : nbits == 2 ? 1 : nbits == 4 ? 2 : 3; }
+// 3-, 5- and 6-plane samples exist only as time-scrunched sums (row f4, reading R38:
+// k samples of 1/2/4 bits added by the pre-pass): sums < 2^13 / 2^16 / 2^16
+// (warps incl. the producer come in fours: the register file is per SM sub-partition)
+#ifndef BS3_NW
+#define BS3_NW 15
+#endif
+#ifndef BS3_TREE_K
+#define BS3_TREE_K 3
+#endif
+#ifndef BS5_NW
+#define BS5_NW 11
+#endif
+#ifndef BS5_TREE_K
+#define BS5_TREE_K 3
+#endif
+#ifndef BS6_NW
+#define BS6_NW 11
+#endif
+#ifndef BS6_TREE_K
+#define BS6_TREE_K 3
+#endif
+using Cfg3 = Cfg<3, BS3_NW, 4, BS3_TREE_K, 3, 13, 96, 224>;
+using Cfg5 = Cfg<5, BS5_NW, 4, BS5_TREE_K, 3, 16, 96, 224>;
+using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160>;
+
+constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8
+constexpr int geom_index(int nplanes) { return nplanes; }
+// planes needed for the block sums of k samples of nbits bits, rounded up to a built geometry (0: none)
+inline int tscrunch_planes(int nbits, int k)
+{
+    const long long maxv = (long long)k * ((1 << nbits) - 1);
+    int nb = 1;
+    while ((1ll << nb) <= maxv) ++nb;
+    return nb <= 6 ? nb : nb <= 8 ? 8 : 0;
+}
 }  // namespace bs
 
 struct BitsliceParams {

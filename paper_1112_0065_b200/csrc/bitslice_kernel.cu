@@ -317,8 +317,8 @@ cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s)
 
 template <class C>
 dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, long long nsamps_out,
-                          const uint8_t *in, size_t row_stride, size_t in_beam_stride, void *out,
-                          size_t out_beam_stride, int out_f32, cudaStream_t s)
+                          const uint8_t *in, size_t row_stride, size_t in_beam_stride, int in_nbits,
+                          int tscrunch, void *out, size_t out_beam_stride, int out_f32, cudaStream_t s)
 {
     const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
     const long long pitch =
@@ -340,8 +340,13 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device));
 
     if (plan->timing) cudaEventRecord(plan->ev[0], s);
-    DEDISP_CUDA_TRY(plan, launch_planes(C::NB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
-                                        plan->d_planes, (int)pitch, G.nchans_pad, s));
+    if (tscrunch == 1)
+        DEDISP_CUDA_TRY(plan, launch_planes(C::NB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
+                                            plan->d_planes, (int)pitch, G.nchans_pad, s));
+    else
+        DEDISP_CUDA_TRY(plan, launch_planes_tscrunch(in_nbits, tscrunch, C::NB, in, in_beam_stride, row_stride,
+                                                     plan->nchans, nbeams, plan->d_planes, (int)pitch,
+                                                     G.nchans_pad, s));
     if (plan->timing) {
         cudaEventRecord(plan->ev[1], s);
         cudaEventRecord(plan->ev[2], s);
@@ -382,20 +387,28 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
 
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
-                               int nbits, void *out, size_t out_beam_stride, int out_f32,
+                               int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
                                cudaStream_t s)
 {
-    const BitsliceGeom &G = plan->geom[geom_index(nbits)];
-    if (!G.usable) return DEDISP_ERR_INVALID_ARG;
-    if (nbits == 2)
-        return execute_cfg<Cfg2>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                 out_beam_stride, out_f32, s);
-    if (nbits == 1)
-        return execute_cfg<Cfg1>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                 out_beam_stride, out_f32, s);
-    if (nbits == 4)
-        return execute_cfg<Cfg4>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                 out_beam_stride, out_f32, s);
-    return execute_cfg<Cfg8>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                             out_beam_stride, out_f32, s);
+    // bit planes per (block-summed) sample; a scrunch factor the pre-pass does not build is not served here
+    const bool pow2 = tscrunch == 2 || tscrunch == 4 || tscrunch == 8 || tscrunch == 16;
+    if (tscrunch != 1 && !(pow2 && nbits * tscrunch <= 32)) return DEDISP_ERR_INVALID_ARG;
+    const int np = tscrunch == 1 ? nbits : tscrunch_planes(nbits, tscrunch);
+    if (np < 1 || np >= NGEOM) return DEDISP_ERR_INVALID_ARG;
+    const BitsliceGeom &G = plan->geom[geom_index(np)];
+    const long long maxsum = (long long)plan->nchans * tscrunch * ((1ll << nbits) - 1);
+    if (!G.usable || maxsum >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
+#define BS_RUN(CFG)                                                                                   \
+    return execute_cfg<CFG>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, nbits, tscrunch, \
+                            out, out_beam_stride, out_f32, s)
+    switch (np) {
+        case 1: BS_RUN(Cfg1);
+        case 2: BS_RUN(Cfg2);
+        case 3: BS_RUN(Cfg3);
+        case 4: BS_RUN(Cfg4);
+        case 5: BS_RUN(Cfg5);
+        case 6: BS_RUN(Cfg6);
+        default: BS_RUN(Cfg8);
+    }
+#undef BS_RUN
 }

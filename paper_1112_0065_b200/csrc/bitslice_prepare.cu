@@ -258,6 +258,128 @@ cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, s
     return cudaGetLastError();
 }
 
+// ---- time-scrunch pre-passes (row f4, reading R38) ----
+// n low bits set in every `period` bits
+__host__ __device__ constexpr uint32_t rep_mask(int n, int period)
+{
+    uint32_t m = 0;
+    for (int b = 0; b < 32; ++b)
+        if (b % period < n) m |= 1u << b;
+    return m;
+}
+
+// bit i*F of x -> bit i  (32/F bits): log2(32/F) mask-shift steps
+template <int F>
+__device__ __forceinline__ uint32_t gather_every(uint32_t x)
+{
+    x &= rep_mask(1, F);
+#pragma unroll
+    for (int g = 1; g * F < 32; g *= 2) x = (x | (x >> (g * (F - 1)))) & rep_mask(2 * g, 2 * g * F);
+    return x;
+}
+
+// Thread i of a row sums blocks of K = 2^LOG2K samples of NBITS bits and emits word i (32 block sums)
+// of each of NPL bit planes.  F = NBITS*K <= 32 bits of the row make one sum, so the thread reads the
+// F words from byte 4*F*i of the (tight, arbitrarily aligned) row: F+1 aligned 32-bit loads and a
+// funnel shift.  Adjacent fields are added pairwise in place (SWAR, LOG2K steps; a sum of K samples
+// fits its F-bit field), then bit p of every field is gathered into plane p.
+template <int NBITS, int LOG2K, int NPL>
+__global__ void __launch_bounds__(128)
+planes_tscrunch_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride,
+                       int nchans, const uint8_t *valid_begin, const uint8_t *valid_end,
+                       uint32_t *__restrict__ planes, int row_pitch, int nchans_pad)
+{
+    constexpr int F = NBITS << LOG2K;     // bits per block
+    constexpr int PER = 32 / F;           // block sums per 32-bit word
+    static_assert(F <= 32, "a block must fit one word");
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y, b = blockIdx.z;
+    if (i >= row_pitch || c >= nchans_pad) return;
+    uint32_t pw[NPL];
+#pragma unroll
+    for (int p = 0; p < NPL; ++p) pw[p] = 0u;
+    const long long nvalid = (long long)row_stride - 4ll * F * i;   // bytes of the row from this thread's first
+    if (c < nchans && nvalid > 0) {
+        const uint8_t *a = in + (size_t)b * in_beam_stride + (size_t)c * row_stride + (size_t)(4 * F) * (size_t)i;
+        const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)3;
+        const int sh = (int)((uintptr_t)a & 3) * 8;
+        uint32_t v[F + 1];
+#pragma unroll
+        for (int q = 0; q <= F; ++q) {
+            const uintptr_t aq = a0 + 4u * q;
+            // an aligned word is loaded only if it overlaps the caller's buffer and the thread's bytes
+            const bool need = (q < F || sh) && 4ll * q - (sh >> 3) < nvalid &&
+                              aq + 4 > (uintptr_t)valid_begin && aq < (uintptr_t)valid_end;
+            v[q] = need ? __ldg(reinterpret_cast<const uint32_t *>(aq)) : 0u;
+        }
+#pragma unroll
+        for (int q = 0; q < F; ++q) {
+            uint32_t x = __funnelshift_r(v[q], v[q + 1], sh);
+            const long long nb = nvalid - 4 * q;
+            if (nb <= 0) x = 0;
+            else if (nb < 4) x &= (1u << (8 * (int)nb)) - 1u;
+#pragma unroll
+            for (int f = NBITS; f < F; f *= 2) x = (x & rep_mask(f, 2 * f)) + ((x >> f) & rep_mask(f, 2 * f));
+#pragma unroll
+            for (int p = 0; p < NPL; ++p)
+                if (p < F) pw[p] |= gather_every<F>(x >> p) << ((q * PER) & 31);
+        }
+    }
+    uint32_t *row0 = planes + (((size_t)b * nchans_pad + c) * NPL) * (size_t)row_pitch;
+#pragma unroll
+    for (int p = 0; p < NPL; ++p) row0[(size_t)p * row_pitch + i] = pw[p];
+}
+
+// Any factor k (k * (2^nbits - 1) <= 255): one byte per block sum, for the DIRECT kernel.
+__global__ void __launch_bounds__(256)
+tscrunch_bytes_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row_stride, int nbits, int k,
+                      long long nsamps_scr, uint8_t *__restrict__ out)
+{
+    const long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= nsamps_scr) return;
+    const int c = blockIdx.y, b = blockIdx.z;
+    const uint8_t *row = in + (size_t)b * in_beam_stride + (size_t)c * row_stride;
+    uint32_t acc = 0;
+    for (int j = 0; j < k; ++j) {
+        const long long bit = (u * k + j) * nbits;
+        acc += (row[bit >> 3] >> (bit & 7)) & ((1u << nbits) - 1u);
+    }
+    out[((size_t)b * gridDim.y + c) * (size_t)nsamps_scr + (size_t)u] = (uint8_t)acc;
+}
+
+cudaError_t launch_planes_tscrunch(int nbits, int k, int nplanes, const uint8_t *in, size_t in_beam_stride,
+                                   size_t row_stride, int nchans, int nbeams, uint32_t *planes,
+                                   int row_pitch, int nchans_pad, cudaStream_t s)
+{
+    const uint8_t *vend = in + (size_t)(nbeams - 1) * in_beam_stride + (size_t)nchans * row_stride;
+    const dim3 block(128), grid((row_pitch + 127) / 128, nchans_pad, nbeams);
+    const int key = nbits * 100 + k;
+#define TSC(NB, LK, NPL)                                                                                    \
+    case NB * 100 + (1 << LK):                                                                              \
+        if (nplanes != NPL) return cudaErrorInvalidValue;                                                   \
+        planes_tscrunch_kernel<NB, LK, NPL><<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nchans,  \
+                                                                   in, vend, planes, row_pitch, nchans_pad); \
+        break;
+    switch (key) {
+        TSC(1, 1, 2) TSC(1, 2, 3) TSC(1, 3, 4) TSC(1, 4, 5)
+        TSC(2, 1, 3) TSC(2, 2, 4) TSC(2, 3, 5) TSC(2, 4, 6)
+        TSC(4, 1, 5) TSC(4, 2, 6) TSC(4, 3, 8)
+        default: return cudaErrorInvalidValue;
+    }
+#undef TSC
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tscrunch_bytes(int nbits, int k, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
+                                  int nchans, int nbeams, long long nsamps_scr, uint8_t *out, cudaStream_t s)
+{
+    const dim3 block(256), grid((unsigned)((nsamps_scr + 255) / 256), nchans, nbeams);
+    tscrunch_bytes_kernel<<<grid, block, 0, s>>>(in, in_beam_stride, row_stride, nbits, k, nsamps_scr, out);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
 // ---- host side of set_dm_list ------------------------------------------------
 void bitslice_release(dedisp_plan p)
 {
@@ -267,14 +389,14 @@ void bitslice_release(dedisp_plan p)
     p->d_rel = nullptr;
     p->d_ws = nullptr;
     p->d_order = nullptr;
-    for (int i = 0; i < 4; ++i) p->geom[i] = BitsliceGeom();
+    for (int i = 0; i < bs::NGEOM; ++i) p->geom[i] = BitsliceGeom();
 }
 
 template <class C>
-static void fill_geom(BitsliceGeom &G, int nbits, int nchans_pad, int ndm_pad, int max_off, long long maxsum)
+static void fill_geom(BitsliceGeom &G, int nchans_pad, int ndm_pad, int max_off)
 {
     G = BitsliceGeom();
-    G.nbits = nbits;
+    G.nbits = C::NB;
     G.nchans_pad = nchans_pad;
     G.ndm_pad = ndm_pad;
     G.ngroups = ndm_pad / 32;
@@ -284,7 +406,7 @@ static void fill_geom(BitsliceGeom &G, int nbits, int nchans_pad, int ndm_pad, i
     if (need <= C::WIN_S) G.win_words = C::WIN_S;
     else if (need <= C::WIN_L) G.win_words = C::WIN_L;
     else return;   // DM steps too coarse for a tile window: the DIRECT kernel serves the plan
-    G.usable = maxsum < (1ll << C::NP);
+    G.usable = true;   // bitslice_execute still checks that the largest possible sum fits nplanes_acc
 }
 
 dedisp_status bitslice_prepare(dedisp_plan p)
@@ -319,9 +441,12 @@ dedisp_status bitslice_prepare(dedisp_plan p)
         p->last_cuda_error = (int)e;
         return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
     }
-    fill_geom<bs::Cfg1>(p->geom[0], 1, nchans_pad, ndm_pad, max_off, 1ll * p->nchans);
-    fill_geom<bs::Cfg2>(p->geom[1], 2, nchans_pad, ndm_pad, max_off, 3ll * p->nchans);
-    fill_geom<bs::Cfg4>(p->geom[2], 4, nchans_pad, ndm_pad, max_off, 15ll * p->nchans);
-    fill_geom<bs::Cfg8>(p->geom[3], 8, nchans_pad, ndm_pad, max_off, 255ll * p->nchans);
+    fill_geom<bs::Cfg1>(p->geom[1], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg2>(p->geom[2], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg3>(p->geom[3], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg4>(p->geom[4], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg5>(p->geom[5], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg6>(p->geom[6], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg8>(p->geom[8], nchans_pad, ndm_pad, max_off);
     return DEDISP_OK;
 }

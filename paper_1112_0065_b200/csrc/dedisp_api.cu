@@ -108,22 +108,25 @@ dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int n
     return st;
 }
 
-dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamps_out,
-                                   const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
-                                   void *out_dev, size_t out_beam_stride_bytes,
-                                   dedisp_out_dtype out_dtype, void *cuda_stream)
+dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams, long long nsamps_out,
+                                      const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
+                                      void *out_dev, size_t out_beam_stride_bytes,
+                                      dedisp_out_dtype out_dtype, void *cuda_stream)
 {
     dedisp_status st = check_exec_args(plan, nbeams, nsamps_out, in_dev, in_nbits, out_dev, out_dtype);
     if (st != DEDISP_OK) return st;
     if (nbeams > 1 && (out_beam_stride_bytes & 3u)) return DEDISP_ERR_INVALID_ARG;
+    const long long maxv = (1ll << in_nbits) - 1;
+    if (tscrunch < 1 || (tscrunch > 1 && tscrunch * maxv > 255)) return DEDISP_ERR_INVALID_ARG;
+    if ((long long)plan->nchans * tscrunch * maxv >= (1ll << 24)) return DEDISP_ERR_OVERFLOW;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const size_t row_stride = dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits);
+    const size_t row_stride = dedisp_get_in_row_stride_bytes_tscrunch(plan, tscrunch, nsamps_out, in_nbits);
     const int f32 = (out_dtype == DEDISP_OUT_F32);
     const uint8_t *in = (const uint8_t *)in_dev;
 
     if (plan->want != DEDISP_KERNEL_DIRECT) {
         st = bitslice_execute(plan, nbeams, nsamps_out, in, row_stride, in_beam_stride_bytes,
-                              in_nbits, out_dev, out_beam_stride_bytes, f32, s);
+                              in_nbits, tscrunch, out_dev, out_beam_stride_bytes, f32, s);
         if (st == DEDISP_OK) {
             plan->last_kernel = DEDISP_KERNEL_BITSLICE;
             return DEDISP_OK;
@@ -131,13 +134,38 @@ dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamp
         // INVALID_ARG from bitslice_execute means "plan does not fit this kernel"
         if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE) return st;
     }
+    int direct_nbits = in_nbits;
+    size_t direct_beam_stride = in_beam_stride_bytes;
+    size_t direct_row_stride = row_stride;
+    if (tscrunch > 1) {
+        // block sums as one byte each in the plan's scratch, then the DIRECT kernel on 8-bit samples
+        const long long n_scr = nsamps_out + plan->max_delay;
+        const size_t need = (size_t)nbeams * plan->nchans * (size_t)n_scr;
+        if (plan->planes_bytes < need) {
+            cudaFree(plan->d_planes);
+            plan->d_planes = nullptr;
+            plan->planes_bytes = 0;
+            if (cudaMalloc(&plan->d_planes, need) != cudaSuccess) {
+                cudaGetLastError();
+                return DEDISP_ERR_ALLOC;
+            }
+            plan->planes_bytes = need;
+        }
+        if (nbeams > 65535 || plan->nchans > 65535) return DEDISP_ERR_INVALID_ARG;
+        DEDISP_CUDA_TRY(plan, launch_tscrunch_bytes(in_nbits, tscrunch, in, in_beam_stride_bytes, row_stride,
+                                                    plan->nchans, nbeams, n_scr, (uint8_t *)plan->d_planes, s));
+        in = (const uint8_t *)plan->d_planes;
+        direct_nbits = 8;
+        direct_row_stride = (size_t)n_scr;
+        direct_beam_stride = (size_t)plan->nchans * (size_t)n_scr;
+    }
     if (plan->timing) cudaEventRecord(plan->ev[2], s);
     // grid.z limit of the direct kernel
     for (int b0 = 0; b0 < nbeams; b0 += 65535) {
         const int nb = (nbeams - b0 < 65535) ? nbeams - b0 : 65535;
         DEDISP_CUDA_TRY(plan, launch_direct(plan->d_delay, plan->nchans, plan->ndm, nsamps_out,
-                                            in + (size_t)b0 * in_beam_stride_bytes, row_stride,
-                                            in_beam_stride_bytes, in_nbits,
+                                            in + (size_t)b0 * direct_beam_stride, direct_row_stride,
+                                            direct_beam_stride, direct_nbits,
                                             (uint8_t *)out_dev + (size_t)b0 * out_beam_stride_bytes,
                                             out_beam_stride_bytes, f32, nb, s));
     }
@@ -148,6 +176,15 @@ dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamp
     }
     plan->last_kernel = DEDISP_KERNEL_DIRECT;
     return DEDISP_OK;
+}
+
+dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamps_out,
+                                   const void *in_dev, size_t in_beam_stride_bytes, int in_nbits,
+                                   void *out_dev, size_t out_beam_stride_bytes,
+                                   dedisp_out_dtype out_dtype, void *cuda_stream)
+{
+    return dedisp_execute_tscrunch(plan, 1, nbeams, nsamps_out, in_dev, in_beam_stride_bytes, in_nbits, out_dev,
+                                   out_beam_stride_bytes, out_dtype, cuda_stream);
 }
 
 dedisp_status dedisp_execute(dedisp_plan plan, long long nsamps_out, const void *in_dev,
@@ -218,6 +255,13 @@ size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, in
     if (!plan || plan->ndm < 1 || nsamps_out < 1 || !nbits_ok(in_nbits)) return 0;
     const unsigned long long n = (unsigned long long)nsamps_out + (unsigned long long)plan->max_delay;
     return (size_t)((n * (unsigned)in_nbits + 7) / 8);
+}
+
+size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, long long nsamps_out, int in_nbits)
+{
+    if (!plan || plan->ndm < 1 || nsamps_out < 1 || tscrunch < 1 || !nbits_ok(in_nbits)) return 0;
+    const unsigned long long n = (unsigned long long)nsamps_out + (unsigned long long)plan->max_delay;
+    return (size_t)((n * (unsigned)tscrunch * (unsigned)in_nbits + 7) / 8);
 }
 
 dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out)

@@ -31,7 +31,7 @@ struct dedisp_plan_s {
     int last_kernel = 0;
     int last_cuda_error = 0;
     // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
-    BitsliceGeom geom[4];         // [log2(nbits)]: 1-, 2-, 4-, 8-bit samples
+    BitsliceGeom geom[9];         // [bit planes per sample]: 1, 2, 4, 8 = packed widths; 3, 5, 6 = time-scrunched sums
     uint32_t *d_rel = nullptr;    // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
     int32_t *d_ws = nullptr;      // [ngroups][nchans_pad] window start word
     int32_t *d_order = nullptr;   // [ndm_pad] trial index of each sorted lane, -1 = padding
@@ -76,10 +76,17 @@ cudaError_t launch_direct(const int32_t *d_delay, int nchans, int ndm, long long
 cudaError_t launch_planes(int nbits, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
                           int nchans, int nbeams, uint32_t *planes, int row_pitch, int nchans_pad,
                           cudaStream_t s);
+// time-scrunch pre-passes (row f4): block sums of k samples -> `nplanes` bit planes / one byte per sum
+cudaError_t launch_planes_tscrunch(int nbits, int k, int nplanes, const uint8_t *in, size_t in_beam_stride,
+                                   size_t row_stride, int nchans, int nbeams, uint32_t *planes,
+                                   int row_pitch, int nchans_pad, cudaStream_t s);
+cudaError_t launch_tscrunch_bytes(int nbits, int k, const uint8_t *in, size_t in_beam_stride, size_t row_stride,
+                                  int nchans, int nbeams, long long nsamps_scr, uint8_t *out, cudaStream_t s);
 dedisp_status bitslice_prepare(dedisp_plan plan);   // called at the end of set_dm_list
 void bitslice_release(dedisp_plan plan);
 // returns DEDISP_OK, or DEDISP_ERR_INVALID_ARG when the plan cannot use this kernel
+// tscrunch = 1: plain; 2/4/8/16: the pre-pass sums blocks of tscrunch samples (row_stride = fine row)
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
-                               int nbits, void *out, size_t out_beam_stride, int out_f32,
+                               int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
                                cudaStream_t s);
