@@ -30,7 +30,7 @@
 
 // ... and of the 8-bit kernel
 #ifndef BS8_NW
-#define BS8_NW 7
+#define BS8_NW 11
 #endif
 #ifndef BS8_W
 #define BS8_W 4
@@ -40,6 +40,12 @@
 #endif
 #ifndef BS8_NSTAGE
 #define BS8_NSTAGE 3
+#endif
+#ifndef BS8_NSPLIT
+#define BS8_NSPLIT 2
+#endif
+#ifndef BS8_WIN_S
+#define BS8_WIN_S 80
 #endif
 
 // ... and of the 4-bit kernel
@@ -55,6 +61,9 @@
 #ifndef BS4_NSTAGE
 #define BS4_NSTAGE 3
 #endif
+#ifndef BS4_NSPLIT
+#define BS4_NSPLIT 1
+#endif
 
 namespace bs {
 constexpr int LANES = 32;    // trial DMs per tile (one per lane)
@@ -63,9 +72,13 @@ constexpr int CH_PAD = 32;   // channels are padded to a multiple of this (>= ev
 // NB  input bit planes (= sample width)     NW  consumer warps per CTA
 // W   32-sample words per thread per tile   K   adder-tree depth: 2^(K+1) channels per stage
 // NP  accumulator bit planes (sums < 2^NP)  WIN_S / WIN_L  window words per (channel, plane)
-template <int NB_, int NW_, int W_, int K_, int NSTAGE_, int NP_, int WIN_S_, int WIN_L_>
+// NSPLIT  the NB planes of a chunk go through NSPLIT adder trees of NB/NSPLIT planes each (a sample
+//         is the sum of its bit fields): shorter-lived temporaries, so more warps fit the register file
+template <int NB_, int NW_, int W_, int K_, int NSTAGE_, int NP_, int WIN_S_, int WIN_L_, int NSPLIT_ = 1>
 struct Cfg {
     static constexpr int NB = NB_, NW = NW_, W = W_, K = K_, NSTAGE = NSTAGE_, NP = NP_;
+    static constexpr int NSPLIT = NSPLIT_, NBS = NB_ / NSPLIT_;
+    static_assert(NB_ % NSPLIT_ == 0, "plane subsets must be equal");
     static constexpr int WIN_S = WIN_S_, WIN_L = WIN_L_;
     static constexpr int TILE_WORDS = NW * W;
     static constexpr int TILE_SAMPS = TILE_WORDS * 32;
@@ -77,16 +90,20 @@ struct Cfg {
 };
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
 using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
-// 8-bit samples: 7 x 4 words = 896-sample tiles, 16-channel trees, sums < 2^20
-// (sweep on B200, wide8: (NW,W,K,NSTAGE) = (14,2,2,3) 81.6 ms, (7,4,2,3) 75.0, (6,4,2,3) 85.8,
-//  (12,2,3,3) 91.5, (10,2,3,3) 101.9, (7,4,3,3) 74.5, (6,4,3,3) 84.9)
-using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, 64, 128>;
+// 8-bit samples: 11 x 4 words = 1408-sample tiles, 16-channel trees run once per nibble (NSPLIT = 2:
+// the temporaries of a 4-plane tree leave room for 11 consumer warps at 168 registers), sums < 2^20
+// (sweeps on B200, wide8, kernel ms.  One 8-plane tree, (NW,W,K,NSTAGE): (14,2,2,3) 81.6, (7,4,2,3) 75.0,
+//  (6,4,2,3) 85.8, (12,2,3,3) 91.5, (10,2,3,3) 101.9, (7,4,3,3) 74.5 [ALU pipe 69 % busy: 2 warps per
+//  sub-partition], (6,4,3,3) 84.9.  Split trees, (NSPLIT,NW,K,NSTAGE): (2,7,3,3) 73.7, (2,11,3,3) 60.7,
+//  (2,11,3,2) 59.3, (2,11,2,3) 62.7, (4,11,3,3) 62.6, (4,15,3,3) 67.1, (8,15,3,3) 78.5, (8,11,3,3) 77.5;
+//  window 80 instead of 128 words: 59.2 for 2, 3 or 4 stages)
+using Cfg8 = Cfg<8, BS8_NW, BS8_W, BS8_TREE_K, BS8_NSTAGE, 20, BS8_WIN_S, 128, BS8_NSPLIT>;
 // 1-bit samples (row f4): the packed row IS the bit plane; sums <= 4096 need 13 planes
 using Cfg1 = Cfg<1, 15, 4, 4, 3, 13, 96, 224>;
 // 4-bit samples (row f4): 11 x 4 words = 1408-sample tiles, 16-channel trees, sums < 2^16
 // (sweep on B200, gulp at 4 bits: (NW,W,K,NSTAGE) = (10,4,2,3) 2.88 ms, (10,4,3,3) 2.62, (10,4,4,3) 2.53,
 //  (11,4,3,3) 2.43, (9,4,3,3) 2.79, (12,3,2,3) 2.88, (14,2,3,3) 3.27)
-using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224>;
+using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224, BS4_NSPLIT>;
 
 // 3-, 5- and 6-plane samples exist only as time-scrunched sums (row f4, reading R38:
 // k samples of 1/2/4 bits added by the pre-pass): sums < 2^13 / 2^16 / 2^16
@@ -139,5 +156,6 @@ struct BitsliceParams {
     int ngroups;
     int ntiles;                // time tiles per (beam, group)
     int nbeams;
+    int gblock;                // work-item order: blocks of gblock DM groups, inside a block tile-major
     int vec_ok;                // output rows are 16-byte aligned: 128-bit stores allowed
 };

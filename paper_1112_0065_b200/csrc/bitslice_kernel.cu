@@ -14,6 +14,8 @@
 //     (2 LOP3 per full adder) into a 12-plane bit-sliced counter held in registers
 //     -- 32 additions per instruction, ~0.2 ALU ops per (channel, DM, sample);
 //   * the counter is un-sliced once per tile and written as uint32 / float32.
+#include <cmath>
+
 #include "bitslice_common.cuh"
 #include "dedisp_internal.h"
 
@@ -81,14 +83,14 @@ struct Stage {
 
 // Load the W+1 words of every plane of channel CI that this thread's W output words
 // need, and align them to the output time axis (one funnel shift per plane-word).
-template <class C, int CI, int WIN>
+template <class C, int CI, int WIN, int P0>
 __device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *relp,
-                                             uint32_t (&x)[C::NB][C::W])
+                                             uint32_t (&x)[C::NBS][C::W])
 {
     const uint32_t r = relp[CI * LANES];
-    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (C::NB * WIN);
+    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (C::NB * WIN) + P0 * WIN;
 #pragma unroll
-    for (int p = 0; p < C::NB; ++p) {
+    for (int p = 0; p < C::NBS; ++p) {
         uint32_t w[C::W + 1];
 #pragma unroll
         for (int j = 0; j <= C::W; ++j) w[j] = wp[p * WIN + j];
@@ -97,36 +99,78 @@ __device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *
     }
 }
 
-// Tree<K> adds 2^(K+1) channels (C0 ...) into counter planes 0 .. K+NB-1 and hands
-// back NB carry words e[i] of weight 2^(K+1+i): carry-save all the way, no ripple.
-template <class C, int K, int C0, int WIN>
+// Tree<K> adds planes P0 .. P0+NBS-1 of 2^(K+1) channels (C0 ...) into counter planes P0 .. P0+K+NBS-1 and
+// hands back NBS carry words e[i] of weight 2^(P0+K+1+i): carry-save all the way, no ripple.
+template <class C, int K, int C0, int WIN, int P0>
 struct Tree {
     static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&e)[C::NB][C::W])
+                                               const uint32_t *relp, uint32_t (&e)[C::NBS][C::W])
     {
-        uint32_t e1[C::NB][C::W], e2[C::NB][C::W];
-        Tree<C, K - 1, C0, WIN>::run(A, tb, relp, e1);
-        Tree<C, K - 1, C0 + (1 << K), WIN>::run(A, tb, relp, e2);
+        uint32_t e1[C::NBS][C::W], e2[C::NBS][C::W];
+        Tree<C, K - 1, C0, WIN, P0>::run(A, tb, relp, e1);
+        Tree<C, K - 1, C0 + (1 << K), WIN, P0>::run(A, tb, relp, e2);
 #pragma unroll
-        for (int i = 0; i < C::NB; ++i)
+        for (int i = 0; i < C::NBS; ++i)
 #pragma unroll
-            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[K + i][j], e1[i][j], e2[i][j]);
+            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[P0 + K + i][j], e1[i][j], e2[i][j]);
     }
 };
-template <class C, int C0, int WIN>
-struct Tree<C, 0, C0, WIN> {
+template <class C, int C0, int WIN, int P0>
+struct Tree<C, 0, C0, WIN, P0> {
     static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&e)[C::NB][C::W])
+                                               const uint32_t *relp, uint32_t (&e)[C::NBS][C::W])
     {
-        uint32_t x0[C::NB][C::W], x1[C::NB][C::W];
-        load_aligned<C, C0, WIN>(tb, relp, x0);
-        load_aligned<C, C0 + 1, WIN>(tb, relp, x1);
+        uint32_t x0[C::NBS][C::W], x1[C::NBS][C::W];
+        load_aligned<C, C0, WIN, P0>(tb, relp, x0);
+        load_aligned<C, C0 + 1, WIN, P0>(tb, relp, x1);
 #pragma unroll
-        for (int i = 0; i < C::NB; ++i)   // bit i of both channels
+        for (int i = 0; i < C::NBS; ++i)   // bit P0 + i of both channels
 #pragma unroll
-            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[i][j], x0[i][j], x1[i][j]);
+            for (int j = 0; j < C::W; ++j) e[i][j] = full_add(A[P0 + i][j], x0[i][j], x1[i][j]);
     }
 };
+
+// One chunk of CH channels: the tree of plane subset S, its carry words rippled into the upper
+// planes, then the next subset.
+template <class C, int WIN, int S>
+__device__ __forceinline__ void add_chunk(uint32_t (&A)[C::NP][C::W], const uint8_t *tb, const uint32_t *relp)
+{
+    constexpr int P0 = S * C::NBS, B = P0 + C::K + 1, NBS = C::NBS, NP = C::NP, W = C::W;
+    uint32_t e[NBS][W];
+    Tree<C, C::K, 0, WIN, P0>::run(A, tb, relp, e);
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        uint32_t c = A[B][j] & e[0][j];
+        A[B][j] ^= e[0][j];
+#pragma unroll
+        for (int i = 1; i < NBS; ++i) c = full_add(A[B + i][j], e[i][j], c);
+#pragma unroll
+        for (int p = B + NBS; p < NP - 1; ++p) {
+            const uint32_t t = A[p][j] & c;
+            A[p][j] ^= c;
+            c = t;
+        }
+        if (B + NBS < NP) A[NP - 1][j] ^= c;
+    }
+    if constexpr (S + 1 < C::NSPLIT) add_chunk<C, WIN, S + 1>(A, tb, relp);
+}
+
+// Work-item order (P.gblock): blocks of gblock DM groups; inside a block consecutive items are the
+// groups of one time tile, so CTAs running at the same time stage overlapping windows of the planes
+// (L2 hits) when the planes do not fit L2.  gblock = 1: consecutive items = consecutive tiles of a group.
+__device__ __forceinline__ void item_coords(const BitsliceParams &P, long long item, int &beam, int &g, int &tile)
+{
+    const long long per_beam = (long long)P.ngroups * P.ntiles;
+    beam = (int)(item / per_beam);
+    const long long r = item - (long long)beam * per_beam;
+    const long long per_blk = (long long)P.gblock * P.ntiles;
+    const int blk = (int)(r / per_blk);
+    const int g0 = blk * P.gblock;
+    const int gb = P.ngroups - g0 < P.gblock ? P.ngroups - g0 : P.gblock;
+    const int rr = (int)(r - (long long)blk * per_blk);
+    tile = rr / gb;
+    g = g0 + rr - tile * gb;
+}
 
 // Transpose step of the un-slice: rows a (index i, i & s == 0) and b (index i + s)
 // exchange the bit blocks (i, j | s) <-> (i + s, j).  m selects columns with j & s == 0.
@@ -218,9 +262,8 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
     if (warp == NW) {
         // ---------------- producer warp: TMA bulk copies into the ring ----------------
         for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
-            const int tile = (int)(item % P.ntiles);
-            const int g = (int)((item / P.ntiles) % P.ngroups);
-            const int beam = (int)(item / ((long long)P.ntiles * P.ngroups));
+            int beam, g, tile;
+            item_coords(P, item, beam, g, tile);
             const uint32_t *pl = P.planes + (size_t)beam * P.beam_pitch_words + (size_t)tile * C::TILE_WORDS;
             const size_t grow = (size_t)g * P.nchans_pad;
             for (int chunk = 0; chunk < nchunks; ++chunk) {
@@ -258,32 +301,15 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
             const uint8_t *sb = smem + stage * S::BYTES;
             const uint8_t *tb = sb + warp * (W * 4);
             const uint32_t *relp = reinterpret_cast<const uint32_t *>(sb + S::DATA_BYTES) + lane;
-            uint32_t e[NB][W];
-            Tree<C, C::K, 0, WIN>::run(A, tb, relp, e);
-            // add the NB carry words (weights 2^(K+1) ...) into the upper planes: ripple carry
-#pragma unroll
-            for (int j = 0; j < W; ++j) {
-                uint32_t c = A[C::K + 1][j] & e[0][j];
-                A[C::K + 1][j] ^= e[0][j];
-#pragma unroll
-                for (int i = 1; i < NB; ++i) c = full_add(A[C::K + 1 + i][j], e[i][j], c);
-#pragma unroll
-                for (int p = C::K + 1 + NB; p < NP - 1; ++p) {
-                    const uint32_t t = A[p][j] & c;
-                    A[p][j] ^= c;
-                    c = t;
-                }
-                if (C::K + 1 + NB < NP) A[NP - 1][j] ^= c;
-            }
+            add_chunk<C, WIN, 0>(A, tb, relp);
             __syncwarp();
             if (lane == 0) mbar_arrive(empty0 + 8 * stage);
             if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
         }
 
         // ---------------- epilogue: un-slice the counter, convert, store ----------------
-        const int tile = (int)(item % P.ntiles);
-        const int g = (int)((item / P.ntiles) % P.ngroups);
-        const int beam = (int)(item / ((long long)P.ntiles * P.ngroups));
+        int beam, g, tile;
+        item_coords(P, item, beam, g, tile);
         const int d = P.order[g * LANES + lane];
         uint8_t *orow = P.out + (size_t)beam * P.out_beam_stride +
                         (size_t)(d < 0 ? 0 : d) * (size_t)P.nsamps_out * 4;
@@ -365,6 +391,15 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     P.ngroups = G.ngroups;
     P.ntiles = (int)ntiles;
     P.nbeams = nbeams;
+    // planes that fit L2 (126 MB) are re-read from it in any order; larger ones (8-bit wideband:
+    // 750 MB) are walked tile-major inside blocks of gblock groups: gblock^2 ~ SMs x tile words x
+    // groups / (max_delay / 32) balances the tiles in flight against the delay spread of a block
+    P.gblock = 1;
+    if (beam_pitch * 4 > (size_t)64 << 20) {
+        const double spread = (double)(plan->max_delay >> 5) + 1.0;
+        int gb = (int)std::sqrt((double)sms * C::TILE_WORDS * G.ngroups / spread);
+        P.gblock = gb < 1 ? 1 : gb > G.ngroups ? G.ngroups : gb;
+    }
     P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
                (nbeams == 1 || out_beam_stride % 16 == 0);
     const long long nitems = (long long)nbeams * G.ngroups * ntiles;
