@@ -27,6 +27,12 @@
 #ifndef BS_NSTAGE
 #define BS_NSTAGE 3
 #endif
+#ifndef BS_NSPLIT
+#define BS_NSPLIT 1
+#endif
+#ifndef BS6_NSPLIT
+#define BS6_NSPLIT 2
+#endif
 
 // ... and of the 8-bit kernel
 #ifndef BS8_NW
@@ -89,7 +95,7 @@ struct Cfg {
     static_assert(NB + K + 1 <= NP, "tree carries must fit the accumulator");
 };
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
-using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224>;
+using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224, BS_NSPLIT>;
 // 8-bit samples: 11 x 4 words = 1408-sample tiles, 16-channel trees run once per nibble (NSPLIT = 2:
 // the temporaries of a 4-plane tree leave room for 11 consumer warps at 168 registers), sums < 2^20
 // (sweeps on B200, wide8, kernel ms.  One 8-plane tree, (NW,W,K,NSTAGE): (14,2,2,3) 81.6, (7,4,2,3) 75.0,
@@ -128,7 +134,7 @@ using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224, BS4_NSPL
 #endif
 using Cfg3 = Cfg<3, BS3_NW, 4, BS3_TREE_K, 3, 13, 96, 224>;
 using Cfg5 = Cfg<5, BS5_NW, 4, BS5_TREE_K, 3, 16, 96, 224>;
-using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160>;
+using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160, BS6_NSPLIT>;
 
 constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8
 constexpr int geom_index(int nplanes) { return nplanes; }
@@ -153,7 +159,8 @@ struct BitsliceParams {
     long long nsamps_out;
     int row_pitch;             // words
     int nchans_pad;
-    int ngroups;
+    int ngroups;               // DM groups this launch covers ...
+    int g_begin;               // ... starting at this group of the sorted list
     int ntiles;                // time tiles per (beam, group)
     int nbeams;
     int gblock;                // work-item order: blocks of gblock DM groups, inside a block tile-major

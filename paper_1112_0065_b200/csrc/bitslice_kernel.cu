@@ -169,7 +169,7 @@ __device__ __forceinline__ void item_coords(const BitsliceParams &P, long long i
     const int gb = P.ngroups - g0 < P.gblock ? P.ngroups - g0 : P.gblock;
     const int rr = (int)(r - (long long)blk * per_blk);
     tile = rr / gb;
-    g = g0 + rr - tile * gb;
+    g = P.g_begin + g0 + rr - tile * gb;
 }
 
 // Transpose step of the un-slice: rows a (index i, i & s == 0) and b (index i + s)
@@ -344,7 +344,8 @@ cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s)
 template <class C>
 dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, long long nsamps_out,
                           const uint8_t *in, size_t row_stride, size_t in_beam_stride, int in_nbits,
-                          int tscrunch, void *out, size_t out_beam_stride, int out_f32, cudaStream_t s)
+                          int tscrunch, void *out, size_t out_beam_stride, int out_f32, cudaStream_t s,
+                          const BitsliceRange &range)
 {
     const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
     const long long pitch =
@@ -366,10 +367,10 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device));
 
     if (plan->timing) cudaEventRecord(plan->ev[0], s);
-    if (tscrunch == 1)
+    if (range.prepass && tscrunch == 1)
         DEDISP_CUDA_TRY(plan, launch_planes(C::NB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
                                             plan->d_planes, (int)pitch, G.nchans_pad, s));
-    else
+    else if (range.prepass)
         DEDISP_CUDA_TRY(plan, launch_planes_tscrunch(in_nbits, tscrunch, C::NB, in, in_beam_stride, row_stride,
                                                      plan->nchans, nbeams, plan->d_planes, (int)pitch,
                                                      G.nchans_pad, s));
@@ -388,7 +389,8 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     P.nsamps_out = nsamps_out;
     P.row_pitch = (int)pitch;
     P.nchans_pad = G.nchans_pad;
-    P.ngroups = G.ngroups;
+    P.ngroups = range.g_count > 0 ? range.g_count : G.ngroups;
+    P.g_begin = range.g_begin;
     P.ntiles = (int)ntiles;
     P.nbeams = nbeams;
     // planes that fit L2 (126 MB) are re-read from it in any order; larger ones (8-bit wideband:
@@ -398,11 +400,11 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     if (beam_pitch * 4 > (size_t)64 << 20) {
         const double spread = (double)(plan->max_delay >> 5) + 1.0;
         int gb = (int)std::sqrt((double)sms * C::TILE_WORDS * G.ngroups / spread);
-        P.gblock = gb < 1 ? 1 : gb > G.ngroups ? G.ngroups : gb;
+        P.gblock = gb < 1 ? 1 : gb > P.ngroups ? P.ngroups : gb;
     }
     P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
                (nbeams == 1 || out_beam_stride % 16 == 0);
-    const long long nitems = (long long)nbeams * G.ngroups * ntiles;
+    const long long nitems = (long long)nbeams * P.ngroups * ntiles;
     const int grid = (int)(nitems < sms ? nitems : sms);
     cudaError_t e;
     if (G.win_words == C::WIN_S)
@@ -423,8 +425,10 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
                                int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
-                               cudaStream_t s)
+                               cudaStream_t s, const BitsliceRange *range)
 {
+    const BitsliceRange full;
+    const BitsliceRange &rg = range ? *range : full;
     // bit planes per (block-summed) sample; a scrunch factor the pre-pass does not build is not served here
     const bool pow2 = tscrunch == 2 || tscrunch == 4 || tscrunch == 8 || tscrunch == 16;
     if (tscrunch != 1 && !(pow2 && nbits * tscrunch <= 32)) return DEDISP_ERR_INVALID_ARG;
@@ -433,9 +437,10 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     const BitsliceGeom &G = plan->geom[geom_index(np)];
     const long long maxsum = (long long)plan->nchans * tscrunch * ((1ll << nbits) - 1);
     if (!G.usable || maxsum >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
+    if (rg.g_begin < 0 || rg.g_count < 0 || rg.g_begin + rg.g_count > G.ngroups) return DEDISP_ERR_INVALID_ARG;
 #define BS_RUN(CFG)                                                                                   \
     return execute_cfg<CFG>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, nbits, tscrunch, \
-                            out, out_beam_stride, out_f32, s)
+                            out, out_beam_stride, out_f32, s, rg)
     switch (np) {
         case 1: BS_RUN(Cfg1);
         case 2: BS_RUN(Cfg2);
@@ -446,4 +451,12 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
         default: BS_RUN(Cfg8);
     }
 #undef BS_RUN
+}
+
+int bitslice_ngroups(dedisp_plan plan, int nbits)
+{
+    if (nbits < 1 || nbits >= NGEOM) return 0;
+    const BitsliceGeom &G = plan->geom[geom_index(nbits)];
+    const long long maxsum = (long long)plan->nchans * ((1ll << nbits) - 1);
+    return (G.usable && maxsum < (1ll << G.nplanes_acc)) ? G.ngroups : 0;
 }

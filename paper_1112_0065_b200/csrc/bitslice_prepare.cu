@@ -419,6 +419,8 @@ dedisp_status bitslice_prepare(dedisp_plan p)
     std::iota(sorted.begin(), sorted.begin() + ndm, 0);
     std::stable_sort(sorted.begin(), sorted.begin() + ndm,
                      [&](int a, int b) { return p->dms[a] < p->dms[b]; });
+    p->order_identity = true;
+    for (int i = 0; i < ndm; ++i) p->order_identity = p->order_identity && sorted[i] == i;
     int *d_max = nullptr;
     const size_t nrows = (size_t)ngroups * nchans_pad;
     cudaError_t e = cudaMalloc(&p->d_order, sizeof(int32_t) * ndm_pad);

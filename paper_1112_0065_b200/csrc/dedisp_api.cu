@@ -224,6 +224,60 @@ dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps
     }
     cudaStream_t s = plan->host_stream;
     DEDISP_CUDA_TRY(plan, cudaMemcpyAsync(plan->d_in_stage, in_host, in_bytes, cudaMemcpyHostToDevice, s));
+    // The result (out_bytes) dominates the transfer time, so it leaves in pieces while the kernel is
+    // still running: one beam at a time, or -- single beam, trial DMs given in ascending order, so that
+    // a range of DM groups is a range of output rows -- one range of DM groups at a time.  Each piece is
+    // copied on a second stream as soon as its kernel has finished.
+    const int ngroups = plan->want == DEDISP_KERNEL_DIRECT ? 0 : bitslice_ngroups(plan, in_nbits);
+    const bool by_beam = ngroups > 0 && nbeams > 1;
+    const bool by_range = ngroups >= 2 && nbeams == 1 && plan->order_identity;
+    if (by_beam || by_range) {
+        dedisp_status chk = check_exec_args(plan, nbeams, nsamps_out, plan->d_in_stage, in_nbits, plan->d_out_stage,
+                                            out_dtype);
+        if (chk != DEDISP_OK) return chk;
+        constexpr int NEV = (int)(sizeof(plan->chunk_ev) / sizeof(plan->chunk_ev[0]));
+        if (!plan->copy_stream)
+            DEDISP_CUDA_TRY(plan, cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < NEV; ++i)
+            if (!plan->chunk_ev[i])
+                DEDISP_CUDA_TRY(plan, cudaEventCreateWithFlags(&plan->chunk_ev[i], cudaEventDisableTiming));
+        const int f32 = (out_dtype == DEDISP_OUT_F32);
+        const int nchunks = by_beam ? nbeams : (ngroups < 8 ? ngroups : 8);
+        const size_t row_bytes = (size_t)nsamps_out * 4;
+        for (int c = 0; c < nchunks; ++c) {
+            size_t off, bytes;
+            dedisp_status st;
+            if (by_beam) {
+                off = (size_t)c * out_beam;
+                bytes = out_beam;
+                st = bitslice_execute(plan, 1, nsamps_out, (const uint8_t *)plan->d_in_stage + (size_t)c * in_beam,
+                                      row, 0, in_nbits, 1, (uint8_t *)plan->d_out_stage + off, 0, f32, s);
+            } else {
+                BitsliceRange rg;
+                rg.g_begin = (int)((long long)ngroups * c / nchunks);
+                rg.g_count = (int)((long long)ngroups * (c + 1) / nchunks) - rg.g_begin;
+                rg.prepass = (c == 0);
+                const long long d0 = 32ll * rg.g_begin;
+                long long d1 = d0 + 32ll * rg.g_count;
+                if (d1 > plan->ndm) d1 = plan->ndm;
+                off = (size_t)d0 * row_bytes;
+                bytes = (size_t)(d1 - d0) * row_bytes;
+                st = bitslice_execute(plan, 1, nsamps_out, (const uint8_t *)plan->d_in_stage, row, 0, in_nbits, 1,
+                                      plan->d_out_stage, 0, f32, s, &rg);
+            }
+            if (st != DEDISP_OK) return st;
+            cudaEvent_t ev = plan->chunk_ev[c % NEV];
+            if (c >= NEV) DEDISP_CUDA_TRY(plan, cudaEventSynchronize(ev));   // its earlier use has been consumed
+            DEDISP_CUDA_TRY(plan, cudaEventRecord(ev, s));
+            DEDISP_CUDA_TRY(plan, cudaStreamWaitEvent(plan->copy_stream, ev, 0));
+            DEDISP_CUDA_TRY(plan, cudaMemcpyAsync((uint8_t *)out_host + off, (uint8_t *)plan->d_out_stage + off, bytes,
+                                                  cudaMemcpyDeviceToHost, plan->copy_stream));
+        }
+        plan->last_kernel = DEDISP_KERNEL_BITSLICE;
+        DEDISP_CUDA_TRY(plan, cudaStreamSynchronize(s));
+        DEDISP_CUDA_TRY(plan, cudaStreamSynchronize(plan->copy_stream));
+        return DEDISP_OK;
+    }
     dedisp_status st = dedisp_execute_batch(plan, nbeams, nsamps_out, plan->d_in_stage, in_beam,
                                             in_nbits, plan->d_out_stage, out_beam, out_dtype, s);
     if (st != DEDISP_OK) return st;
@@ -240,6 +294,9 @@ dedisp_status dedisp_destroy(dedisp_plan plan)
     cudaFree(plan->d_in_stage);
     cudaFree(plan->d_out_stage);
     if (plan->host_stream) cudaStreamDestroy(plan->host_stream);
+    if (plan->copy_stream) cudaStreamDestroy(plan->copy_stream);
+    for (cudaEvent_t e : plan->chunk_ev)
+        if (e) cudaEventDestroy(e);
     for (int i = 0; i < 4; ++i)
         if (plan->ev[i]) cudaEventDestroy(plan->ev[i]);
     delete plan;

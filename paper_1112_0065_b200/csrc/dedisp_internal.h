@@ -43,6 +43,9 @@ struct dedisp_plan_s {
     void *d_out_stage = nullptr;
     size_t out_stage_bytes = 0;
     cudaStream_t host_stream = nullptr;
+    cudaStream_t copy_stream = nullptr;   // device->host copies of finished DM ranges / beams
+    cudaEvent_t chunk_ev[16] = {};
+    bool order_identity = false;          // trial DMs were given in ascending order: sorted lane = output row
     // optional per-kernel timing: ev[0..1] around the pre-pass, ev[2..3] around the main kernel
     bool timing = false;
     bool timing_valid = false;
@@ -86,7 +89,16 @@ dedisp_status bitslice_prepare(dedisp_plan plan);   // called at the end of set_
 void bitslice_release(dedisp_plan plan);
 // returns DEDISP_OK, or DEDISP_ERR_INVALID_ARG when the plan cannot use this kernel
 // tscrunch = 1: plain; 2/4/8/16: the pre-pass sums blocks of tscrunch samples (row_stride = fine row)
+// range (optional): only DM groups [g_begin, g_begin + g_count) of the sorted list; prepass = false
+// re-uses the bit planes a previous call on this plan left in the scratch (same input, same shape)
+struct BitsliceRange {
+    int g_begin = 0;
+    int g_count = 0;      // 0 = all groups
+    bool prepass = true;
+};
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
                                int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
-                               cudaStream_t s);
+                               cudaStream_t s, const BitsliceRange *range = nullptr);
+// DM groups of the plan's bit-sliced geometry for this sample width, or 0 if the kernel cannot serve it
+int bitslice_ngroups(dedisp_plan plan, int nbits);

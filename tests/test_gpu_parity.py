@@ -210,6 +210,39 @@ def test_execute_host_end_to_end():
     dd.dedisp_destroy(p)
 
 
+@pytest.mark.parametrize("order", ["ascending", "shuffled", "direct"])
+@pytest.mark.parametrize("ndm", [1, 33, 330, 1000])
+def test_execute_host_single_beam_pieces(order, ndm):
+    # one beam: ascending DM lists leave in up to 8 ranges of DM groups (copy overlapped with the kernel);
+    # any other list, or the DIRECT kernel, takes the one-piece path.  All must equal the oracle.
+    w = W.CONFIGS["htru_gulp"].scaled(nchans=64, ndm=ndm, nsamps_out=3001, df=-6.0, dm_hi=250.0)
+    dms = w.dms()
+    if order == "shuffled":
+        dms = np.random.default_rng(ndm).permutation(dms)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, dms)
+    x = W.generate(w, md)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, dms,
+                  kernel=dd.DEDISP_KERNEL_DIRECT if order == "direct" else dd.DEDISP_KERNEL_AUTO)
+    out = torch.full((ndm, w.nsamps_out), -1, dtype=torch.int32).pin_memory()
+    for _ in range(2):      # the second call re-uses the staging buffers, streams and events
+        out.fill_(-1)
+        dd.dedisp_execute_host(p, 1, w.nsamps_out, torch.from_numpy(x).pin_memory(), 2, out, dd.DEDISP_OUT_U32)
+        assert np.array_equal(out.numpy().view(np.uint32), oracle.dedisperse(delay, x, 2, w.nsamps_out))
+    dd.dedisp_destroy(p)
+
+
+def test_execute_host_many_beams():
+    # more beams than the plan holds events for (16): one piece per beam
+    w = W.CONFIGS["beams13"].scaled(nchans=32, ndm=40, nsamps_out=700, df=-12.0, dm_hi=100.0, nbeams=19)
+    delay, md, x = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    out = torch.empty((19, w.ndm, w.nsamps_out), dtype=torch.float32).pin_memory()
+    dd.dedisp_execute_host(p, 19, w.nsamps_out, torch.from_numpy(x).pin_memory(), 2, out, dd.DEDISP_OUT_F32)
+    for b in range(19):
+        assert np.array_equal(out[b].numpy(), oracle.to_f32(oracle.dedisperse(delay, x[b], 2, w.nsamps_out)))
+    dd.dedisp_destroy(p)
+
+
 def test_execute_errors():
     p = make_plan(8, 64e-6, 1500.0, -10.0, [0.0, 10.0])
     x = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
