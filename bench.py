@@ -338,6 +338,8 @@ def run_matched_filter(args) -> None:
 
     if args.op == "find_events":
         return _bench_find_events(args, dd, torch, w, widths, z, step, flush, stream)
+    if args.op == "search":
+        return _bench_search(args, dd, torch, w, widths, radius, x_max, x, z, flush, stream)
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -476,6 +478,78 @@ def _bench_find_events(args, dd, torch, w, widths, z, make_z, flush, stream) -> 
                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
            "cpu_baseline": cpu,
            "e2e": {"value": ns * n / e2e_s, "unit": "searched samples/s", "h2d_bytes_per_step": z.numel() * 4,
+                   "d2h_bytes_per_step": k * 20 + 8, "steps": 1},
+           "gpu_launches": launches, "clocks": clocks,
+           "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
+    print(json.dumps(res), flush=True)
+
+
+def _bench_search(args, dd, torch, w, widths, radius, x_max, x, z, flush, stream) -> None:
+    """--op search: rows f1 + f2 chained on the dedispersed output of --config.  A step =
+    dedisp_matched_filter_rms (z and the RMS of every filtered series in one pass over x) +
+    dedisp_find_events at 6 sigma: x read once, z written once and read once, the bit mask written and read."""
+    dev = x.device
+    nw, nrows, n = z.shape
+    ns = nw * nrows
+    nsigma, cap = 6.0, 1 << 20
+    wsb = dd.dedisp_find_events_workspace_bytes(ns, n)
+    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+    mwb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, nw)
+    mws = torch.empty(mwb, dtype=torch.uint8, device=dev)
+    rms = torch.empty(ns, dtype=torch.float32, device=dev)
+    ev = torch.empty((cap, 5), dtype=torch.int32, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def step():
+        dd.dedisp_matched_filter_rms(x, dd.DEDISP_OUT_U32, nrows, n, radius, widths, x_max, z, rms, mws, mwb,
+                                     stream.cuda_stream)
+        dd.dedisp_find_events(z, ns, n, rms, nsigma, ws, wsb, ev, cap, cnt, stream.cuda_stream)
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = dd.dedisp_get_launch_count()
+    step_ms = _time_steps(torch, step, flush, stream, args.warmup, args.steps)
+    launches = (dd.dedisp_get_launch_count() - launches0) * args.steps // (args.steps + args.warmup)
+    clocks = sampler.stop()
+    ms = statistics.mean(step_ms)
+    found = int(cnt.item())
+    hx = x.cpu().pin_memory()
+    hev = torch.empty((cap, 5), dtype=torch.int32).pin_memory()
+    t0 = time.perf_counter()
+    x.copy_(hx, non_blocking=True)
+    step()
+    k = min(int(cnt.item()), cap)
+    hev[:k].copy_(ev[:k], non_blocking=True)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    alg_bytes = x.numel() * 4 + 2 * z.numel() * 4 + 2 * (z.numel() // 8)
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import matched_filter as MF, peak_finding as PF
+        rows = x[:: max(1, nrows // 24)].cpu().numpy().view(np.uint32)
+        t0 = time.perf_counter()
+        zz = MF.matched_filter(rows, radius, widths).astype(np.float32).reshape(-1, n)
+        PF.find_events(zz, PF.series_rms(zz).astype(np.float32), nsigma)
+        dt = time.perf_counter() - t0
+        cpu = {"value": zz.size / dt, "unit": "searched samples/s", "cores": 1, "kind": "oracle",
+               "sample": f"{rows.shape[0]} of {nrows} rows x {n} samples x {nw} widths "
+                         f"(matched filter + rms + find_events), {dt:.2f} s"}
+    res = {"metric": "filtered and searched samples/sec", "value": ns * n / (ms * 1e-3), "unit": "searched samples/s",
+           "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "exact int -> f32",
+           "data": "synthetic",
+           "config": {"workload": f"matched_filter_rms + find_events on dedispersed {w.name}", "nrows": nrows,
+                      "nsamps": n, "widths": widths, "radius": radius, "nsigma": nsigma, "events_found": found,
+                      "l2": "256 MiB flush buffer zeroed between timed iterations"},
+           "roofline": {"bound": "hbm", "achieved": alg_bytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": ncu_traffic_bytes("search_" + w.name),
+                        "kernel": "matched_filter_kernel + sigma_cut_kernel (+ 4 small kernels)", "kernel_ms": ms,
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
+           "cpu_baseline": cpu,
+           "e2e": {"value": ns * n / e2e_s, "unit": "searched samples/s", "h2d_bytes_per_step": x.numel() * 4,
                    "d2h_bytes_per_step": k * 20 + 8, "steps": 1},
            "gpu_launches": launches, "clocks": clocks,
            "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
@@ -654,14 +728,14 @@ def main():
     ap.add_argument("--tscrunch", type=int, default=1,
                     help="--op dedisperse only: sum blocks of K input samples and dedisperse on the grid K*dt "
                          "(row f4; the input then holds K x as many samples per output sample)")
-    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events", "rfi_mask", "transpose"],
+    ap.add_argument("--op", default="dedisperse", choices=["dedisperse", "matched_filter", "find_events", "search", "rfi_mask", "transpose"],
                     help="dedisperse = the hot path (default, the metric BASELINE.json names); "
-                         "matched_filter = row f1 downstream of it; find_events = row f2 downstream of f1; rfi_mask = row f3; transpose = row f4")
+                         "matched_filter = row f1 downstream of it; find_events = row f2 downstream of f1; search = f1 + f2 chained (matched_filter_rms + find_events); rfi_mask = row f3; transpose = row f4")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
-    elif args.op in ("matched_filter", "find_events"):
+    elif args.op in ("matched_filter", "find_events", "search"):
         run_matched_filter(args)
     elif args.op in ("rfi_mask", "transpose"):
         run_small_op(args)

@@ -201,6 +201,23 @@ dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
                                     int nwidths, unsigned int x_max, float *z_dev,
                                     void *cuda_stream);
 
+/* dedisp_matched_filter that also returns the noise level of every filtered series, so that the
+ * sigma-cut of dedisp_find_events needs no extra pass over z (reading R28):
+ *     rms_dev[iw*nrows + r] = float32( sqrt( (1/nsamps) * sum_t z_w[r][t]^2 ) )
+ * -- what dedisp_series_rms returns for the same series, up to summation order: z^2 is summed in float32
+ * over the <= 64 outputs a thread writes per (width, 16 384-sample segment), then in float64 in a fixed
+ * order (deterministic); relative difference to the float64 definition < 2^-20.
+ *   rms_dev        DEVICE float32 [nwidths*nrows], 4-byte aligned, written completely.
+ *   workspace_dev  DEVICE scratch, 8-byte aligned, >= dedisp_matched_filter_rms_workspace_bytes();
+ *                  owned by the caller, free to reuse once the call's work has completed.
+ * Other arguments, layouts and errors as dedisp_matched_filter; a null rms_dev, a null, misaligned
+ * or too small workspace: INVALID_ARG.  Only enqueues work on cuda_stream (2 kernels). */
+size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths);
+dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
+                                        long long nsamps, int radius, const int *widths_host,
+                                        int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
+                                        void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
 /* ---- peak finding ---- */
 
 /* One detected event: a maximal run of consecutive samples of one series above threshold. */

@@ -55,6 +55,9 @@ ABI = {
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
     "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
     "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
+    "dedisp_matched_filter_rms_workspace_bytes": (_sz, [_ll, _ll, _i]),
+    "dedisp_matched_filter_rms": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp, _vp, _sz,
+                                       _vp]),
     "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
     "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
@@ -224,6 +227,22 @@ def dedisp_matched_filter(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: 
     st = lib().dedisp_matched_filter(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths),
                                      x_max, _ptr(z_ptr), stream or None)
     _check(None, st, "dedisp_matched_filter")
+
+
+def dedisp_matched_filter_rms_workspace_bytes(nrows: int, nsamps: int, nwidths: int) -> int:
+    return int(lib().dedisp_matched_filter_rms_workspace_bytes(nrows, nsamps, nwidths))
+
+
+def dedisp_matched_filter_rms(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: int, widths,
+                              x_max: int, z_ptr, rms_ptr, workspace_ptr, workspace_bytes: int,
+                              stream: int = 0) -> None:
+    """dedisp_matched_filter + the RMS of every filtered series in the same pass (include/dedisp.h)."""
+    w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
+    st = lib().dedisp_matched_filter_rms(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths), x_max,
+                                         _ptr(z_ptr), _ptr(rms_ptr) if rms_ptr is not None else None,
+                                         _ptr(workspace_ptr) if workspace_ptr is not None else None,
+                                         workspace_bytes, stream or None)
+    _check(None, st, "dedisp_matched_filter_rms")
 
 
 def dedisp_find_events_workspace_bytes(nseries: int, nsamps: int) -> int:

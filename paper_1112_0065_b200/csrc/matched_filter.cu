@@ -45,6 +45,7 @@ struct MFParams {
     int guard_hist;              // mask of the step flags the outputs of one step depend on
     int w[MAXW];
     float scale[MAXW];           // fl32(1 / (N sqrt(w)))
+    double *partial;             // RMS variant: [nw][nrows][nseg] sums of z^2 over a segment
 };
 
 // inclusive block scan of one value per thread; returns the thread's inclusive prefix and
@@ -110,7 +111,10 @@ template <> struct Vec8<unsigned long long> {
 // it.  Every step flags |NY| > (2^31-1)/wmax block-wide; outputs that depend on a flagged
 // step are summed sample by sample in 64 bits from NY[t] = P[t+1]-P[t] (exact, slow, never
 // taken on noise-like data), all others use the 32-bit differences, which are then exact.
-template <class ACC, bool XF32, bool GUARD>
+// RMS: the kernel also accumulates sum z^2 per (width, row, segment) -- float32 per thread over the
+// <= 64 outputs it writes per width and segment, then float64 across the block in a fixed order --
+// so that the noise level of every filtered series is known without reading z back.
+template <class ACC, bool XF32, bool GUARD, bool RMS>
 __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
 {
     static_assert(!GUARD || sizeof(ACC) == 4, "the guard belongs to the 32-bit path");
@@ -124,6 +128,9 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
     ACC *sc = reinterpret_cast<ACC *>(sD + E);                      // [NT/32]
     ACC *ring = sc + NT / 32;                                       // [2*ring] slot i (and i+ring) holds P[i+1]
     const int RING = P.ring;                                        // multiple of 8, >= E + wmax + 1
+    float *sAcc = reinterpret_cast<float *>(ring + (MIRROR ? 2 : 1) * RING);   // RMS: [nw][NT]
+    if (RMS)
+        for (int iw = 0; iw < P.nw; ++iw) sAcc[iw * NT + threadIdx.x] = 0.f;
 
     const long long row = blockIdx.x / P.nseg;
     const int seg = (int)(blockIdx.x % P.nseg);
@@ -263,6 +270,7 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;
+                float ss = 0.f;
 #pragma unroll 1
                 for (int k = 0; k < V; ++k) {
                     const int o = ob + k * NT;
@@ -279,25 +287,33 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
                             prev = cur;
                         }
                     }
-                    __stcs(zp + k * NT, (float)zz * scl);
+                    const float z = (float)zz * scl;
+                    if (RMS) ss += z * z;
+                    __stcs(zp + k * NT, z);
                 }
+                if (RMS) sAcc[iw * NT + j] += ss;
             }
         } else if (interior) {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
+                float ss = 0.f;
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     int sl = rs[k] + w;
                     if (!MIRROR && sl >= RING) sl -= RING;
-                    __stcs(zp + k * NT, acc_to_float((ACC)(ring[sl] - p0[k])) * scl);
+                    const float z = acc_to_float((ACC)(ring[sl] - p0[k])) * scl;
+                    if (RMS) ss += z * z;
+                    __stcs(zp + k * NT, z);
                 }
+                if (RMS) sAcc[iw * NT + j] += ss;
             }
         } else {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;                 // t + w <= n  <=>  o <= lim
+                float ss = 0.f;
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     const int o = ob + k * NT;
@@ -305,9 +321,11 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
                         int sl = rs[k] + w;
                         if (!MIRROR && sl >= RING) sl -= RING;
                         const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
+                        if (RMS) ss += z * z;
                         __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
                     }
                 }
+                if (RMS) sAcc[iw * NT + j] += ss;
             }
         }
         wslot += E;
@@ -316,14 +334,51 @@ __global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
         if (rslot >= RING) rslot -= RING;
         __syncthreads();
     }
+    if (RMS) {
+        // block sum per width in float64, fixed order: lanes by shuffle, then the 8 warp sums in sequence
+        double *sw = reinterpret_cast<double *>(sX);      // sX is free now: [NT/32] doubles
+        for (int iw = 0; iw < P.nw; ++iw) {
+            double v = (double)sAcc[iw * NT + j];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+            if ((j & 31) == 0) sw[j >> 5] = v;
+            __syncthreads();
+            if (j == 0) {
+                double t = 0.0;
+                for (int q = 0; q < NT / 32; ++q) t += sw[q];
+                P.partial[((size_t)iw * (size_t)P.nrows + (size_t)row) * P.nseg + seg] = t;
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// rms[s] = fl32( sqrt( (sum of the nseg partials of series s, in order) / n ) )
+__global__ void mf_rms_finish_kernel(const double *__restrict__ partial, long long nseries, int nseg, long long n,
+                                     float *__restrict__ rms)
+{
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nseries) return;
+    double t = 0.0;
+    for (int q = 0; q < nseg; ++q) t += partial[s * nseg + q];
+    rms[s] = (float)sqrt(t / (double)n);
 }
 
 }  // namespace
 
-extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
-                                               long long nrows, long long nsamps, int radius,
-                                               const int *widths_host, int nwidths,
-                                               unsigned int x_max, float *z_dev, void *cuda_stream)
+namespace {
+long long mf_segment(long long nsamps)
+{
+    // segments: about 8 steps each, so that the grid is many waves deep
+    long long seg = 8ll * E;
+    if (seg > nsamps) seg = (nsamps + E - 1) / E * E;
+    return seg;
+}
+}  // namespace
+
+static dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps, int radius,
+                            const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
+                            void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
 {
     if (!x_dev || !z_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0)
         return DEDISP_ERR_INVALID_ARG;
@@ -352,9 +407,7 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     for (int i = nwidths; i < MAXW; ++i) { P.w[i] = 1; P.scale[i] = 0.f; }
     const int ring = (E + P.wmax + 1 + 7) & ~7;
     P.ring = ring;
-    // segments: about 8 steps each, so that the grid is many waves deep
-    long long seg = 8ll * E;
-    if (seg > nsamps) seg = (nsamps + E - 1) / E * E;
+    const long long seg = mf_segment(nsamps);
     P.seg = (int)seg;
     const long long nseg = (nsamps + seg - 1) / seg;
     P.nseg = (int)nseg;
@@ -370,15 +423,28 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
     P.guard_lim = (int)(2147483647ll / P.wmax);
     P.guard_hist = (1 << ((P.wmax + E - 1) / E + 1)) - 1;
     const size_t accb = wide ? 8 : 4;
-    const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (wide ? 1 : 2) * (size_t)ring * accb;
+    const bool rms = rms_dev != nullptr;
+    P.partial = (double *)workspace_dev;
+    if (rms) {
+        if (!workspace_dev || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)rms_dev & 3u) ||
+            workspace_bytes < (size_t)nwidths * (size_t)nrows * (size_t)nseg * sizeof(double))
+            return DEDISP_ERR_INVALID_ARG;
+    }
+    const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (wide ? 1 : 2) * (size_t)ring * accb +
+                        (rms ? (size_t)nwidths * NT * 4 : 0);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
-#define MF_LAUNCH(ACC, F, G)                                                                     \
+#define MF_LAUNCH1(ACC, F, G, R)                                                                  \
     do {                                                                                         \
-        e = cudaFuncSetAttribute(matched_filter_kernel<ACC, F, G>,                               \
+        e = cudaFuncSetAttribute(matched_filter_kernel<ACC, F, G, R>,                            \
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
-        if (e == cudaSuccess) matched_filter_kernel<ACC, F, G><<<grid, block, smem, s>>>(P);     \
+        if (e == cudaSuccess) matched_filter_kernel<ACC, F, G, R><<<grid, block, smem, s>>>(P);  \
+    } while (0)
+#define MF_LAUNCH(ACC, F, G)                     \
+    do {                                         \
+        if (rms) MF_LAUNCH1(ACC, F, G, true);    \
+        else MF_LAUNCH1(ACC, F, G, false);       \
     } while (0)
     const bool f32 = (x_dtype == DEDISP_OUT_F32);
     if (wide) {
@@ -392,8 +458,41 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
         else MF_LAUNCH(uint32_t, false, false);
     }
 #undef MF_LAUNCH
+#undef MF_LAUNCH1
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return DEDISP_ERR_CUDA;
     ++g_launch_count;
+    if (rms) {
+        const long long nseries = (long long)nwidths * nrows;
+        mf_rms_finish_kernel<<<(unsigned)((nseries + 255) / 256), 256, 0, s>>>(P.partial, nseries, P.nseg, nsamps, rms_dev);
+        if (cudaGetLastError() != cudaSuccess) return DEDISP_ERR_CUDA;
+        ++g_launch_count;
+    }
     return DEDISP_OK;
+}
+
+extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
+                                               long long nrows, long long nsamps, int radius,
+                                               const int *widths_host, int nwidths,
+                                               unsigned int x_max, float *z_dev, void *cuda_stream)
+{
+    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, nullptr, nullptr, 0,
+                  cuda_stream);
+}
+
+extern "C" size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths)
+{
+    if (nrows < 1 || nsamps < 1 || nwidths < 1 || nwidths > MAXW) return 0;
+    const long long seg = mf_segment(nsamps);
+    return (size_t)nwidths * (size_t)nrows * (size_t)((nsamps + seg - 1) / seg) * sizeof(double);
+}
+
+extern "C" dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
+                                                   long long nsamps, int radius, const int *widths_host,
+                                                   int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
+                                                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!rms_dev) return DEDISP_ERR_INVALID_ARG;
+    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, rms_dev, workspace_dev,
+                  workspace_bytes, cuda_stream);
 }

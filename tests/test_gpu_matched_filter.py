@@ -148,3 +148,61 @@ def test_full_size_htru_gulp_sampled_rows():
     got = gpu_mf(x, R, widths, 3072)
     check(got[:, rows, :], MF.matched_filter(x[rows], R, widths))
     assert not np.isnan(got).any()
+
+
+# ---- dedisp_matched_filter_rms: the same z plus the RMS of every filtered series in one pass ----
+def gpu_mf_rms(x, radius, widths, x_max):
+    x = np.ascontiguousarray(x)
+    nrows, n = x.shape
+    xd = torch.from_numpy(x.view(np.int32)).cuda()
+    z = torch.full((len(widths), nrows, n), float("nan"), dtype=torch.float32, device="cuda")
+    rms = torch.full((len(widths) * nrows,), float("nan"), dtype=torch.float32, device="cuda")
+    nb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, len(widths))
+    assert nb > 0
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    dd.dedisp_matched_filter_rms(xd, dd.DEDISP_OUT_U32, nrows, n, radius, widths, x_max, z, rms, ws, nb,
+                                 torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return z.cpu().numpy(), rms.cpu().numpy().reshape(len(widths), nrows), z
+
+
+@pytest.mark.parametrize("shape,radius,widths,kw", [
+    ((5, 5000), 100, [1, 2, 4, 8, 16, 32, 64], {}),                       # one segment, 32-bit words
+    ((3, 40001), 700, [1, 3, 8, 50, 64], {}),                             # 3 segments, ragged tail
+    ((2, 65536), 15625, [1, 2, 4, 8, 16, 32, 64], {}),                    # 2 s window: guarded 32-bit words
+    ((2, 30000), 2000, [1, 2, 64, 512], dict(mean=524288.0, sigma=1024.0, x_max=1044480, wiggle=3000.0)),  # 64-bit
+])
+def test_fused_rms_equals_the_definition(shape, radius, widths, kw):
+    from oracle import peak_finding as PF
+    x = W.dedispersed_like(31, shape[0], shape[1], **kw)
+    x_max = kw.get("x_max", 3072)
+    want_z = MF.matched_filter(x, radius, widths)
+    z, rms, zd = gpu_mf_rms(x, radius, widths, x_max)
+    check(z, want_z)                                           # z is what dedisp_matched_filter writes
+    assert np.array_equal(z, gpu_mf(x, radius, widths, x_max))
+    # tolerance (include/dedisp.h): z within 2^-22 => z^2 within 2^-21; float32 partial sums of <= 64 squares
+    # and float64 above => sum within ~2^-19.4, its square root within 2^-20
+    want = PF.series_rms(want_z.reshape(-1, shape[1])).reshape(len(widths), shape[0])
+    np.testing.assert_allclose(rms.astype(np.float64), want, rtol=2.0 ** -20, atol=0)
+    # and against the stand-alone kernel on the z this call wrote
+    r2 = torch.empty(len(widths) * shape[0], dtype=torch.float32, device="cuda")
+    dd.dedisp_series_rms(zd, len(widths) * shape[0], shape[1], r2, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(rms.reshape(-1), r2.cpu().numpy(), rtol=2.0 ** -20, atol=0)
+
+
+def test_fused_rms_is_deterministic_and_checks_its_arguments():
+    x = W.dedispersed_like(32, 4, 33000)
+    _, a, _ = gpu_mf_rms(x, 300, [1, 4, 16], 3072)
+    _, b, _ = gpu_mf_rms(x, 300, [1, 4, 16], 3072)
+    assert np.array_equal(a, b)
+    xd = torch.from_numpy(x.view(np.int32)).cuda()
+    z = torch.empty((3, 4, 33000), dtype=torch.float32, device="cuda")
+    rms = torch.empty(12, dtype=torch.float32, device="cuda")
+    nb = dd.dedisp_matched_filter_rms_workspace_bytes(4, 33000, 3)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    for args in [(z, None, ws, nb), (z, rms, None, nb), (z, rms, ws, nb - 8)]:
+        with pytest.raises(dd.DedispError) as e:
+            dd.dedisp_matched_filter_rms(xd, dd.DEDISP_OUT_U32, 4, 33000, 300, [1, 4, 16], 3072, *args, 0)
+        assert e.value.status == dd.DEDISP_ERR_INVALID_ARG
+    assert dd.dedisp_matched_filter_rms_workspace_bytes(0, 10, 1) == 0
