@@ -163,6 +163,8 @@ struct BitsliceParams {
     int g_begin;               // ... starting at this group of the sorted list
     int ntiles;                // time tiles per (beam, group)
     int nbeams;
+    int chunk0, nchunks;       // channel chunks [chunk0, chunk0 + nchunks) of Cfg::CH channels are summed ...
+    int accumulate;            // ... and added to what out already holds (channel blocks, sums >= 2^NP)
     int gblock;                // work-item order: blocks of gblock DM groups, inside a block tile-major
     int vec_ok;                // output rows are 16-byte aligned: 128-bit stores allowed
 };

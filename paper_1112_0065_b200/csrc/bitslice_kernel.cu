@@ -194,7 +194,7 @@ __device__ __forceinline__ uint32_t cvt_out(uint32_t v)
 // NP > 16: a full 32x32 transpose.
 template <int NP, int W, bool F32>
 __device__ __forceinline__ void unslice_store(uint32_t (&A)[NP][W], int j, uint8_t *orow, long long t0,
-                                              long long nsamps_out, bool fast)
+                                              long long nsamps_out, bool fast, bool accumulate)
 {
     constexpr int R = (NP <= 16) ? 16 : 32;
     uint32_t M[R];
@@ -219,10 +219,29 @@ __device__ __forceinline__ void unslice_store(uint32_t (&A)[NP][W], int j, uint8
     uint32_t o[32];
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
-        uint32_t v;
-        if (R == 32) v = M[i];
-        else v = (i < 16) ? (M[i] & 0xFFFFu) : (M[i - 16] >> 16);
-        o[i] = cvt_out<F32>(v);
+        if (R == 32) o[i] = M[i];
+        else o[i] = (i < 16) ? (M[i] & 0xFFFFu) : (M[i - 16] >> 16);
+    }
+    if (accumulate) {
+        // a later channel block: add the uint32 partial sums the earlier blocks left in out; the total
+        // may reach 2^24 - 1, beyond the magic-number conversion, so convert with I2F here
+        if (fast) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const uint4 old = *reinterpret_cast<const uint4 *>(orow + (size_t)(t0 + 4 * q) * 4);
+                o[4 * q] += old.x; o[4 * q + 1] += old.y; o[4 * q + 2] += old.z; o[4 * q + 3] += old.w;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                if (t0 + i < nsamps_out) o[i] += *reinterpret_cast<const uint32_t *>(orow + (size_t)(t0 + i) * 4);
+        }
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+            if (F32) o[i] = __float_as_uint((float)o[i]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) o[i] = cvt_out<F32>(o[i]);
     }
     if (fast) {
 #pragma unroll
@@ -254,7 +273,7 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
     }
     __syncthreads();
 
-    const int nchunks = P.nchans_pad / CH;
+    const int nchunks = P.nchunks;
     const long long nitems = (long long)P.nbeams * P.ngroups * P.ntiles;
     int stage = 0;
     uint32_t phase = 0;
@@ -275,12 +294,12 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                 // one copy per (channel, plane) of the chunk, spread over the lanes
 #pragma unroll
                 for (int i = lane; i < CH * NB; i += 32) {
-                    const int c = chunk * CH + i / NB, pidx = i % NB;
+                    const int c = (P.chunk0 + chunk) * CH + i / NB, pidx = i % NB;
                     const uint32_t *src = pl + ((size_t)c * NB + pidx) * P.row_pitch + P.ws[grow + c];
                     bulk_g2s(sb + i * (WIN * 4), src, WIN * 4, fb);
                 }
                 if (lane == 0)
-                    bulk_g2s(sb + S::DATA_BYTES, P.rel + (grow + (size_t)chunk * CH) * LANES,
+                    bulk_g2s(sb + S::DATA_BYTES, P.rel + (grow + (size_t)(P.chunk0 + chunk) * CH) * LANES,
                              S::REL_BYTES, fb);
                 if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
             }
@@ -318,7 +337,7 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
             const long long t0 = (long long)tile * C::TILE_SAMPS + (warp * W + j) * 32;
             if (d >= 0 && t0 < P.nsamps_out)
                 unslice_store<NP, W, F32>(A, j, orow, t0, P.nsamps_out,
-                                          P.vec_ok && t0 + 32 <= P.nsamps_out);
+                                          P.vec_ok && t0 + 32 <= P.nsamps_out, P.accumulate != 0);
 #pragma unroll
             for (int p = 0; p < NP; ++p) A[p][j] = 0;
         }
@@ -406,12 +425,25 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
                (nbeams == 1 || out_beam_stride % 16 == 0);
     const long long nitems = (long long)nbeams * P.ngroups * ntiles;
     const int grid = (int)(nitems < sms ? nitems : sms);
-    cudaError_t e;
-    if (G.win_words == C::WIN_S)
-        e = out_f32 ? launch_one<C, C::WIN_S, true>(P, grid, s) : launch_one<C, C::WIN_S, false>(P, grid, s);
-    else
-        e = out_f32 ? launch_one<C, C::WIN_L, true>(P, grid, s) : launch_one<C, C::WIN_L, false>(P, grid, s);
-    DEDISP_CUDA_TRY(plan, e);
+    // channel blocks: a block's largest possible sum must fit the NP counter planes; later blocks add to
+    // the uint32 partial sums in out (float32 output: converted by the last block)
+    const long long per_chan = (long long)tscrunch * ((1ll << in_nbits) - 1);
+    long long cblk = (((1ll << C::NP) - 1) / per_chan) / CH_PAD * CH_PAD;
+    if (cblk < CH_PAD) return DEDISP_ERR_INVALID_ARG;
+    if (cblk > G.nchans_pad) cblk = G.nchans_pad;
+    for (long long c0 = 0; c0 < G.nchans_pad; c0 += cblk) {
+        const long long c1 = c0 + cblk < G.nchans_pad ? c0 + cblk : G.nchans_pad;
+        P.chunk0 = (int)(c0 / C::CH);
+        P.nchunks = (int)((c1 - c0) / C::CH);
+        P.accumulate = c0 > 0;
+        const bool f32 = out_f32 && c1 == G.nchans_pad;
+        cudaError_t e;
+        if (G.win_words == C::WIN_S)
+            e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s) : launch_one<C, C::WIN_S, false>(P, grid, s);
+        else
+            e = f32 ? launch_one<C, C::WIN_L, true>(P, grid, s) : launch_one<C, C::WIN_L, false>(P, grid, s);
+        DEDISP_CUDA_TRY(plan, e);
+    }
     if (plan->timing) {
         cudaEventRecord(plan->ev[3], s);
         plan->timing_valid = true;
@@ -435,8 +467,9 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     const int np = tscrunch == 1 ? nbits : tscrunch_planes(nbits, tscrunch);
     if (np < 1 || np >= NGEOM) return DEDISP_ERR_INVALID_ARG;
     const BitsliceGeom &G = plan->geom[geom_index(np)];
-    const long long maxsum = (long long)plan->nchans * tscrunch * ((1ll << nbits) - 1);
-    if (!G.usable || maxsum >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
+    // (sums beyond the counter planes are served in channel blocks as long as 32 channels fit)
+    const long long per_chan = (long long)tscrunch * ((1ll << nbits) - 1);
+    if (!G.usable || CH_PAD * per_chan >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
     if (rg.g_begin < 0 || rg.g_count < 0 || rg.g_begin + rg.g_count > G.ngroups) return DEDISP_ERR_INVALID_ARG;
 #define BS_RUN(CFG)                                                                                   \
     return execute_cfg<CFG>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, nbits, tscrunch, \
@@ -457,6 +490,5 @@ int bitslice_ngroups(dedisp_plan plan, int nbits)
 {
     if (nbits < 1 || nbits >= NGEOM) return 0;
     const BitsliceGeom &G = plan->geom[geom_index(nbits)];
-    const long long maxsum = (long long)plan->nchans * ((1ll << nbits) - 1);
-    return (G.usable && maxsum < (1ll << G.nplanes_acc)) ? G.ngroups : 0;
+    return (G.usable && CH_PAD * ((1ll << nbits) - 1) < (1ll << G.nplanes_acc)) ? G.ngroups : 0;
 }

@@ -24,6 +24,16 @@
 
 #include "dedisp_internal.h"
 
+// resident CTAs per SM the register budget is set for (measured on the gulp, 7 widths: plain kernel
+// 4 / 5 / 6 CTAs = 0.534 / 0.526 / 0.626 ms; with the fused sum of squares 0.925 / 1.000 / 1.010 ms per
+// matched_filter_rms + find_events step)
+#ifndef MF_MINB
+#define MF_MINB 5
+#endif
+#ifndef MF_MINB_RMS
+#define MF_MINB_RMS 4
+#endif
+
 namespace {
 
 constexpr int NT = 256;          // threads per CTA
@@ -115,7 +125,7 @@ template <> struct Vec8<unsigned long long> {
 // <= 64 outputs it writes per width and segment, then float64 across the block in a fixed order --
 // so that the noise level of every filtered series is known without reading z back.
 template <class ACC, bool XF32, bool GUARD, bool RMS>
-__global__ void __launch_bounds__(NT, 5) matched_filter_kernel(const MFParams P)
+__global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filter_kernel(const MFParams P)
 {
     static_assert(!GUARD || sizeof(ACC) == 4, "the guard belongs to the 32-bit path");
     // 32-bit rings are stored twice (slot i and i+RING) so that reads at slot+w never wrap;

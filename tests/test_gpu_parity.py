@@ -231,6 +231,22 @@ def test_execute_host_single_beam_pieces(order, ndm):
     dd.dedisp_destroy(p)
 
 
+@pytest.mark.parametrize("nbits,nchans,od", [(2, 2048, "u32"), (2, 4100, "f32"), (1, 9000, "u32"), (4, 4400, "f32"),
+                                             (8, 4200, "u32"), (8, 9000, "f32")])
+def test_many_channels_run_in_channel_blocks(nbits, nchans, od):
+    # sums beyond the counter planes of the bit-sliced kernel (e.g. 2-bit: 3 * nchans >= 4096): the channels
+    # are summed in blocks and later blocks add to the partial sums in out -- still the bit-sliced kernel
+    w = W.CONFIGS["htru_gulp"].scaled(nchans=nchans, nbits=nbits, ndm=40, nsamps_out=1500, df=-400.0 / nchans,
+                                      dm_hi=60.0, kind="uniform", out_dtype=od)
+    delay, md, x = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    got = gpu_dedisperse(p, x, nbits, w.nsamps_out, od)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
+    want = oracle.dedisperse(delay, x[0], nbits, w.nsamps_out)
+    assert np.array_equal(got[0], want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
 def test_execute_host_many_beams():
     # more beams than the plan holds events for (16): one piece per beam
     w = W.CONFIGS["beams13"].scaled(nchans=32, ndm=40, nsamps_out=700, df=-12.0, dm_hi=100.0, nbeams=19)

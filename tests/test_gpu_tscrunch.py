@@ -93,6 +93,18 @@ def test_forced_direct_kernel_and_float_output():
         dd.dedisp_destroy(plan)
 
 
+def test_many_channels_run_in_channel_blocks():
+    # 2-bit x 16: block sums up to 48, 1500 channels => 72 000 >= 2^16 counter range: two channel blocks
+    args, delay, packed = case(1500, 24, 60.0, 700, 2, 16, 9)
+    plan = make_plan(*args)
+    for f32 in (False, True):
+        got = run_gpu(plan, 16, packed, 2, 700, f32=f32)
+        assert dd.dedisp_get_last_kernel(plan) == dd.DEDISP_KERNEL_BITSLICE
+        want = TS.dedisperse_tscrunch_bytes(delay, packed[0], 2, 16, 700)
+        assert np.array_equal(got[0], want.astype(np.float32) if f32 else want)
+    dd.dedisp_destroy(plan)
+
+
 def test_hand_worked_example():
     # tests/test_tscrunch_pins.py::test_hand_worked_example, through the C ABI
     rows = ["00123112210323301010313010001232", "03223323011210301101113222230111",
