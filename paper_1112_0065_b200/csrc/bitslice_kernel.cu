@@ -399,9 +399,10 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     }
     BitsliceParams P;
     P.planes = plan->d_planes;
-    P.ws = plan->d_ws;
-    P.rel = plan->d_rel;
-    P.order = plan->d_order;
+    const BitsliceTables &T = plan->tab[G.tab];
+    P.ws = T.d_ws;
+    P.rel = T.d_rel;
+    P.order = T.d_order;
     P.out = (uint8_t *)out;
     P.out_beam_stride = out_beam_stride;
     P.beam_pitch_words = beam_pitch;
@@ -490,5 +491,7 @@ int bitslice_ngroups(dedisp_plan plan, int nbits)
 {
     if (nbits < 1 || nbits >= NGEOM) return 0;
     const BitsliceGeom &G = plan->geom[geom_index(nbits)];
-    return (G.usable && CH_PAD * ((1ll << nbits) - 1) < (1ll << G.nplanes_acc)) ? G.ngroups : 0;
+    // (the host path maps a range of groups to a range of output rows: needs 32 trials in every group)
+    return (G.usable && plan->tab[G.tab].dms_per_group == 32 &&
+            CH_PAD * ((1ll << nbits) - 1) < (1ll << G.nplanes_acc)) ? G.ngroups : 0;
 }

@@ -381,74 +381,116 @@ cudaError_t launch_tscrunch_bytes(int nbits, int k, const uint8_t *in, size_t in
 }
 
 // ---- host side of set_dm_list ------------------------------------------------
+static void free_tables(BitsliceTables &T)
+{
+    cudaFree(T.d_rel);
+    cudaFree(T.d_ws);
+    cudaFree(T.d_order);
+    T = BitsliceTables();
+}
+
 void bitslice_release(dedisp_plan p)
 {
-    cudaFree(p->d_rel);
-    cudaFree(p->d_ws);
-    cudaFree(p->d_order);
-    p->d_rel = nullptr;
-    p->d_ws = nullptr;
-    p->d_order = nullptr;
+    if (p->tab[1].d_rel != p->tab[0].d_rel) free_tables(p->tab[1]);
+    else p->tab[1] = BitsliceTables();
+    free_tables(p->tab[0]);
     for (int i = 0; i < bs::NGEOM; ++i) p->geom[i] = BitsliceGeom();
 }
 
 template <class C>
-static void fill_geom(BitsliceGeom &G, int nchans_pad, int ndm_pad, int max_off)
+static void fill_geom(BitsliceGeom &G, int nchans_pad, const BitsliceTables &T, int tab)
 {
     G = BitsliceGeom();
     G.nbits = C::NB;
     G.nchans_pad = nchans_pad;
-    G.ndm_pad = ndm_pad;
-    G.ngroups = ndm_pad / 32;
+    G.ndm_pad = T.ngroups * 32;
+    G.ngroups = T.ngroups;
     G.nplanes_acc = C::NP;
+    G.tab = tab;
     // a thread reads words off + warp*W + j, j = 0..W  =>  off_max + TILE_WORDS + 1 words
-    const int need = max_off + C::TILE_WORDS + 1;
+    const int need = T.max_off + C::TILE_WORDS + 1;
     if (need <= C::WIN_S) G.win_words = C::WIN_S;
     else if (need <= C::WIN_L) G.win_words = C::WIN_L;
-    else return;   // DM steps too coarse for a tile window: the DIRECT kernel serves the plan
-    G.usable = true;   // bitslice_execute still checks that the largest possible sum fits nplanes_acc
+    else return;   // cannot happen once dms_per_group is 1 (max_off = 3); the DIRECT kernel would serve the plan
+    G.usable = T.d_rel != nullptr;
+}
+
+// Build the tables with `dpg` trials per group; cudaSuccess and T filled, or an error and T empty.
+static cudaError_t build_tables(dedisp_plan p, const std::vector<int32_t> &sorted_dms, int dpg, int nchans_pad,
+                                BitsliceTables &T)
+{
+    const int ndm = p->ndm;
+    const int ngroups = (ndm + dpg - 1) / dpg;
+    std::vector<int32_t> lanes((size_t)ngroups * 32, -1);
+    for (int i = 0; i < ndm; ++i) lanes[(size_t)(i / dpg) * 32 + i % dpg] = sorted_dms[i];
+    T = BitsliceTables();
+    T.ngroups = ngroups;
+    T.dms_per_group = dpg;
+    int *d_max = nullptr;
+    const size_t nrows = (size_t)ngroups * nchans_pad;
+    cudaError_t e = cudaMalloc(&T.d_order, sizeof(int32_t) * lanes.size());
+    if (e == cudaSuccess) e = cudaMalloc(&T.d_ws, sizeof(int32_t) * nrows);
+    if (e == cudaSuccess) e = cudaMalloc(&T.d_rel, sizeof(uint32_t) * nrows * 32);
+    if (e == cudaSuccess) e = cudaMalloc(&d_max, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(d_max, 0, sizeof(int));
+    if (e == cudaSuccess)
+        e = cudaMemcpy(T.d_order, lanes.data(), sizeof(int32_t) * lanes.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        bitslice_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, T.d_order, nchans_pad, T.d_ws,
+                                                 T.d_rel, d_max);
+        ++g_launch_count;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(&T.max_off, d_max, sizeof(int), cudaMemcpyDeviceToHost);
+    cudaFree(d_max);
+    if (e != cudaSuccess) free_tables(T);
+    return e;
 }
 
 dedisp_status bitslice_prepare(dedisp_plan p)
 {
     const int ndm = p->ndm;
-    const int ndm_pad = (ndm + 31) / 32 * 32, ngroups = ndm_pad / 32;
     const int nchans_pad = (p->nchans + bs::CH_PAD - 1) / bs::CH_PAD * bs::CH_PAD;
     // trial DMs sorted ascending (stable) -> lanes of a group have nearby, monotone delays
-    std::vector<int32_t> sorted(ndm_pad, -1);
-    std::iota(sorted.begin(), sorted.begin() + ndm, 0);
-    std::stable_sort(sorted.begin(), sorted.begin() + ndm,
-                     [&](int a, int b) { return p->dms[a] < p->dms[b]; });
+    std::vector<int32_t> sorted(ndm);
+    std::iota(sorted.begin(), sorted.end(), 0);
+    std::stable_sort(sorted.begin(), sorted.end(), [&](int a, int b) { return p->dms[a] < p->dms[b]; });
     p->order_identity = true;
     for (int i = 0; i < ndm; ++i) p->order_identity = p->order_identity && sorted[i] == i;
-    int *d_max = nullptr;
-    const size_t nrows = (size_t)ngroups * nchans_pad;
-    cudaError_t e = cudaMalloc(&p->d_order, sizeof(int32_t) * ndm_pad);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws, sizeof(int32_t) * nrows);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_rel, sizeof(uint32_t) * nrows * 32);
-    if (e == cudaSuccess) e = cudaMalloc(&d_max, sizeof(int));
-    if (e == cudaSuccess) e = cudaMemset(d_max, 0, sizeof(int));
-    if (e == cudaSuccess)
-        e = cudaMemcpy(p->d_order, sorted.data(), sizeof(int32_t) * ndm_pad, cudaMemcpyHostToDevice);
-    int max_off = 0;
-    if (e == cudaSuccess) {
-        bitslice_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, p->d_order, nchans_pad,
-                                                 p->d_ws, p->d_rel, d_max);
-        ++g_launch_count;
-        e = cudaGetLastError();
+    // largest window offset each family of geometries can take: WIN_L - tile words - 1
+    const int lim0 = std::min({bs::Cfg1::WIN_L - bs::Cfg1::TILE_WORDS, bs::Cfg2::WIN_L - bs::Cfg2::TILE_WORDS,
+                               bs::Cfg3::WIN_L - bs::Cfg3::TILE_WORDS, bs::Cfg4::WIN_L - bs::Cfg4::TILE_WORDS,
+                               bs::Cfg5::WIN_L - bs::Cfg5::TILE_WORDS}) - 1;
+    const int lim1 = std::min(bs::Cfg6::WIN_L - bs::Cfg6::TILE_WORDS, bs::Cfg8::WIN_L - bs::Cfg8::TILE_WORDS) - 1;
+    cudaError_t e = cudaSuccess;
+    int dpg = 32;
+    for (; dpg >= 1; dpg >>= 1) {       // 32 trials per group unless the DM steps are too coarse for the window
+        e = build_tables(p, sorted, dpg, nchans_pad, p->tab[0]);
+        if (e != cudaSuccess || p->tab[0].max_off <= lim0 || dpg == 1) break;
+        free_tables(p->tab[0]);
     }
-    if (e == cudaSuccess) e = cudaMemcpy(&max_off, d_max, sizeof(int), cudaMemcpyDeviceToHost);
-    cudaFree(d_max);
+    if (e == cudaSuccess) {
+        if (p->tab[0].max_off <= lim1) {
+            p->tab[1] = p->tab[0];      // shared (bitslice_release frees it once)
+        } else {
+            for (dpg >>= 1; dpg >= 1; dpg >>= 1) {
+                e = build_tables(p, sorted, dpg, nchans_pad, p->tab[1]);
+                if (e != cudaSuccess || p->tab[1].max_off <= lim1 || dpg == 1) break;
+                free_tables(p->tab[1]);
+            }
+        }
+    }
     if (e != cudaSuccess) {
         p->last_cuda_error = (int)e;
+        bitslice_release(p);
         return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
     }
-    fill_geom<bs::Cfg1>(p->geom[1], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg2>(p->geom[2], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg3>(p->geom[3], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg4>(p->geom[4], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg5>(p->geom[5], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg6>(p->geom[6], nchans_pad, ndm_pad, max_off);
-    fill_geom<bs::Cfg8>(p->geom[8], nchans_pad, ndm_pad, max_off);
+    fill_geom<bs::Cfg1>(p->geom[1], nchans_pad, p->tab[0], 0);
+    fill_geom<bs::Cfg2>(p->geom[2], nchans_pad, p->tab[0], 0);
+    fill_geom<bs::Cfg3>(p->geom[3], nchans_pad, p->tab[0], 0);
+    fill_geom<bs::Cfg4>(p->geom[4], nchans_pad, p->tab[0], 0);
+    fill_geom<bs::Cfg5>(p->geom[5], nchans_pad, p->tab[0], 0);
+    fill_geom<bs::Cfg6>(p->geom[6], nchans_pad, p->tab[1], 1);
+    fill_geom<bs::Cfg8>(p->geom[8], nchans_pad, p->tab[1], 1);
     return DEDISP_OK;
 }

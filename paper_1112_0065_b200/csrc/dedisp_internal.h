@@ -17,6 +17,19 @@ struct BitsliceGeom {
     int ngroups = 0;         // ndm_pad / 32
     int win_words = 0;       // smem words per (channel, plane) window
     int nplanes_acc = 0;     // accumulator bit planes
+    int tab = 0;             // which table set (dedisp_plan_s::tab) the geometry reads
+};
+
+// Tables of the tiled kernel for one grouping of the sorted trial DMs: groups of 32 lanes of which
+// the first dms_per_group hold trials (32 unless the DM steps are so coarse that the delays of 32
+// neighbouring trials would not fit a tile window; then 16, 8, ... and the other lanes idle).
+struct BitsliceTables {
+    uint32_t *d_rel = nullptr;    // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
+    int32_t *d_ws = nullptr;      // [ngroups][nchans_pad] window start word
+    int32_t *d_order = nullptr;   // [ngroups*32] trial index of each lane, -1 = idle lane
+    int ngroups = 0;
+    int dms_per_group = 0;
+    int max_off = 0;              // largest (delay >> 5) - window start over the table, words
 };
 
 struct dedisp_plan_s {
@@ -32,9 +45,7 @@ struct dedisp_plan_s {
     int last_cuda_error = 0;
     // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
     BitsliceGeom geom[9];         // [bit planes per sample]: 1, 2, 4, 8 = packed widths; 3, 5, 6 = time-scrunched sums
-    uint32_t *d_rel = nullptr;    // [ngroups][nchans_pad][32] packed (byte offset<<16 | shift)
-    int32_t *d_ws = nullptr;      // [ngroups][nchans_pad] window start word
-    int32_t *d_order = nullptr;   // [ndm_pad] trial index of each sorted lane, -1 = padding
+    BitsliceTables tab[2];        // [0] for the 96/224-word windows, [1] for the narrower 8-/6-plane windows
     uint32_t *d_planes = nullptr; // bit-plane copy of the input
     size_t planes_bytes = 0;
     // dedisp_execute_host staging

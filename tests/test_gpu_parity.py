@@ -247,6 +247,26 @@ def test_many_channels_run_in_channel_blocks(nbits, nchans, od):
     dd.dedisp_destroy(p)
 
 
+@pytest.mark.parametrize("nbits", [1, 2, 4, 8])
+@pytest.mark.parametrize("ndm", [3, 20, 150, 400])
+def test_coarse_dm_steps_stay_on_the_bit_sliced_kernel(nbits, ndm):
+    # DM steps so coarse that the delays of 32 neighbouring trials do not fit a tile window: the groups
+    # then hold 16, 8, ... 1 trials (idle lanes) instead of handing the plan to the DIRECT kernel
+    w = W.CONFIGS["htru_gulp"].scaled(nchans=256, nbits=nbits, ndm=ndm, nsamps_out=2500, df=-400.0 / 256,
+                                      kind="uniform")
+    dms = np.random.default_rng(ndm).permutation(w.dms())          # and in any order
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, dms)
+    x = W.generate(w, md)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, dms)
+    got = gpu_dedisperse(p, x[None], nbits, w.nsamps_out)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
+    assert np.array_equal(got[0], oracle.dedisperse(delay, x, nbits, w.nsamps_out))
+    out = torch.empty((ndm, w.nsamps_out), dtype=torch.int32).pin_memory()
+    dd.dedisp_execute_host(p, 1, w.nsamps_out, torch.from_numpy(x).pin_memory(), nbits, out, dd.DEDISP_OUT_U32)
+    assert np.array_equal(out.numpy().view(np.uint32), got[0])
+    dd.dedisp_destroy(p)
+
+
 def test_execute_host_many_beams():
     # more beams than the plan holds events for (16): one piece per beam
     w = W.CONFIGS["beams13"].scaled(nchans=32, ndm=40, nsamps_out=700, df=-12.0, dm_hi=100.0, nbeams=19)
