@@ -86,6 +86,24 @@ time_major_kernel(const uint32_t *__restrict__ in, int row_words, int nchans, lo
     const int sub = lane / TS, j = lane % TS;
     const uint32_t *rowj = sm + (warp * RPI + sub) * TSP + j;            // word j of row (k = 0, lc0)
     const int cstep = 8 * RPI * E;                                       // channels between a warp's iterations
+    if ((((uintptr_t)out | (uintptr_t)out_row_stride) & 3) == 0) {
+        // every row starts on a word (rows of a multiple of 4 bytes): shared word j IS aligned global word j
+        const bool full = 4 * j + 4 <= nb;
+        const int tail = nb - 4 * j;                                     // 1..3: the row ends inside this word
+        for (int k = 0; k < E; ++k) {
+            int c = (wc0 + warp * RPI + sub) * E + k;
+            uint8_t *dst = out + (size_t)c * out_row_stride + (size_t)tile_byte0 + 4 * j;
+            const uint32_t *row = rowj + k * 32 * TSP;
+#pragma unroll 4
+            for (int it = 0; it < 32 / (8 * RPI); ++it, c += cstep, dst += (size_t)cstep * out_row_stride,
+                     row += 8 * RPI * TSP) {
+                if (c >= nchans) break;
+                if (full) *reinterpret_cast<uint32_t *>(dst) = row[0];
+                else if (tail > 0) store_some_bytes(dst, row[0], 0, tail);
+            }
+        }
+        return;
+    }
     for (int k = 0; k < E; ++k) {
         int c = (wc0 + warp * RPI + sub) * E + k;
         uint8_t *dst = out + (size_t)c * out_row_stride + (size_t)tile_byte0;

@@ -23,7 +23,9 @@ def gpu_tm(stream, nchans, nsamps, nbits):
 
 @pytest.mark.parametrize("nbits,nchans,nsamps", [
     (2, 1024, 3000), (2, 1024, 257), (2, 16, 1), (1, 32, 5), (1, 1024, 1001), (1, 96, 300), (4, 8, 7),
-    (4, 1024, 777), (8, 4, 3), (8, 4096, 513), (2, 48, 1023), (1, 4096, 130)])
+    (4, 1024, 777), (8, 4, 3), (8, 4096, 513), (2, 48, 1023), (1, 4096, 130),
+    # rows of a multiple of 4 bytes (word-aligned store path), small and large grids, and a large ragged one
+    (8, 4096, 516), (2, 1024, 4112), (1, 64, 96), (4, 40, 2056), (8, 100, 4100), (8, 1024, 40000), (8, 1024, 40001)])
 def test_transpose_matches_oracle(nbits, nchans, nsamps):
     rng = np.random.default_rng(nbits * 7 + nchans + nsamps)
     stream = rng.integers(0, 256, nsamps * nchans * nbits // 8, dtype=np.uint8)
