@@ -345,15 +345,16 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
 }
 
 template <class C, int WIN, bool F32>
-cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s)
+cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s, int device)
 {
     constexpr int SMEM = Stage<C, WIN>::SMEM;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static unsigned long long attr_done = 0;     // the attribute is per device: one bit per device id
+    const unsigned long long bit = 1ull << (device & 63);
+    if (device > 63 || !(attr_done & bit)) {
         cudaError_t e = cudaFuncSetAttribute(bitslice_dedisperse<C, WIN, F32>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done |= bit;
     }
     bitslice_dedisperse<C, WIN, F32><<<grid, C::NTHREADS, SMEM, s>>>(P);
     ++g_launch_count;
@@ -440,9 +441,9 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
         const bool f32 = out_f32 && c1 == G.nchans_pad;
         cudaError_t e;
         if (G.win_words == C::WIN_S)
-            e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s) : launch_one<C, C::WIN_S, false>(P, grid, s);
+            e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s, plan->device) : launch_one<C, C::WIN_S, false>(P, grid, s, plan->device);
         else
-            e = f32 ? launch_one<C, C::WIN_L, true>(P, grid, s) : launch_one<C, C::WIN_L, false>(P, grid, s);
+            e = f32 ? launch_one<C, C::WIN_L, true>(P, grid, s, plan->device) : launch_one<C, C::WIN_L, false>(P, grid, s, plan->device);
         DEDISP_CUDA_TRY(plan, e);
     }
     if (plan->timing) {
