@@ -272,7 +272,7 @@ def run_ours(args) -> None:
                 "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
     try:
         probe = {n: dd.dedisp_probe_alu_rate(i) / 1e12 for i, n in
-                 enumerate(["iadd3", "lop3", "shf", "fadd", "imad", "lop3+imad"])}
+                 enumerate(["iadd3", "lop3", "shf", "fadd", "imad", "lop3+imad", "lds32", "lds128", "prmt", "dp4a"])}
     except Exception as e:  # noqa: BLE001
         probe = {"error": str(e)}
     cpu = None

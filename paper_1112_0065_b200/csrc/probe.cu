@@ -20,6 +20,12 @@ __global__ void __launch_bounds__(1024) probe_kernel(uint32_t *out, uint32_t see
         f[i] = (float)(r[i] & 1023);
     }
     uint32_t k = seed | 1u, m = seed * 7u + 3u;
+    __shared__ __align__(16) uint32_t sh[8192];
+    for (int i = threadIdx.x; i < 8192; i += blockDim.x) sh[i] = seed + i;
+    __syncthreads();
+    // conflict-free shared-memory reads: consecutive lanes read consecutive words (u32) / 16-byte vectors (v4)
+    const uint32_t a32 = (uint32_t)__cvta_generic_to_shared(sh) + 4u * threadIdx.x;
+    const uint32_t a128 = (uint32_t)__cvta_generic_to_shared(sh) + 16u * threadIdx.x;
     for (int it = 0; it < ITERS; ++it) {
 #pragma unroll
         for (int i = 0; i < CHAINS; ++i) {
@@ -33,6 +39,19 @@ __global__ void __launch_bounds__(1024) probe_kernel(uint32_t *out, uint32_t see
                 asm volatile("add.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(1.5f));
             else if (WHICH == 4)  // IMAD
                 asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k), "r"(m));
+            else if (WHICH == 6) {  // LDS.32 (+ one XOR so that the load is used)
+                uint32_t t;
+                asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(t) : "r"(a32 + 128u * i + 4096u * (it & 3)) : "memory");
+                r[i] ^= t;
+            } else if (WHICH == 7) {  // LDS.128
+                uint32_t t0, t1, t2, t3;
+                asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                             : "=r"(t0), "=r"(t1), "=r"(t2), "=r"(t3) : "r"(a128 + 512u * i + 8192u * (it & 1)) : "memory");
+                r[i] ^= t0 ^ t1 ^ t2 ^ t3;
+            } else if (WHICH == 8)  // PRMT (byte permute)
+                asm volatile("prmt.b32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(k), "r"(m));
+            else if (WHICH == 9)  // DP4A
+                asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(r[i]) : "r"(k), "r"(m));
             else {  // alternate LOP3 (alu pipe) and IMAD (fma pipe)
                 if (i & 1)
                     asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[i]) : "r"(k), "r"(m));
@@ -49,7 +68,7 @@ __global__ void __launch_bounds__(1024) probe_kernel(uint32_t *out, uint32_t see
 
 extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s)
 {
-    if (!lane_ops_per_s || which < 0 || which > 5) return DEDISP_ERR_INVALID_ARG;
+    if (!lane_ops_per_s || which < 0 || which > 9) return DEDISP_ERR_INVALID_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return DEDISP_ERR_CUDA;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
@@ -69,7 +88,11 @@ extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s
             case 2: probe_kernel<2><<<blocks, threads>>>(d, 12345u + rep); break;
             case 3: probe_kernel<3><<<blocks, threads>>>(d, 12345u + rep); break;
             case 4: probe_kernel<4><<<blocks, threads>>>(d, 12345u + rep); break;
-            default: probe_kernel<5><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 5: probe_kernel<5><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 6: probe_kernel<6><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 7: probe_kernel<7><<<blocks, threads>>>(d, 12345u + rep); break;
+            case 8: probe_kernel<8><<<blocks, threads>>>(d, 12345u + rep); break;
+            default: probe_kernel<9><<<blocks, threads>>>(d, 12345u + rep); break;
         }
         ++g_launch_count;
         cudaEventRecord(e1, 0);
