@@ -131,8 +131,11 @@ size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, l
 
 /* End-to-end convenience with HOST buffers (tight beam strides): copies the
  * packed input host->device, runs dedisp_execute_batch, copies the result back
- * and synchronises.  Device staging buffers are owned and reused by the plan.
- * Pinned host memory gives full PCIe rate; pageable memory works too. */
+ * and synchronises.  Device staging buffers, two streams and a few events are owned
+ * and reused by the plan.  The result dominates the transfer time, so it leaves in
+ * pieces while the kernel still runs on the rest: one beam at a time, or -- single
+ * beam, trial DMs given in ascending order -- up to 8 ranges of DM groups (output rows).
+ * Pinned host memory gives full PCIe rate and the overlap; pageable memory works too. */
 dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps_out,
                                   const void *in_host, int in_nbits, void *out_host,
                                   dedisp_out_dtype out_dtype);
