@@ -211,15 +211,26 @@ dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
  * over the <= 64 outputs a thread writes per (width, 16 384-sample segment), then in float64 in a fixed
  * order (deterministic); relative difference to the float64 definition < 2^-20.
  *   rms_dev        DEVICE float32 [nwidths*nrows], 4-byte aligned, written completely.
+ *   blockmax_dev   optional (may be NULL) DEVICE int32 [nwidths*nrows][nblocks], 4-byte aligned: a hint for
+ *                  dedisp_find_events_hinted.  With (nblocks, hint_block, hint_offset) from
+ *                  dedisp_matched_filter_hint_blocks(), entry [s][b] is >= the order-preserving integer
+ *                  image (bits(x) for x >= 0, bits(x) ^ 0x7fffffff below) of every z[s][t] with
+ *                  b*hint_block - hint_offset <= t < (b+1)*hint_block - hint_offset: the largest output of
+ *                  one 2048-sample step of the kernel, gathered with warp maxima and atomicMax.
  *   workspace_dev  DEVICE scratch, 8-byte aligned, >= dedisp_matched_filter_rms_workspace_bytes();
  *                  owned by the caller, free to reuse once the call's work has completed.
  * Other arguments, layouts and errors as dedisp_matched_filter; a null rms_dev, a null, misaligned
- * or too small workspace: INVALID_ARG.  Only enqueues work on cuda_stream (2 kernels). */
+ * or too small workspace: INVALID_ARG.  Only enqueues work on cuda_stream (2 kernels, 1 memset). */
 size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths);
 dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
                                         long long nsamps, int radius, const int *widths_host,
                                         int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
-                                        void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+                                        int *blockmax_dev, void *workspace_dev, size_t workspace_bytes,
+                                        void *cuda_stream);
+/* Blocks per series of blockmax_dev for these widths (0 on a bad argument); *hint_block and
+ * *hint_offset (either may be NULL) receive the block length (2048) and the offset (largest width). */
+long long dedisp_matched_filter_hint_blocks(long long nsamps, const int *widths_host, int nwidths,
+                                            int *hint_block, int *hint_offset);
 
 /* ---- peak finding ---- */
 
@@ -258,6 +269,19 @@ dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long lon
                                  const float *sigma_dev, float nsigma, void *workspace_dev,
                                  size_t workspace_bytes, dedisp_event *events_dev,
                                  long long max_events, long long *count_dev, void *cuda_stream);
+
+/* dedisp_find_events with a hint that lets the sigma-cut skip what cannot hold an event: hint_dev is
+ * DEVICE int32 [nseries][ceil((nsamps + hint_offset) / hint_block)] with the meaning given at
+ * dedisp_matched_filter_rms (blockmax_dev).  A 1024-sample chunk of z whose blocks are all at or below
+ * the threshold is not read; the event list is identical to dedisp_find_events' for any valid hint
+ * (entries may be larger than the true maxima, never smaller).  At a 6 sigma cut on noise nearly all of
+ * z stays unread.  Errors as dedisp_find_events, plus INVALID_ARG for a null or misaligned hint,
+ * hint_block < 1, hint_offset < 0. */
+dedisp_status dedisp_find_events_hinted(const float *z_dev, long long nseries, long long nsamps,
+                                        const float *sigma_dev, float nsigma, const int *hint_dev,
+                                        int hint_block, int hint_offset, void *workspace_dev,
+                                        size_t workspace_bytes, dedisp_event *events_dev,
+                                        long long max_events, long long *count_dev, void *cuda_stream);
 
 /* rms_dev[s] = float32( sqrt( (1/nsamps) * sum_t z[s][t]^2 ) ), accumulated in float64: the
  * noise estimate of a baseline-removed (zero-mean) series, offered as sigma for the

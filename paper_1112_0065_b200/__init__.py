@@ -56,8 +56,10 @@ ABI = {
     "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
     "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
     "dedisp_matched_filter_rms_workspace_bytes": (_sz, [_ll, _ll, _i]),
-    "dedisp_matched_filter_rms": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp, _vp, _sz,
-                                       _vp]),
+    "dedisp_matched_filter_rms": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp, _vp, _vp,
+                                       _sz, _vp]),
+    "dedisp_matched_filter_hint_blocks": (_ll, [_ll, ctypes.POINTER(_i), _i, ctypes.POINTER(_i), ctypes.POINTER(_i)]),
+    "dedisp_find_events_hinted": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _i, _i, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
     "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
@@ -235,14 +237,36 @@ def dedisp_matched_filter_rms_workspace_bytes(nrows: int, nsamps: int, nwidths: 
 
 def dedisp_matched_filter_rms(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: int, widths,
                               x_max: int, z_ptr, rms_ptr, workspace_ptr, workspace_bytes: int,
-                              stream: int = 0) -> None:
-    """dedisp_matched_filter + the RMS of every filtered series in the same pass (include/dedisp.h)."""
+                              stream: int = 0, blockmax_ptr=None) -> None:
+    """dedisp_matched_filter + the RMS of every filtered series (and, optionally, the block maxima that
+    dedisp_find_events_hinted uses) in the same pass (include/dedisp.h)."""
     w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
     st = lib().dedisp_matched_filter_rms(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths), x_max,
                                          _ptr(z_ptr), _ptr(rms_ptr) if rms_ptr is not None else None,
+                                         _ptr(blockmax_ptr) if blockmax_ptr is not None else None,
                                          _ptr(workspace_ptr) if workspace_ptr is not None else None,
                                          workspace_bytes, stream or None)
     _check(None, st, "dedisp_matched_filter_rms")
+
+
+def dedisp_matched_filter_hint_blocks(nsamps: int, widths) -> tuple[int, int, int]:
+    """(blocks per series, hint_block, hint_offset) of the blockmax array for these widths."""
+    w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
+    hb, ho = ctypes.c_int(), ctypes.c_int()
+    nb = lib().dedisp_matched_filter_hint_blocks(nsamps, w, len(widths), ctypes.byref(hb), ctypes.byref(ho))
+    return int(nb), hb.value, ho.value
+
+
+def dedisp_find_events_hinted(z_ptr, nseries: int, nsamps: int, sigma_ptr, nsigma: float, hint_ptr,
+                              hint_block: int, hint_offset: int, workspace_ptr, workspace_bytes: int,
+                              events_ptr, max_events: int, count_ptr, stream: int = 0) -> None:
+    """dedisp_find_events that skips the chunks of z the hint rules out (include/dedisp.h)."""
+    st = lib().dedisp_find_events_hinted(_ptr(z_ptr), nseries, nsamps, _ptr(sigma_ptr), nsigma,
+                                         _ptr(hint_ptr) if hint_ptr is not None else None, hint_block, hint_offset,
+                                         _ptr(workspace_ptr), workspace_bytes,
+                                         _ptr(events_ptr) if events_ptr is not None else None, max_events,
+                                         _ptr(count_ptr), stream or None)
+    _check(None, st, "dedisp_find_events_hinted")
 
 
 def dedisp_find_events_workspace_bytes(nseries: int, nsamps: int) -> int:

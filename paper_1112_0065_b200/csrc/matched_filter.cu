@@ -56,6 +56,8 @@ struct MFParams {
     int w[MAXW];
     float scale[MAXW];           // fl32(1 / (N sqrt(w)))
     double *partial;             // RMS variant: [nw][nrows][nseg] sums of z^2 over a segment
+    int *blockmax;               // RMS variant, optional: [nw][nrows][nblk] upper bounds of z per block of E outputs
+    int nblk;
 };
 
 // inclusive block scan of one value per thread; returns the thread's inclusive prefix and
@@ -115,6 +117,16 @@ template <> struct Vec8<unsigned long long> {
             reinterpret_cast<ulonglong2 *>(p)[q] = make_ulonglong2(v[2 * q], v[2 * q + 1]);
     }
 };
+
+// Push a thread's maximum of z over the outputs of one step into blockmax (see dedisp.h: hint of
+// dedisp_find_events_hinted): order-preserving int image of the float, warp maximum, one atomicMax.
+__device__ __forceinline__ void push_block_max(int *dst, float mx)
+{
+    int o = __float_as_int(mx);
+    o = o >= 0 ? o : o ^ 0x7fffffff;
+    o = __reduce_max_sync(0xffffffffu, o);
+    if ((threadIdx.x & 31) == 0) atomicMax(dst, o);
+}
 
 // GUARD (32-bit words only, host has checked N*x_max < 2^31 so that NY is exact in int32):
 // the worst-case boxcar wmax*N*x_max does not fit 32 bits, but real series stay far below
@@ -275,12 +287,15 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
         const bool interior = (tb - P.wmax >= 0) && (tb - P.wmax + E <= seglen) &&
                               (tb + E - 1 <= nrem);      // every output valid, every boxcar complete
         float *zp = zrow + ob;
+        // outputs of this step are t = lo + tb - wmax + [0, E): block (lo + tb) / E of the hint
+        int *const bmax = (RMS && P.blockmax) ? P.blockmax + (size_t)row * P.nblk + (lo + tb) / E : nullptr;
+        const size_t bstride = (size_t)P.nrows * (size_t)P.nblk;
         if (GUARD && (slowbits & P.guard_hist)) {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;
-                float ss = 0.f;
+                float ss = 0.f, mx = -INFINITY;
 #pragma unroll 1
                 for (int k = 0; k < V; ++k) {
                     const int o = ob + k * NT;
@@ -298,32 +313,34 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                         }
                     }
                     const float z = (float)zz * scl;
-                    if (RMS) ss += z * z;
+                    if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
                     __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
+                if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
         } else if (interior) {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
-                float ss = 0.f;
+                float ss = 0.f, mx = -INFINITY;
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     int sl = rs[k] + w;
                     if (!MIRROR && sl >= RING) sl -= RING;
                     const float z = acc_to_float((ACC)(ring[sl] - p0[k])) * scl;
-                    if (RMS) ss += z * z;
+                    if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
                     __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
+                if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
         } else {
             for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;                 // t + w <= n  <=>  o <= lim
-                float ss = 0.f;
+                float ss = 0.f, mx = -INFINITY;
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     const int o = ob + k * NT;
@@ -331,11 +348,12 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                         int sl = rs[k] + w;
                         if (!MIRROR && sl >= RING) sl -= RING;
                         const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
-                        if (RMS) ss += z * z;
+                        if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
                         __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
                     }
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
+                if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
         }
         wslot += E;
@@ -388,7 +406,7 @@ long long mf_segment(long long nsamps)
 
 static dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps, int radius,
                             const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
-                            void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+                            int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
 {
     if (!x_dev || !z_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0)
         return DEDISP_ERR_INVALID_ARG;
@@ -435,6 +453,9 @@ static dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long lo
     const size_t accb = wide ? 8 : 4;
     const bool rms = rms_dev != nullptr;
     P.partial = (double *)workspace_dev;
+    P.blockmax = blockmax_dev;
+    P.nblk = (int)((nsamps + P.wmax + E - 1) / E);
+    if (blockmax_dev && (!rms || ((uintptr_t)blockmax_dev & 3u))) return DEDISP_ERR_INVALID_ARG;
     if (rms) {
         if (!workspace_dev || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)rms_dev & 3u) ||
             workspace_bytes < (size_t)nwidths * (size_t)nrows * (size_t)nseg * sizeof(double))
@@ -445,6 +466,9 @@ static dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long lo
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
+    if (blockmax_dev &&   // every byte 0x80: below the image of any finite float
+        cudaMemsetAsync(blockmax_dev, 0x80, (size_t)nwidths * (size_t)nrows * (size_t)P.nblk * 4, s) != cudaSuccess)
+        return DEDISP_ERR_CUDA;
 #define MF_LAUNCH1(ACC, F, G, R)                                                                  \
     do {                                                                                         \
         e = cudaFuncSetAttribute(matched_filter_kernel<ACC, F, G, R>,                            \
@@ -486,8 +510,8 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
                                                const int *widths_host, int nwidths,
                                                unsigned int x_max, float *z_dev, void *cuda_stream)
 {
-    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, nullptr, nullptr, 0,
-                  cuda_stream);
+    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, nullptr, nullptr, nullptr,
+                  0, cuda_stream);
 }
 
 extern "C" size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths)
@@ -500,9 +524,24 @@ extern "C" size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, lon
 extern "C" dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,
                                                    long long nsamps, int radius, const int *widths_host,
                                                    int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
-                                                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+                                                   int *blockmax_dev, void *workspace_dev, size_t workspace_bytes,
+                                                   void *cuda_stream)
 {
     if (!rms_dev) return DEDISP_ERR_INVALID_ARG;
-    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, rms_dev, workspace_dev,
-                  workspace_bytes, cuda_stream);
+    return mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, rms_dev, blockmax_dev,
+                  workspace_dev, workspace_bytes, cuda_stream);
+}
+
+extern "C" long long dedisp_matched_filter_hint_blocks(long long nsamps, const int *widths_host, int nwidths,
+                                                       int *hint_block, int *hint_offset)
+{
+    if (nsamps < 1 || !widths_host || nwidths < 1 || nwidths > MAXW) return 0;
+    int wmax = 0;
+    for (int i = 0; i < nwidths; ++i) {
+        if (widths_host[i] < 1 || widths_host[i] > DEDISP_MF_MAX_WIDTH) return 0;
+        if (widths_host[i] > wmax) wmax = widths_host[i];
+    }
+    if (hint_block) *hint_block = E;
+    if (hint_offset) *hint_offset = wmax;
+    return (nsamps + wmax + E - 1) / E;
 }

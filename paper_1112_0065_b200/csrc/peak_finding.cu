@@ -57,7 +57,8 @@ __device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
 __global__ void __launch_bounds__(WARPS * 32)
 sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
                  const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
-                 uint32_t *__restrict__ counts, int vec_ok)
+                 uint32_t *__restrict__ counts, int vec_ok, const int *__restrict__ hint, int hint_block,
+                 int hint_offset, long long hint_nblocks)
 {
     const int lane = threadIdx.x & 31;
     const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
@@ -66,6 +67,22 @@ sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, lo
     const float thr = __fmul_rn(nsigma, __ldg(sigma + s));
     const float *zr = z + s * n;
     const long long t0 = c * CHUNK;
+    if (hint) {
+        // hint[s][b] bounds (order-preserving int image of the float) every z[s][t] with
+        // b*hint_block - hint_offset <= t < (b+1)*hint_block - hint_offset from above: a chunk all of
+        // whose blocks stay at or below the threshold holds no sample above it and is not read
+        const long long tl = t0 + CHUNK - 1 < n - 1 ? t0 + CHUNK - 1 : n - 1;
+        const long long b0 = (t0 + hint_offset) / hint_block, b1 = (tl + hint_offset) / hint_block;
+        int hi = (int)0x80000000;
+        for (long long b = b0 + lane; b <= b1; b += 32) hi = max(hi, __ldg(hint + s * hint_nblocks + b));
+        hi = __reduce_max_sync(0xffffffffu, hi);
+        const int ti = __float_as_int(thr);
+        if (thr == thr && hi <= (ti >= 0 ? ti : ti ^ 0x7fffffff)) {
+            mask[(s * nchunks + c) * CHUNK_WORDS + lane] = 0u;
+            if (lane == 0) counts[s * nchunks + c] = 0u;
+            return;
+        }
+    }
     uint32_t mine = 0;
     if (vec_ok && t0 + CHUNK <= n) {
         // 128-bit loads: lane l of pass i holds samples 128 i + 4 l .. + 3 -> a nibble of word
@@ -301,10 +318,11 @@ size_t dedisp_find_events_workspace_bytes(long long nseries, long long nsamps)
     return make_layout(nseries, nsamps).total;
 }
 
-dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long long nsamps,
-                                 const float *sigma_dev, float nsigma, void *workspace_dev,
-                                 size_t workspace_bytes, dedisp_event *events_dev,
-                                 long long max_events, long long *count_dev, void *cuda_stream)
+static dedisp_status find_events_run(const float *z_dev, long long nseries, long long nsamps,
+                                     const float *sigma_dev, float nsigma, const int *hint_dev, int hint_block,
+                                     int hint_offset, void *workspace_dev, size_t workspace_bytes,
+                                     dedisp_event *events_dev, long long max_events, long long *count_dev,
+                                     void *cuda_stream)
 {
     if (!z_dev || !sigma_dev || !workspace_dev || !count_dev || max_events < 0 ||
         (max_events > 0 && !events_dev))
@@ -326,7 +344,8 @@ dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long lon
     const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
     const int vec_ok = (((uintptr_t)z_dev & 15u) == 0) && (nsamps % 4 == 0);
     sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
-                                                 mask, counts, vec_ok);
+                                                 mask, counts, vec_ok, hint_dev, hint_block, hint_offset,
+                                                 hint_dev ? (nsamps + hint_offset + hint_block - 1) / hint_block : 0);
     chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
                                                                     chunk_off, series_tot);
     series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
@@ -338,6 +357,26 @@ dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long lon
                                                      chunk_off, series_base, events_dev, max_events);
     g_launch_count += 4;
     return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
+}
+
+dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long long nsamps,
+                                 const float *sigma_dev, float nsigma, void *workspace_dev,
+                                 size_t workspace_bytes, dedisp_event *events_dev,
+                                 long long max_events, long long *count_dev, void *cuda_stream)
+{
+    return find_events_run(z_dev, nseries, nsamps, sigma_dev, nsigma, nullptr, 0, 0, workspace_dev, workspace_bytes,
+                           events_dev, max_events, count_dev, cuda_stream);
+}
+
+dedisp_status dedisp_find_events_hinted(const float *z_dev, long long nseries, long long nsamps,
+                                        const float *sigma_dev, float nsigma, const int *hint_dev,
+                                        int hint_block, int hint_offset, void *workspace_dev,
+                                        size_t workspace_bytes, dedisp_event *events_dev,
+                                        long long max_events, long long *count_dev, void *cuda_stream)
+{
+    if (!hint_dev || hint_block < 1 || hint_offset < 0 || ((uintptr_t)hint_dev & 3u)) return DEDISP_ERR_INVALID_ARG;
+    return find_events_run(z_dev, nseries, nsamps, sigma_dev, nsigma, hint_dev, hint_block, hint_offset,
+                           workspace_dev, workspace_bytes, events_dev, max_events, count_dev, cuda_stream);
 }
 
 dedisp_status dedisp_series_rms(const float *z_dev, long long nseries, long long nsamps,

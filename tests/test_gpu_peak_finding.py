@@ -163,3 +163,105 @@ def test_full_size_filtered_gulp():
     same(ev[np.isin(ev["series"], rows)], want)
     key = ev["series"].astype(np.int64) * n + ev["t_start"]
     assert np.all(np.diff(key) > 0)
+
+
+# ---- dedisp_find_events_hinted: block maxima let the sigma-cut skip chunks; the event list must not change ----
+def ordered(x):
+    """order-preserving int32 image of float32 values (include/dedisp.h, blockmax_dev)."""
+    b = np.asarray(x, np.float32).view(np.int32)
+    return np.where(b >= 0, b, b ^ 0x7FFFFFFF).astype(np.int32)
+
+
+def gpu_events_hinted(z, sigma, nsigma, hint, hint_block, hint_offset):
+    z = np.ascontiguousarray(z, dtype=np.float32)
+    ns, n = z.shape
+    zd = torch.from_numpy(z).cuda()
+    sd = torch.from_numpy(np.asarray(sigma, dtype=np.float32)).cuda()
+    hd = torch.from_numpy(np.ascontiguousarray(hint, dtype=np.int32)).cuda()
+    wsb = dd.dedisp_find_events_workspace_bytes(ns, n)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    cap = min(ns * n, 4_000_000)
+    ev = torch.zeros((cap, 5), dtype=torch.int32, device="cuda")
+    cnt = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    dd.dedisp_find_events_hinted(zd, ns, n, sd, float(nsigma), hd, hint_block, hint_offset, ws, wsb, ev, cap, cnt,
+                                 torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    total = int(cnt.item())
+    raw = ev[: min(total, cap)].cpu().numpy()
+    out = np.empty(len(raw), dtype=PF.EVENT_DTYPE)
+    for i, k in enumerate(("series", "t_start", "length", "t_peak")):
+        out[k] = raw[:, i]
+    out["peak"] = raw[:, 4].copy().view(np.float32)
+    return total, out
+
+
+def exact_hint(z, block, offset):
+    ns, n = z.shape
+    nb = (n + offset + block - 1) // block
+    h = np.full((ns, nb), np.iinfo(np.int32).min, np.int32)
+    o = ordered(z)
+    for b in range(nb):
+        lo, hi = max(0, b * block - offset), min(n, (b + 1) * block - offset)
+        if hi > lo:
+            h[:, b] = o[:, lo:hi].max(axis=1)
+    return h
+
+
+@pytest.mark.parametrize("block,offset", [(2048, 64), (2048, 0), (100, 37), (5000, 4999), (1, 0)])
+@pytest.mark.parametrize("nsigma", [2.0, 4.5, 50.0])
+def test_hinted_events_equal_the_oracle(block, offset, nsigma):
+    z = W.filtered_like(77, 6, 9001, npulses=5).astype(np.float32)
+    z[2, 1020:1030] = 400.0            # runs across chunk (1024) and block boundaries
+    z[4, 2040:2060] = 300.0
+    z[5, -3:] = 500.0
+    z[1, 0] = 600.0
+    sigma = PF.series_rms(z).astype(np.float32)
+    want = PF.find_events(z, sigma, nsigma)
+    total, got = gpu_events_hinted(z, sigma, nsigma, exact_hint(z, block, offset), block, offset)
+    assert total == len(want)
+    same(got, want)
+    # a looser (larger) hint is still valid
+    total, got = gpu_events_hinted(z, sigma, nsigma, exact_hint(z, block, offset) + 12345, block, offset)
+    assert total == len(want)
+    same(got, want)
+
+
+def test_matched_filter_hint_feeds_the_search():
+    # the chain the bench times as --op search: matched_filter_rms (z, rms, block maxima) -> find_events_hinted
+    from oracle import matched_filter as MF
+    x = W.dedispersed_like(41, 6, 40001, npulses=6)
+    widths = [1, 2, 4, 8, 16, 32, 64]
+    nrows, n = x.shape
+    nb, hb, ho = dd.dedisp_matched_filter_hint_blocks(n, widths)
+    assert (hb, ho) == (2048, 64) and nb == (n + ho + hb - 1) // hb
+    xd = torch.from_numpy(x.view(np.int32)).cuda()
+    z = torch.empty((len(widths), nrows, n), dtype=torch.float32, device="cuda")
+    rms = torch.empty(len(widths) * nrows, dtype=torch.float32, device="cuda")
+    hint = torch.zeros((len(widths) * nrows, nb), dtype=torch.int32, device="cuda")
+    mwb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, len(widths))
+    mws = torch.empty(mwb, dtype=torch.uint8, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    dd.dedisp_matched_filter_rms(xd, dd.DEDISP_OUT_U32, nrows, n, 700, widths, 3072, z, rms, mws, mwb, s, blockmax_ptr=hint)
+    torch.cuda.synchronize()
+    zh = z.cpu().numpy().reshape(-1, n)
+    # the hint is exactly the block maxima of the z this call wrote
+    assert np.array_equal(hint.cpu().numpy(), exact_hint(zh, hb, ho))
+    sig = rms.cpu().numpy()
+    for nsigma in (3.0, 6.0):
+        want = PF.find_events(zh, sig, nsigma)
+        total, got = gpu_events_hinted(zh, sig, nsigma, hint.cpu().numpy(), hb, ho)
+        assert total == len(want) and (total > 0 or nsigma > 3.0)
+        same(got, want)
+
+
+def test_hinted_rejects_bad_arguments():
+    z = torch.zeros((2, 64), dtype=torch.float32, device="cuda")
+    sg = torch.ones(2, dtype=torch.float32, device="cuda")
+    wsb = dd.dedisp_find_events_workspace_bytes(2, 64)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    h = torch.zeros((2, 1), dtype=torch.int32, device="cuda")
+    for args in [(None, 64, 0), (h, 0, 0), (h, 64, -1)]:
+        with pytest.raises(dd.DedispError) as e:
+            dd.dedisp_find_events_hinted(z, 2, 64, sg, 5.0, args[0], args[1], args[2], ws, wsb, None, 0, cnt, 0)
+        assert e.value.status == dd.DEDISP_ERR_INVALID_ARG
