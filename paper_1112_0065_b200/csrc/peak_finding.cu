@@ -53,36 +53,13 @@ __device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
     return m & ~((m << 1) | (prev_word >> 31));
 }
 
-// ---- transform: one warp per (series, chunk) ----
-__global__ void __launch_bounds__(WARPS * 32)
-sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
-                 const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
-                 uint32_t *__restrict__ counts, int vec_ok, const int *__restrict__ hint, int hint_block,
-                 int hint_offset, long long hint_nblocks)
+// ---- transform of one (series, chunk) by one warp ----
+__device__ __forceinline__ void cut_chunk(const float *__restrict__ z, long long n, long long nchunks, long long s,
+                                          long long c, float thr, uint32_t *__restrict__ mask,
+                                          uint32_t *__restrict__ counts, int vec_ok, int lane)
 {
-    const int lane = threadIdx.x & 31;
-    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    if (item >= nseries * nchunks) return;
-    const long long s = item / nchunks, c = item % nchunks;
-    const float thr = __fmul_rn(nsigma, __ldg(sigma + s));
     const float *zr = z + s * n;
     const long long t0 = c * CHUNK;
-    if (hint) {
-        // hint[s][b] bounds (order-preserving int image of the float) every z[s][t] with
-        // b*hint_block - hint_offset <= t < (b+1)*hint_block - hint_offset from above: a chunk all of
-        // whose blocks stay at or below the threshold holds no sample above it and is not read
-        const long long tl = t0 + CHUNK - 1 < n - 1 ? t0 + CHUNK - 1 : n - 1;
-        const long long b0 = (t0 + hint_offset) / hint_block, b1 = (tl + hint_offset) / hint_block;
-        int hi = (int)0x80000000;
-        for (long long b = b0 + lane; b <= b1; b += 32) hi = max(hi, __ldg(hint + s * hint_nblocks + b));
-        hi = __reduce_max_sync(0xffffffffu, hi);
-        const int ti = __float_as_int(thr);
-        if (thr == thr && hi <= (ti >= 0 ? ti : ti ^ 0x7fffffff)) {
-            mask[(s * nchunks + c) * CHUNK_WORDS + lane] = 0u;
-            if (lane == 0) counts[s * nchunks + c] = 0u;
-            return;
-        }
-    }
     uint32_t mine = 0;
     if (vec_ok && t0 + CHUNK <= n) {
         // 128-bit loads: lane l of pass i holds samples 128 i + 4 l .. + 3 -> a nibble of word
@@ -122,6 +99,56 @@ sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, lo
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     mask[(s * nchunks + c) * CHUNK_WORDS + lane] = mine;
     if (lane == 0) counts[s * nchunks + c] = (uint32_t)cnt;
+}
+
+// one warp per (series, chunk)
+__global__ void __launch_bounds__(WARPS * 32)
+sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+                 const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
+                 uint32_t *__restrict__ counts, int vec_ok)
+{
+    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (item >= nseries * nchunks) return;
+    const long long s = item / nchunks;
+    cut_chunk(z, n, nchunks, s, item % nchunks, __fmul_rn(nsigma, __ldg(sigma + s)), mask, counts, vec_ok,
+              threadIdx.x & 31);
+}
+
+// Hinted form: mask and counts have been zeroed; a warp looks at 32 (series, chunk) items, lane = item,
+// and transforms only those the hint does not rule out.  hint[s][b] bounds (order-preserving int image of
+// the float) every z[s][t] with b*hint_block - hint_offset <= t < (b+1)*hint_block - hint_offset from
+// above: a chunk all of whose blocks stay at or below the threshold holds no sample above it.
+__global__ void __launch_bounds__(WARPS * 32)
+sigma_cut_hinted_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+                        const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
+                        uint32_t *__restrict__ counts, int vec_ok, const int *__restrict__ hint, int hint_block,
+                        int hint_offset, long long hint_nblocks)
+{
+    const int lane = threadIdx.x & 31;
+    const long long base = ((long long)blockIdx.x * WARPS + (threadIdx.x >> 5)) * 32;
+    const long long nitems = nseries * nchunks;
+    if (base >= nitems) return;
+    const long long item = base + lane;
+    bool look = false;
+    float thr = 0.f;
+    if (item < nitems) {
+        const long long s = item / nchunks, t0 = (item % nchunks) * CHUNK;
+        thr = __fmul_rn(nsigma, __ldg(sigma + s));
+        const long long tl = t0 + CHUNK - 1 < n - 1 ? t0 + CHUNK - 1 : n - 1;
+        const long long b1 = (tl + hint_offset) / hint_block;
+        int hi = (int)0x80000000;
+        for (long long b = (t0 + hint_offset) / hint_block; b <= b1; ++b) hi = max(hi, __ldg(hint + s * hint_nblocks + b));
+        const int ti = __float_as_int(thr);
+        look = !(thr == thr) || hi > (ti >= 0 ? ti : ti ^ 0x7fffffff);
+    }
+    uint32_t todo = __ballot_sync(0xffffffffu, look);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const long long it = base + src;
+        cut_chunk(z, n, nchunks, it / nchunks, it % nchunks, __shfl_sync(0xffffffffu, thr, src), mask, counts, vec_ok,
+                  lane);
+    }
 }
 
 // ---- scan 1: one warp per series: exclusive offsets of its chunks + series total ----
@@ -343,9 +370,18 @@ static dedisp_status find_events_run(const float *z_dev, long long nseries, long
     const long long items = nseries * L.nchunks;
     const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
     const int vec_ok = (((uintptr_t)z_dev & 15u) == 0) && (nsamps % 4 == 0);
-    sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
-                                                 mask, counts, vec_ok, hint_dev, hint_block, hint_offset,
-                                                 hint_dev ? (nsamps + hint_offset + hint_block - 1) / hint_block : 0);
+    if (hint_dev) {
+        // mask and counts (adjacent in the workspace) start at zero; only the chunks the hint cannot rule out
+        // are transformed
+        if (cudaMemsetAsync(mask, 0, L.off_chunk_off, s) != cudaSuccess) return DEDISP_ERR_CUDA;
+        const unsigned hgrid = (unsigned)((items + 32 * WARPS - 1) / (32 * WARPS));
+        sigma_cut_hinted_kernel<<<hgrid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
+                                                             mask, counts, vec_ok, hint_dev, hint_block, hint_offset,
+                                                             (nsamps + hint_offset + hint_block - 1) / hint_block);
+    } else {
+        sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
+                                                     mask, counts, vec_ok);
+    }
     chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
                                                                     chunk_off, series_tot);
     series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
