@@ -73,13 +73,17 @@ __device__ __forceinline__ ACC block_scan(ACC v, ACC *sc, ACC &total)
     }
     if (lane == 31) sc[warp] = v;
     __syncthreads();
-    ACC base = 0, tot = 0;
+    // the NT/32 = 8 warp totals: every lane takes one (lane & 7), an 8-wide shuffle scan gives the
+    // exclusive prefix of this thread's warp and the block total
+    const ACC mine = sc[lane & (NT / 32 - 1)];
+    ACC inc = mine;
 #pragma unroll
-    for (int k = 0; k < NT / 32; ++k) {
-        const ACC s = sc[k];
-        if (k < warp) base += s;
-        tot += s;
+    for (int o = 1; o < NT / 32; o <<= 1) {
+        const ACC u = __shfl_up_sync(0xffffffffu, inc, o, NT / 32);
+        if ((lane & (NT / 32 - 1)) >= o) inc += u;
     }
+    const ACC base = __shfl_sync(0xffffffffu, inc - mine, warp, NT / 32);
+    const ACC tot = __shfl_sync(0xffffffffu, inc, NT / 32 - 1, NT / 32);
     total = tot;
     __syncthreads();
     return v + base;
@@ -313,7 +317,7 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                         }
                     }
                     const float z = (float)zz * scl;
-                    if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
+                    if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
                     __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
@@ -329,7 +333,7 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                     int sl = rs[k] + w;
                     if (!MIRROR && sl >= RING) sl -= RING;
                     const float z = acc_to_float((ACC)(ring[sl] - p0[k])) * scl;
-                    if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
+                    if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
                     __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
@@ -348,7 +352,7 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                         int sl = rs[k] + w;
                         if (!MIRROR && sl >= RING) sl -= RING;
                         const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
-                        if (RMS) { ss += z * z; mx = fmaxf(mx, z); }
+                        if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
                         __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
                     }
                 }
