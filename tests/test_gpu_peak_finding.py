@@ -265,3 +265,30 @@ def test_hinted_rejects_bad_arguments():
         with pytest.raises(dd.DedispError) as e:
             dd.dedisp_find_events_hinted(z, 2, 64, sg, 5.0, args[0], args[1], args[2], ws, wsb, None, 0, cnt, 0)
         assert e.value.status == dd.DEDISP_ERR_INVALID_ARG
+
+
+def test_matched_filter_hint_with_a_width_beyond_the_block():
+    # widest boxcar 3000 > 2048-sample block: the first block of the hint covers no sample at all
+    from oracle import matched_filter as MF
+    x = W.dedispersed_like(43, 3, 20000, npulses=4)
+    widths = [1, 3000]
+    nrows, n = x.shape
+    nb, hb, ho = dd.dedisp_matched_filter_hint_blocks(n, widths)
+    assert (hb, ho) == (2048, 3000)
+    xd = torch.from_numpy(x.view(np.int32)).cuda()
+    z = torch.empty((2, nrows, n), dtype=torch.float32, device="cuda")
+    rms = torch.empty(2 * nrows, dtype=torch.float32, device="cuda")
+    hint = torch.zeros((2 * nrows, nb), dtype=torch.int32, device="cuda")
+    mwb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, 2)
+    mws = torch.empty(mwb, dtype=torch.uint8, device="cuda")
+    dd.dedisp_matched_filter_rms(xd, dd.DEDISP_OUT_U32, nrows, n, 400, widths, 3072, z, rms, mws, mwb,
+                                 torch.cuda.current_stream().cuda_stream, blockmax_ptr=hint)
+    torch.cuda.synchronize()
+    zh = z.cpu().numpy().reshape(-1, n)
+    h = hint.cpu().numpy()
+    assert (h[:, 1:] >= exact_hint(zh, hb, ho)[:, 1:]).all()
+    for nsigma in (2.5, 5.0):
+        want = PF.find_events(zh, rms.cpu().numpy(), nsigma)
+        total, got = gpu_events_hinted(zh, rms.cpu().numpy(), nsigma, h, hb, ho)
+        assert total == len(want)
+        same(got, want)
