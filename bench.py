@@ -163,6 +163,8 @@ def run_ours(args) -> None:
     t0 = time.perf_counter()
     dd.dedisp_set_dm_list(plan, list(w.dms()))
     set_dm_ms = (time.perf_counter() - t0) * 1e3
+    dd.dedisp_set_kernel(plan, {"auto": dd.DEDISP_KERNEL_AUTO, "bitslice": dd.DEDISP_KERNEL_BITSLICE,
+                                "pairs": dd.DEDISP_KERNEL_PAIRS}[args.kernel])
     md = dd.dedisp_get_max_delay(plan)
     kw = {}
     if w.kind == "gauss2_pulses":   # pulse sweeps from the product's own delay builder
@@ -263,7 +265,8 @@ def run_ours(args) -> None:
     achieved = adds / mm
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
                 "frac": achieved / alu_peak, "traffic": ncu_traffic_bytes(args.config),
-                "kernel": "bitslice_dedisperse" if kernel_used == 2 else "direct_kernel",
+                "kernel": {2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows (Cfg3P)"}.get(
+                    kernel_used, "direct_kernel"),
                 "kernel_ms": mm * 1e3, "prepass_ms": statistics.mean(pre_ms),
                 "kernel_share_of_step": mm * 1e3 / ms_per_step,
                 "peak_source": f"{props.multi_processor_count} SMs x {ADDS_PER_CLK_PER_SM} adds/clk x "
@@ -729,6 +732,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER + W.EXTRA_CONFIGS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "bitslice", "pairs"],
+                    help="A/B: force the plain tiled kernel or its pair-row variant (dedisp_set_kernel)")
     ap.add_argument("--tscrunch", type=int, default=1,
                     help="--op dedisperse only: sum blocks of K input samples and dedisperse on the grid K*dt "
                          "(row f4; the input then holds K x as many samples per output sample)")

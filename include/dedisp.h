@@ -70,7 +70,12 @@ typedef enum { DEDISP_OUT_U32 = 0, DEDISP_OUT_F32 = 1 } dedisp_out_dtype;
 typedef enum {
     DEDISP_KERNEL_AUTO = 0,     /* bit-sliced tiled kernel when the plan fits it, else DIRECT */
     DEDISP_KERNEL_DIRECT = 1,   /* one thread per output group, reads packed input from global */
-    DEDISP_KERNEL_BITSLICE = 2  /* TMA-staged (DM x time) tiles, bit-plane carry-save adders */
+    DEDISP_KERNEL_BITSLICE = 2, /* TMA-staged (DM x time) tiles, bit-plane carry-save adders */
+    DEDISP_KERNEL_PAIRS = 3     /* the same tiled kernel on pair rows: in[2p][t] + in[2p+1][t + delta] is formed
+                                   once per delay difference delta of the DM list (3 bit planes) and the tiles
+                                   add nchans/2 such rows -- the identical integer sum, re-associated.  2-bit
+                                   samples only; AUTO picks it when the plan fits (see dedisp_get_last_kernel),
+                                   BITSLICE forces the plain tiled kernel */
 } dedisp_kernel;
 
 /* Create a plan for nchans channels, sample time dt_s (s), channel 0 at f_top_mhz,
@@ -157,9 +162,9 @@ size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, in
 dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out);
 
 /* Force a kernel variant for subsequent executes (default DEDISP_KERNEL_AUTO).
- * Forcing BITSLICE on a plan it cannot serve makes execute return INVALID_ARG. */
+ * Forcing BITSLICE or PAIRS on a plan it cannot serve makes execute return INVALID_ARG. */
 dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which);
-/* Variant the last execute on this plan used (DEDISP_KERNEL_DIRECT/BITSLICE), 0 if none. */
+/* Variant the last execute on this plan used (DEDISP_KERNEL_DIRECT/BITSLICE/PAIRS), 0 if none. */
 int dedisp_get_last_kernel(dedisp_plan plan);
 
 /* Per-kernel device timing (for the bench's roofline line).  When enabled, execute

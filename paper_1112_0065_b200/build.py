@@ -14,7 +14,7 @@ CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libdedisp_b200.so"
 SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
-           "probe.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
+           "pair_rows.cu", "probe.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=false", "-Xptxas", "-v"]
 

@@ -80,11 +80,22 @@ constexpr int CH_PAD = 32;   // channels are padded to a multiple of this (>= ev
 // NP  accumulator bit planes (sums < 2^NP)  WIN_S / WIN_L  window words per (channel, plane)
 // NSPLIT  the NB planes of a chunk go through NSPLIT adder trees of NB/NSPLIT planes each (a sample
 //         is the sum of its bit fields): shorter-lived temporaries, so more warps fit the register file
-template <int NB_, int NW_, int W_, int K_, int NSTAGE_, int NP_, int WIN_S_, int WIN_L_, int NSPLIT_ = 1>
+// NV  variant windows staged per channel slot (1; 3 for the pair-sum rows, see Cfg3P below)
+template <int NB_, int NW_, int W_, int K_, int NSTAGE_, int NP_, int WIN_S_, int WIN_L_, int NSPLIT_ = 1, int NV_ = 1>
 struct Cfg {
-    static constexpr int NB = NB_, NW = NW_, W = W_, K = K_, NSTAGE = NSTAGE_, NP = NP_;
+    static constexpr int NB = NB_, NW = NW_, W = W_, K = K_, NSTAGE = NSTAGE_, NP = NP_, NV = NV_;
     static constexpr int NSPLIT = NSPLIT_, NBS = NB_ / NSPLIT_;
-    static_assert(NB_ % NSPLIT_ == 0, "plane subsets must be equal");
+    // variant windows (NV > 1) are fetched as 2-D TMA boxes of NB plane lines x (WIN + VSKEW) words; the box of
+    // an odd variant starts VSKEW = 16 words early, so its window sits 16 banks away from an even variant's:
+    // two lanes at the same window offset in neighbouring variants do not collide (offsets differ by less than
+    // 16 words in all but the widest groups; the outer two of three variants belong to the low and the high
+    // lanes of a group, whose offsets differ)
+    static constexpr int VSKEW = NV_ > 1 ? 16 : 0;
+    template <int WIN> static constexpr int plane_words() { return WIN + VSKEW; }
+    template <int WIN> static constexpr int vslot_words()
+    {
+        return NV_ > 1 ? (NB_ * (WIN + VSKEW) + 31) / 32 * 32 : NB_ * WIN;   // boxes land 128-byte aligned
+    }
     static constexpr int WIN_S = WIN_S_, WIN_L = WIN_L_;
     static constexpr int TILE_WORDS = NW * W;
     static constexpr int TILE_SAMPS = TILE_WORDS * 32;
@@ -136,6 +147,21 @@ using Cfg3 = Cfg<3, BS3_NW, 4, BS3_TREE_K, 3, 13, 96, 224>;
 using Cfg5 = Cfg<5, BS5_NW, 4, BS5_TREE_K, 3, 16, 96, 224>;
 using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160, BS6_NSPLIT>;
 
+// Pair sums: a virtual channel is the exact sum of two adjacent 2-bit
+// channels, in[2p][t] + in[2p+1][t + delta], one 3-plane row per delay difference delta that occurs in the
+// DM list; the trials of a group need at most NV = 3 consecutive differences (else the plan stays on Cfg2).
+// Same tile as Cfg2 so that both paths share the DM groups and the row pitch.
+#ifndef BS3P_NW
+#define BS3P_NW 15
+#endif
+#ifndef BS3P_TREE_K
+#define BS3P_TREE_K 3
+#endif
+#ifndef BS3P_NSTAGE
+#define BS3P_NSTAGE 3
+#endif
+using Cfg3P = Cfg<3, BS3P_NW, 4, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3>;
+
 constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8
 constexpr int geom_index(int nplanes) { return nplanes; }
 // planes needed for the block sums of k samples of nbits bits, rounded up to a built geometry (0: none)
@@ -167,4 +193,8 @@ struct BitsliceParams {
     int accumulate;            // ... and added to what out already holds (channel blocks, sums >= 2^NP)
     int gblock;                // work-item order: blocks of gblock DM groups, inside a block tile-major
     int vec_ok;                // output rows are 16-byte aligned: 128-bit stores allowed
+    // pair rows (Cfg::NV > 1): planes = [nbeams][nrows][NB][row_pitch], a channel slot of group g stages rows
+    // (vinfo & 0x0fffffff) .. + (vinfo >> 28) of it; rel carries the lane's variant in its byte offset
+    const uint32_t *vinfo;     // [ngroups][nchans_pad]
+    int vrows;                 // rows per beam
 };

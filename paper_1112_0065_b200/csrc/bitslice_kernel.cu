@@ -14,12 +14,28 @@
 //     (2 LOP3 per full adder) into a 12-plane bit-sliced counter held in registers
 //     -- 32 additions per instruction, ~0.2 ALU ops per (channel, DM, sample);
 //   * the counter is un-sliced once per tile and written as uint32 / float32.
+#include <cuda.h>
+
 #include <cmath>
 
 #include "bitslice_common.cuh"
 #include "dedisp_internal.h"
 
 using namespace bs;
+
+// AUTO takes the pair rows when the tiles saved outweigh building the rows once per execute: measured on B200
+// (HTRU gulp, profiles/r1j_pairs.md) a tile of a DM group is 6.2 us / 35 cheaper per 512 pairs and a row costs
+// 12 bytes per word at 3.7 TB/s, i.e. break-even near ngroups * npairs = 0.6 * nrows; and when the rows of all
+// beams stay below PAIRS_MAX_BYTES of scratch.
+#ifndef PAIRS_GAIN_NUM
+#define PAIRS_GAIN_NUM 4       // pairs when PAIRS_GAIN_DEN * ngroups * npairs >= PAIRS_GAIN_NUM * nrows
+#endif
+#ifndef PAIRS_GAIN_DEN
+#define PAIRS_GAIN_DEN 5
+#endif
+#ifndef PAIRS_MAX_BYTES
+#define PAIRS_MAX_BYTES (24ull << 30)
+#endif
 
 namespace {
 
@@ -62,6 +78,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
         : "memory");
 }
 
+// one 2-D box (plane lines x words) of the pair rows, through the tensor map
+__device__ __forceinline__ void tma_box_g2s(uint32_t dst, const CUtensorMap *tm, int x, int y, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+        "l"(tm), "r"(x), "r"(y), "r"(bar)
+        : "memory");
+}
+
 // full adder on 32 independent bit positions: acc <- acc ^ x ^ y, returns majority(acc, x, y)
 __device__ __forceinline__ uint32_t full_add(uint32_t &acc, uint32_t x, uint32_t y)
 {
@@ -74,7 +99,10 @@ __device__ __forceinline__ uint32_t full_add(uint32_t &acc, uint32_t x, uint32_t
 
 template <class C, int WIN>
 struct Stage {
-    static constexpr int CPITCH = C::NB * WIN * 4;      // bytes per channel: plane 0, plane 1, ...
+    static constexpr int PLW = C::template plane_words<WIN>();         // words per plane line in the slot
+    static constexpr int VSLOT = C::template vslot_words<WIN>() * 4;   // bytes per variant: [plane][PLW]
+    static constexpr int BOX_BYTES = C::NB * PLW * 4;                  // bytes one TMA box delivers (NV > 1)
+    static constexpr int CPITCH = C::NV * VSLOT;                       // bytes per channel slot
     static constexpr int DATA_BYTES = C::CH * CPITCH;
     static constexpr int REL_BYTES = C::CH * LANES * 4;
     static constexpr int BYTES = DATA_BYTES + REL_BYTES;
@@ -88,12 +116,12 @@ __device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *
                                              uint32_t (&x)[C::NBS][C::W])
 {
     const uint32_t r = relp[CI * LANES];
-    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (C::NB * WIN) + P0 * WIN;
+    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (Stage<C, WIN>::CPITCH / 4) + P0 * Stage<C, WIN>::PLW;
 #pragma unroll
     for (int p = 0; p < C::NBS; ++p) {
         uint32_t w[C::W + 1];
 #pragma unroll
-        for (int j = 0; j <= C::W; ++j) w[j] = wp[p * WIN + j];
+        for (int j = 0; j <= C::W; ++j) w[j] = wp[p * Stage<C, WIN>::PLW + j];
 #pragma unroll
         for (int j = 0; j < C::W; ++j) x[p][j] = __funnelshift_r(w[j], w[j + 1], r);   // shift = r & 31
     }
@@ -256,7 +284,7 @@ __device__ __forceinline__ void unslice_store(uint32_t (&A)[NP][W], int j, uint8
 }
 
 template <class C, int WIN, bool F32>
-__global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const BitsliceParams P)
+__global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const BitsliceParams P, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int NW = C::NW, W = C::W, NP = C::NP, NB = C::NB, CH = C::CH, NSTAGE = C::NSTAGE;
     extern __shared__ __align__(128) uint8_t smem[];
@@ -289,14 +317,34 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                 mbar_wait(empty0 + 8 * stage, phase ^ 1);
                 const uint32_t sb = smem_u32(smem) + stage * S::BYTES;
                 const uint32_t fb = full0 + 8 * stage;
-                if (lane == 0) mbar_expect_tx(fb, S::BYTES);
-                __syncwarp();
-                // one copy per (channel, plane) of the chunk, spread over the lanes
+                if constexpr (C::NV == 1) {
+                    if (lane == 0) mbar_expect_tx(fb, S::BYTES);
+                    __syncwarp();
+                    // one copy per (channel, plane) of the chunk, spread over the lanes
 #pragma unroll
-                for (int i = lane; i < CH * NB; i += 32) {
-                    const int c = (P.chunk0 + chunk) * CH + i / NB, pidx = i % NB;
-                    const uint32_t *src = pl + ((size_t)c * NB + pidx) * P.row_pitch + P.ws[grow + c];
-                    bulk_g2s(sb + i * (WIN * 4), src, WIN * 4, fb);
+                    for (int i = lane; i < CH * NB; i += 32) {
+                        const int c = (P.chunk0 + chunk) * CH + i / NB, pidx = i % NB;
+                        const uint32_t *src = pl + ((size_t)c * NB + pidx) * P.row_pitch + P.ws[grow + c];
+                        bulk_g2s(sb + i * (WIN * 4), src, WIN * 4, fb);
+                    }
+                } else {
+                    // pair rows: one box (NB plane lines x PLW words) per (channel slot, variant the group uses)
+                    static_assert(C::NV == 1 || CH <= 32, "one lane per channel slot counts the variants");
+                    const size_t c0 = grow + (size_t)(P.chunk0 + chunk) * CH;
+                    const int mine = lane < CH ? (int)(P.vinfo[c0 + lane] >> 28) + 1 : 0;
+                    const int nbox = __reduce_add_sync(0xffffffffu, mine);
+                    if (lane == 0) mbar_expect_tx(fb, S::REL_BYTES + nbox * S::BOX_BYTES);
+                    __syncwarp();
+#pragma unroll
+                    for (int i = lane; i < CH * C::NV; i += 32) {
+                        const int cl = i / C::NV, v = i % C::NV;
+                        const uint32_t info = P.vinfo[c0 + cl];
+                        if (v <= (int)(info >> 28)) {
+                            const int x = P.ws[c0 + cl] + tile * C::TILE_WORDS - (v & 1) * C::VSKEW;
+                            const int y = (beam * P.vrows + (int)(info & 0x0fffffffu) + v) * NB;
+                            tma_box_g2s(sb + cl * S::CPITCH + v * S::VSLOT, &tmap, x, y, fb);
+                        }
+                    }
                 }
                 if (lane == 0)
                     bulk_g2s(sb + S::DATA_BYTES, P.rel + (grow + (size_t)(P.chunk0 + chunk) * CH) * LANES,
@@ -345,8 +393,9 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
 }
 
 template <class C, int WIN, bool F32>
-cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s, int device)
+cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s, int device, const CUtensorMap *tm = nullptr)
 {
+    static const CUtensorMap no_map = {};
     constexpr int SMEM = Stage<C, WIN>::SMEM;
     static unsigned long long attr_done = 0;     // the attribute is per device: one bit per device id
     const unsigned long long bit = 1ull << (device & 63);
@@ -356,7 +405,7 @@ cudaError_t launch_one(const BitsliceParams &P, int grid, cudaStream_t s, int de
         if (e != cudaSuccess) return e;
         attr_done |= bit;
     }
-    bitslice_dedisperse<C, WIN, F32><<<grid, C::NTHREADS, SMEM, s>>>(P);
+    bitslice_dedisperse<C, WIN, F32><<<grid, C::NTHREADS, SMEM, s>>>(P, tm ? *tm : no_map);
     ++g_launch_count;
     return cudaGetLastError();
 }
@@ -400,6 +449,8 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     }
     BitsliceParams P;
     P.planes = plan->d_planes;
+    P.vinfo = nullptr;
+    P.vrows = 0;
     const BitsliceTables &T = plan->tab[G.tab];
     P.ws = T.d_ws;
     P.rel = T.d_rel;
@@ -454,6 +505,131 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     return DEDISP_OK;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// Pair rows (pair_rows.cu): 2-bit planes -> one 3-plane row per (channel pair, delay difference) -> the tiled
+// kernel over nchans/2 virtual channels (Cfg3P).  Same DM groups, tiles and row pitch as Cfg2.
+dedisp_status execute_pairs(dedisp_plan plan, int nbeams, long long nsamps_out, const uint8_t *in,
+                            size_t row_stride, size_t in_beam_stride, void *out, size_t out_beam_stride,
+                            int out_f32, cudaStream_t s, const BitsliceRange &range)
+{
+    using C = Cfg3P;
+    static_assert(C::TILE_WORDS == Cfg2::TILE_WORDS, "pair rows share the tiling of the 2-bit planes");
+    const PairTables &T = plan->pairs;
+    const BitsliceGeom &G = plan->geom[geom_index(2)];
+    const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
+    const long long pitch =
+        (((long long)(plan->max_delay >> 5) + ntiles * C::TILE_WORDS + C::WIN_S + 4) + 3) & ~3ll;
+    if (ntiles > 0x7fffffff / C::TILE_WORDS || pitch > 0x7fffffff || nbeams > 65535) return DEDISP_ERR_INVALID_ARG;
+    const size_t raw_beam = (size_t)G.nchans_pad * 2 * (size_t)pitch;
+    const size_t rows_beam = (size_t)T.nrows * C::NB * (size_t)pitch;
+    const size_t need_raw = raw_beam * (size_t)nbeams * 4, need_rows = rows_beam * (size_t)nbeams * 4;
+    if (plan->planes_bytes < need_raw) {
+        cudaFree(plan->d_planes);
+        plan->d_planes = nullptr;
+        plan->planes_bytes = 0;
+        if (cudaMalloc(&plan->d_planes, need_raw) != cudaSuccess) {
+            cudaGetLastError();
+            return DEDISP_ERR_ALLOC;
+        }
+        plan->planes_bytes = need_raw;
+    }
+    if (plan->pair_rows_bytes < need_rows) {
+        cudaFree(plan->d_pair_rows);
+        plan->d_pair_rows = nullptr;
+        plan->pair_rows_bytes = 0;
+        if (cudaMalloc(&plan->d_pair_rows, need_rows) != cudaSuccess) {
+            cudaGetLastError();
+            return DEDISP_ERR_ALLOC;
+        }
+        plan->pair_rows_bytes = need_rows;
+    }
+    int sms = 0;
+    DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device));
+    if (plan->timing) cudaEventRecord(plan->ev[0], s);
+    if (range.prepass) {
+        DEDISP_CUDA_TRY(plan, launch_planes(2, in, in_beam_stride, row_stride, plan->nchans, nbeams, plan->d_planes,
+                                            (int)pitch, G.nchans_pad, s));
+        DEDISP_CUDA_TRY(plan, launch_pair_rows(T, plan->d_planes, raw_beam, G.nchans_pad, plan->d_pair_rows,
+                                               rows_beam, (int)pitch, nbeams, s));
+    }
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[1], s);
+        cudaEventRecord(plan->ev[2], s);
+    }
+    // the rows as a 2-D tensor [nbeams * nrows * NB lines][pitch words]; a box = the NB plane lines of one row x
+    // one window (words outside the tensor read as zero: odd variants start VSKEW words early)
+    CUtensorMap tm;
+    {
+        EncodeTiledFn enc = encode_tiled_fn();
+        if (!enc) return DEDISP_ERR_CUDA;
+        const cuuint64_t dims[2] = {(cuuint64_t)pitch, (cuuint64_t)nbeams * T.nrows * C::NB};
+        const cuuint64_t strides[1] = {(cuuint64_t)pitch * 4};
+        const cuuint32_t box[2] = {(cuuint32_t)C::plane_words<C::WIN_S>(), (cuuint32_t)C::NB};
+        const cuuint32_t estr[2] = {1, 1};
+        if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, plan->d_pair_rows, dims, strides, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return DEDISP_ERR_CUDA;
+    }
+    BitsliceParams P;
+    P.planes = plan->d_pair_rows;
+    P.vrows = T.nrows;
+    P.ws = T.d_ws;
+    P.rel = T.d_rel;
+    P.vinfo = T.d_vinfo;
+    P.order = plan->tab[G.tab].d_order;
+    P.out = (uint8_t *)out;
+    P.out_beam_stride = out_beam_stride;
+    P.beam_pitch_words = rows_beam;
+    P.nsamps_out = nsamps_out;
+    P.row_pitch = (int)pitch;
+    P.nchans_pad = T.npairs_pad;
+    P.ngroups = range.g_count > 0 ? range.g_count : G.ngroups;
+    P.g_begin = range.g_begin;
+    P.ntiles = (int)ntiles;
+    P.nbeams = nbeams;
+    P.gblock = 1;
+    P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
+               (nbeams == 1 || out_beam_stride % 16 == 0);
+    const long long nitems = (long long)nbeams * P.ngroups * ntiles;
+    const int grid = (int)(nitems < sms ? nitems : sms);
+    // channel blocks as in execute_cfg: a pair sum is at most 6
+    long long cblk = (((1ll << C::NP) - 1) / 6) / CH_PAD * CH_PAD;
+    if (cblk > T.npairs_pad) cblk = T.npairs_pad;
+    for (long long c0 = 0; c0 < T.npairs_pad; c0 += cblk) {
+        const long long c1 = c0 + cblk < T.npairs_pad ? c0 + cblk : T.npairs_pad;
+        P.chunk0 = (int)(c0 / C::CH);
+        P.nchunks = (int)((c1 - c0) / C::CH);
+        P.accumulate = c0 > 0;
+        const bool f32 = out_f32 && c1 == T.npairs_pad;
+        const cudaError_t e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s, plan->device, &tm)
+                                  : launch_one<C, C::WIN_S, false>(P, grid, s, plan->device, &tm);
+        DEDISP_CUDA_TRY(plan, e);
+    }
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[3], s);
+        plan->timing_valid = true;
+        plan->timing_has_prepass = true;
+    }
+    return DEDISP_OK;
+}
+
 }  // namespace
 
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
@@ -473,6 +649,25 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     const long long per_chan = (long long)tscrunch * ((1ll << nbits) - 1);
     if (!G.usable || CH_PAD * per_chan >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
     if (rg.g_begin < 0 || rg.g_count < 0 || rg.g_begin + rg.g_count > G.ngroups) return DEDISP_ERR_INVALID_ARG;
+    // pair rows: 2-bit samples at full time resolution.  AUTO takes them when the DM list is long enough for
+    // the rows (built once per execute, ~max_delay/2 + nchans/2 of them) to pay for themselves.
+    const bool pairs_fit = nbits == 2 && tscrunch == 1 && plan->pairs.usable;
+    if (plan->want == DEDISP_KERNEL_PAIRS && !pairs_fit) return DEDISP_ERR_INVALID_ARG;
+    bool pairs_pay = false;
+    if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO) {
+        const PairTables &T = plan->pairs;
+        const long long ntiles = (nsamps_out + Cfg3P::TILE_SAMPS - 1) / Cfg3P::TILE_SAMPS;
+        const unsigned long long bytes = (unsigned long long)T.nrows * Cfg3P::NB * 4ull * (unsigned long long)nbeams *
+                                         (unsigned long long)((plan->max_delay >> 5) + ntiles * Cfg3P::TILE_WORDS + 128);
+        pairs_pay = (long long)PAIRS_GAIN_DEN * G.ngroups * T.npairs_pad >= (long long)PAIRS_GAIN_NUM * T.nrows &&
+                    bytes <= PAIRS_MAX_BYTES;
+    }
+    if (pairs_fit && (plan->want == DEDISP_KERNEL_PAIRS || pairs_pay)) {
+        plan->bitslice_kind = DEDISP_KERNEL_PAIRS;
+        return execute_pairs(plan, nbeams, nsamps_out, in, row_stride, in_beam_stride, out, out_beam_stride,
+                             out_f32, s, rg);
+    }
+    plan->bitslice_kind = DEDISP_KERNEL_BITSLICE;
 #define BS_RUN(CFG)                                                                                   \
     return execute_cfg<CFG>(plan, G, nbeams, nsamps_out, in, row_stride, in_beam_stride, nbits, tscrunch, \
                             out, out_beam_stride, out_f32, s, rg)

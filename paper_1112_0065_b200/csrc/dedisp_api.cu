@@ -35,6 +35,7 @@ void free_dm_state(dedisp_plan p)
     p->ndm = 0;
     p->max_delay = -1;
     p->dms.clear();
+    pair_release(p);
     bitslice_release(p);
 }
 
@@ -104,6 +105,7 @@ dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int n
     plan->ndm = ndm;
     plan->max_delay = flags[0];
     dedisp_status st = bitslice_prepare(plan);
+    if (st == DEDISP_OK) st = pair_prepare(plan);
     if (st != DEDISP_OK) free_dm_state(plan);
     return st;
 }
@@ -128,11 +130,12 @@ dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams
         st = bitslice_execute(plan, nbeams, nsamps_out, in, row_stride, in_beam_stride_bytes,
                               in_nbits, tscrunch, out_dev, out_beam_stride_bytes, f32, s);
         if (st == DEDISP_OK) {
-            plan->last_kernel = DEDISP_KERNEL_BITSLICE;
+            plan->last_kernel = plan->bitslice_kind;
             return DEDISP_OK;
         }
         // INVALID_ARG from bitslice_execute means "plan does not fit this kernel"
-        if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE) return st;
+        if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE || plan->want == DEDISP_KERNEL_PAIRS)
+            return st;
     }
     int direct_nbits = in_nbits;
     size_t direct_beam_stride = in_beam_stride_bytes;
@@ -273,7 +276,7 @@ dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps
             DEDISP_CUDA_TRY(plan, cudaMemcpyAsync((uint8_t *)out_host + off, (uint8_t *)plan->d_out_stage + off, bytes,
                                                   cudaMemcpyDeviceToHost, plan->copy_stream));
         }
-        plan->last_kernel = DEDISP_KERNEL_BITSLICE;
+        plan->last_kernel = plan->bitslice_kind;
         DEDISP_CUDA_TRY(plan, cudaStreamSynchronize(s));
         DEDISP_CUDA_TRY(plan, cudaStreamSynchronize(plan->copy_stream));
         return DEDISP_OK;
@@ -290,6 +293,7 @@ dedisp_status dedisp_destroy(dedisp_plan plan)
 {
     if (!plan) return DEDISP_OK;
     free_dm_state(plan);
+    cudaFree(plan->d_pair_rows);
     cudaFree(plan->d_planes);
     cudaFree(plan->d_in_stage);
     cudaFree(plan->d_out_stage);
@@ -333,7 +337,7 @@ dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out)
 
 dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which)
 {
-    if (!plan || (int)which < 0 || (int)which > 2) return DEDISP_ERR_INVALID_ARG;
+    if (!plan || (int)which < 0 || (int)which > 3) return DEDISP_ERR_INVALID_ARG;
     plan->want = which;
     return DEDISP_OK;
 }

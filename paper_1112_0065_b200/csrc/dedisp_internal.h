@@ -32,6 +32,19 @@ struct BitsliceTables {
     int max_off = 0;              // largest (delay >> 5) - window start over the table, words
 };
 
+// Tables of the pair-row path (pair_rows.cu): virtual channel p = channels 2p and 2p+1 summed at a fixed
+// delay difference; one 3-plane row per (pair, difference) that occurs in the DM list.
+struct PairTables {
+    uint32_t *d_rel = nullptr;      // [ngroups][npairs_pad][32] ((variant slot + window offset) bytes << 16) | shift
+    int32_t *d_ws = nullptr;        // [ngroups][npairs_pad] window start word (of channel 2p)
+    uint32_t *d_vinfo = nullptr;    // [ngroups][npairs_pad] first row | (rows - 1) << 28
+    int32_t *d_row_pair = nullptr;  // [nrows] pair of each row
+    int32_t *d_row_delta = nullptr; // [nrows] delay difference of each row
+    int nrows = 0;
+    int npairs_pad = 0;
+    bool usable = false;
+};
+
 struct dedisp_plan_s {
     int nchans = 0;
     double dt = 0, f_top = 0, df = 0;
@@ -42,12 +55,16 @@ struct dedisp_plan_s {
     int max_delay = -1;
     dedisp_kernel want = DEDISP_KERNEL_AUTO;
     int last_kernel = 0;
+    int bitslice_kind = DEDISP_KERNEL_BITSLICE;   // which tiled variant the last bitslice_execute ran
     int last_cuda_error = 0;
     // bit-sliced path: tables built by set_dm_list, scratch grown lazily by execute
     BitsliceGeom geom[9];         // [bit planes per sample]: 1, 2, 4, 8 = packed widths; 3, 5, 6 = time-scrunched sums
     BitsliceTables tab[2];        // [0] for the 96/224-word windows, [1] for the narrower 8-/6-plane windows
     uint32_t *d_planes = nullptr; // bit-plane copy of the input
     size_t planes_bytes = 0;
+    PairTables pairs;             // pair-row path (2-bit samples)
+    uint32_t *d_pair_rows = nullptr;
+    size_t pair_rows_bytes = 0;
     // dedisp_execute_host staging
     void *d_in_stage = nullptr;
     size_t in_stage_bytes = 0;
@@ -111,5 +128,10 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
                                int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
                                cudaStream_t s, const BitsliceRange *range = nullptr);
+// pair_rows.cu
+dedisp_status pair_prepare(dedisp_plan plan);       // after bitslice_prepare; leaves pairs.usable
+void pair_release(dedisp_plan plan);
+cudaError_t launch_pair_rows(const PairTables &T, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
+                             uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s);
 // DM groups of the plan's bit-sliced geometry for this sample width, or 0 if the kernel cannot serve it
 int bitslice_ngroups(dedisp_plan plan, int nbits);

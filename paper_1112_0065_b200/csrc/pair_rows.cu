@@ -1,0 +1,251 @@
+// pair_rows.cu -- set-up and pre-pass of the pair-row path of the tiled gather-sum (2-bit samples).
+//
+//   out[d][t] = sum_c in[c][t + delay[c][d]]                      (BASELINE.json:north_star)
+//             = sum_p S_{p, delta_p(d)}[t + delay[2p][d]],   S_{p,delta}[u] = in[2p][u] + in[2p+1][u + delta],
+//               delta_p(d) = delay[2p+1][d] - delay[2p][d]   (exact: the same integer sum, re-associated)
+//
+// Neighbouring trial DMs share delta_p, so the sum of a channel pair is formed ONCE per delay difference (a
+// "pair row" of 3 bit planes, built by pair_rows_kernel from the 2-bit planes) instead of once per trial; the
+// tiled kernel then adds nchans/2 three-plane rows per output sample instead of nchans two-plane rows.
+//   * pair_range_kernel : the range of delta_p over the whole DM list -> the list of rows to build;
+//   * pair_tables_kernel: per (DM group, pair) the first row the group's trials use, how many consecutive rows
+//     (<= Cfg3P::NV, else the plan stays on the plain path), window start and per-lane offset/shift words;
+//   * pair_rows_kernel  : the rows themselves, once per execute.
+#include <vector>
+
+#include "bitslice_common.cuh"
+#include "dedisp_internal.h"
+
+using namespace bs;
+
+namespace {
+
+// one warp per pair: min / max of delay[2p+1][d] - delay[2p][d] over all trials (0 for padding channels)
+__global__ void pair_range_kernel(const int32_t *__restrict__ delay, int nchans, int ndm, int npairs,
+                                  int32_t *__restrict__ dlo, int32_t *__restrict__ dhi)
+{
+    const int p = blockIdx.x, lane = threadIdx.x;
+    if (p >= npairs) return;
+    int lo = 0x7fffffff, hi = 0;
+    if (2 * p + 1 < nchans) {
+        const int32_t *d0 = delay + (size_t)(2 * p) * ndm, *d1 = d0 + ndm;
+        for (int d = lane; d < ndm; d += 32) {
+            const int v = d1[d] - d0[d];
+            lo = min(lo, v);
+            hi = max(hi, v);
+        }
+    } else {
+        lo = 0;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (lane == 0) {
+        dlo[p] = lo;
+        dhi[p] = hi;
+    }
+}
+
+// One block per DM group, threads over pairs.  flags[0] = largest window offset (words), flags[1] = 1 when a
+// (group, pair) needs more than nv consecutive rows.
+__global__ void pair_tables_kernel(const int32_t *__restrict__ delay, int nchans, int ndm,
+                                   const int32_t *__restrict__ sorted, int npairs_pad,
+                                   const int32_t *__restrict__ dlo, const int32_t *__restrict__ row0, int nv,
+                                   int slot_bytes, int skew_bytes, int32_t *__restrict__ ws, uint32_t *__restrict__ rel,
+                                   uint32_t *__restrict__ vinfo, int *flags)
+{
+    const int g = blockIdx.x;
+    int worst = 0;
+    for (int p = threadIdx.x; p < npairs_pad; p += blockDim.x) {
+        const size_t row = (size_t)g * npairs_pad + p;
+        if (2 * p >= nchans) {
+            ws[row] = 0;
+            vinfo[row] = (uint32_t)row0[p];
+            for (int l = 0; l < 32; ++l) rel[row * 32 + l] = 0;
+            continue;
+        }
+        const int32_t *d0 = delay + (size_t)(2 * p) * ndm;
+        const bool two = 2 * p + 1 < nchans;
+        const int first = sorted[g * 32];
+        const int w0 = (d0[first] >> 5) & ~3;
+        ws[row] = w0;
+        int lo = 0x7fffffff, hi = 0, last = first;
+        for (int l = 0; l < 32; ++l) {
+            const int d = sorted[g * 32 + l];
+            if (d >= 0) last = d;
+            const int v = two ? d0[ndm + last] - d0[last] : 0;
+            lo = min(lo, v);
+            hi = max(hi, v);
+        }
+        if (hi - lo + 1 > nv) {
+            atomicOr(flags + 1, 1);
+            hi = lo + nv - 1;
+        }
+        vinfo[row] = (uint32_t)(row0[p] + lo - dlo[p]) | ((uint32_t)(hi - lo) << 28);
+        last = first;
+        for (int l = 0; l < 32; ++l) {
+            const int d = sorted[g * 32 + l];
+            if (d >= 0) last = d;
+            const int dv = d0[last];
+            int v = (two ? d0[ndm + last] - dv : 0) - lo;
+            v = v > nv - 1 ? nv - 1 : v;
+            const int off = (dv >> 5) - w0;
+            worst = max(worst, off);
+            rel[row * 32 + l] = ((uint32_t)(off * 4 + v * slot_bytes + (v & 1) * skew_bytes) << 16) | (uint32_t)(dv & 31);
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) worst = max(worst, __shfl_xor_sync(0xffffffffu, worst, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(flags, worst);
+}
+
+// Row r = (pair p, difference delta): word w of its 3 planes = planes of in[2p][u] + in[2p+1][u + delta] for the
+// 32 samples u of word w.  Thread = 4 consecutive words (128-bit loads of the even channel and stores; the odd
+// channel is read at a word offset of delta >> 5, funnel-shifted by delta & 31).
+__global__ void __launch_bounds__(128)
+pair_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nchans_pad,
+                 const int32_t *__restrict__ row_pair, const int32_t *__restrict__ row_delta,
+                 uint32_t *__restrict__ rows, size_t rows_beam_pitch, int row_pitch)
+{
+    const int w = 4 * (blockIdx.y * blockDim.x + threadIdx.x);
+    const int r = blockIdx.x, b = blockIdx.z;
+    if (w >= row_pitch) return;
+    const int p = row_pair[r], delta = row_delta[r];
+    uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0, s2 = s0;
+    if (2 * p < nchans_pad) {
+        const uint32_t *a = raw + (size_t)b * raw_beam_pitch + (size_t)(2 * p) * 2 * row_pitch;
+        const uint32_t *o = a + 2 * (size_t)row_pitch;   // odd channel (nchans_pad is even)
+        const uint4 a0 = *reinterpret_cast<const uint4 *>(a + w);
+        const uint4 a1 = *reinterpret_cast<const uint4 *>(a + row_pitch + w);
+        const int wo = w + (delta >> 5), sh = delta & 31;
+        uint32_t q0[5], q1[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            const bool in = wo + j < row_pitch;
+            q0[j] = in ? o[wo + j] : 0u;
+            q1[j] = in ? o[row_pitch + wo + j] : 0u;
+        }
+        const uint32_t A0[4] = {a0.x, a0.y, a0.z, a0.w}, A1[4] = {a1.x, a1.y, a1.z, a1.w};
+        uint32_t R0[4], R1[4], R2[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t b0 = __funnelshift_r(q0[j], q0[j + 1], sh), b1 = __funnelshift_r(q1[j], q1[j + 1], sh);
+            const uint32_t k = A0[j] & b0;
+            R0[j] = A0[j] ^ b0;
+            R1[j] = A1[j] ^ b1 ^ k;
+            R2[j] = (A1[j] & b1) | (k & (A1[j] ^ b1));
+        }
+        s0 = make_uint4(R0[0], R0[1], R0[2], R0[3]);
+        s1 = make_uint4(R1[0], R1[1], R1[2], R1[3]);
+        s2 = make_uint4(R2[0], R2[1], R2[2], R2[3]);
+    }
+    uint32_t *dst = rows + (size_t)b * rows_beam_pitch + (size_t)r * 3 * row_pitch + w;
+    *reinterpret_cast<uint4 *>(dst) = s0;
+    *reinterpret_cast<uint4 *>(dst + row_pitch) = s1;
+    *reinterpret_cast<uint4 *>(dst + 2 * (size_t)row_pitch) = s2;
+}
+
+}  // namespace
+
+void pair_release(dedisp_plan p)
+{
+    PairTables &T = p->pairs;
+    cudaFree(T.d_rel);
+    cudaFree(T.d_ws);
+    cudaFree(T.d_vinfo);
+    cudaFree(T.d_row_pair);
+    cudaFree(T.d_row_delta);
+    T = PairTables();
+}
+
+// Called after bitslice_prepare: same DM groups (tab[0]) and the 96-word windows of Cfg3P.  A plan the pair
+// rows cannot serve (too few channels or trials to pay for the rows, a group whose trials need more than
+// Cfg3P::NV differences of a pair, offsets beyond the window) leaves pairs.usable false; that is not an error.
+dedisp_status pair_prepare(dedisp_plan p)
+{
+    pair_release(p);
+    const BitsliceGeom &G2 = p->geom[2];
+    const BitsliceTables &B = p->tab[0];
+    if (!G2.usable || !B.d_order || p->nchans < 2) return DEDISP_OK;
+    using C = Cfg3P;
+    PairTables &T = p->pairs;
+    const int npairs_pad = ((G2.nchans_pad / 2) + CH_PAD - 1) / CH_PAD * CH_PAD;
+    const int ndm = p->ndm, ngroups = B.ngroups;
+    int32_t *d_lo = nullptr, *d_hi = nullptr, *d_row0 = nullptr;
+    int *d_flags = nullptr;
+    std::vector<int32_t> lo(npairs_pad), hi(npairs_pad), row0(npairs_pad);
+    cudaError_t e = cudaMalloc(&d_lo, sizeof(int32_t) * npairs_pad);
+    if (e == cudaSuccess) e = cudaMalloc(&d_hi, sizeof(int32_t) * npairs_pad);
+    if (e == cudaSuccess) e = cudaMalloc(&d_row0, sizeof(int32_t) * npairs_pad);
+    if (e == cudaSuccess) e = cudaMalloc(&d_flags, 2 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(d_flags, 0, 2 * sizeof(int));
+    if (e == cudaSuccess) {
+        pair_range_kernel<<<npairs_pad, 32>>>(p->d_delay, p->nchans, ndm, npairs_pad, d_lo, d_hi);
+        ++g_launch_count;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(lo.data(), d_lo, sizeof(int32_t) * npairs_pad, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(hi.data(), d_hi, sizeof(int32_t) * npairs_pad, cudaMemcpyDeviceToHost);
+    long long nrows = 0;
+    bool fits = true;
+    if (e == cudaSuccess) {
+        for (int q = 0; q < npairs_pad; ++q) {
+            row0[q] = (int32_t)nrows;
+            nrows += (long long)hi[q] - lo[q] + 1;
+            if (nrows > 0x07ffffff) { fits = false; break; }
+        }
+    }
+    if (e == cudaSuccess && fits) {
+        std::vector<int32_t> rp((size_t)nrows), rd((size_t)nrows);
+        for (int q = 0; q < npairs_pad; ++q)
+            for (int v = 0; v <= hi[q] - lo[q]; ++v) {
+                rp[(size_t)row0[q] + v] = q;
+                rd[(size_t)row0[q] + v] = lo[q] + v;
+            }
+        const size_t ntab = (size_t)ngroups * npairs_pad;
+        e = cudaMemcpy(d_row0, row0.data(), sizeof(int32_t) * npairs_pad, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_row_pair, sizeof(int32_t) * (size_t)nrows);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_row_delta, sizeof(int32_t) * (size_t)nrows);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_ws, sizeof(int32_t) * ntab);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_vinfo, sizeof(uint32_t) * ntab);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_rel, sizeof(uint32_t) * ntab * 32);
+        if (e == cudaSuccess)
+            e = cudaMemcpy(T.d_row_pair, rp.data(), sizeof(int32_t) * (size_t)nrows, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess)
+            e = cudaMemcpy(T.d_row_delta, rd.data(), sizeof(int32_t) * (size_t)nrows, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) {
+            pair_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, B.d_order, npairs_pad, d_lo, d_row0,
+                                                 C::NV, C::vslot_words<C::WIN_S>() * 4, C::VSKEW * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
+            ++g_launch_count;
+            e = cudaGetLastError();
+        }
+        int flags[2] = {0, 0};
+        if (e == cudaSuccess) e = cudaMemcpy(flags, d_flags, sizeof(flags), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) {
+            T.nrows = (int)nrows;
+            T.npairs_pad = npairs_pad;
+            T.usable = !flags[1] && flags[0] + C::TILE_WORDS + 1 <= C::WIN_S;
+        }
+    }
+    cudaFree(d_lo);
+    cudaFree(d_hi);
+    cudaFree(d_row0);
+    cudaFree(d_flags);
+    if (e != cudaSuccess) {
+        p->last_cuda_error = (int)e;
+        pair_release(p);
+        return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
+    }
+    if (!T.usable) pair_release(p);
+    return DEDISP_OK;
+}
+
+cudaError_t launch_pair_rows(const PairTables &T, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
+                             uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s)
+{
+    const dim3 block(128), grid(T.nrows, (row_pitch / 4 + 127) / 128, nbeams);
+    pair_rows_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
+                                            rows_beam_pitch, row_pitch);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
