@@ -265,7 +265,7 @@ def run_ours(args) -> None:
     achieved = adds / mm
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
                 "frac": achieved / alu_peak, "traffic": ncu_traffic_bytes(args.config),
-                "kernel": {2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows (Cfg3P)"}.get(
+                "kernel": {2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows"}.get(
                     kernel_used, "direct_kernel"),
                 "kernel_ms": mm * 1e3, "prepass_ms": statistics.mean(pre_ms),
                 "kernel_share_of_step": mm * 1e3 / ms_per_step,

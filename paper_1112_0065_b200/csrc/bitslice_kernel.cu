@@ -33,6 +33,9 @@ using namespace bs;
 #ifndef PAIRS_GAIN_DEN
 #define PAIRS_GAIN_DEN 5
 #endif
+#ifndef PAIRS8_AUTO
+#define PAIRS8_AUTO 1          // 8-bit pair rows (wide8: 59.9 -> 41.2 ms per step; the same break-even holds)
+#endif
 #ifndef PAIRS_MAX_BYTES
 #define PAIRS_MAX_BYTES (24ull << 30)
 #endif
@@ -522,22 +525,23 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-// Pair rows (pair_rows.cu): 2-bit planes -> one 3-plane row per (channel pair, delay difference) -> the tiled
-// kernel over nchans/2 virtual channels (Cfg3P).  Same DM groups, tiles and row pitch as Cfg2.
-dedisp_status execute_pairs(dedisp_plan plan, int nbeams, long long nsamps_out, const uint8_t *in,
-                            size_t row_stride, size_t in_beam_stride, void *out, size_t out_beam_stride,
-                            int out_f32, cudaStream_t s, const BitsliceRange &range)
+// Pair rows (pair_rows.cu): RAWNB-bit planes -> one (RAWNB+1)-plane row per (channel pair, delay difference) ->
+// the tiled kernel over nchans/2 virtual channels (geometry C).  Same DM groups, tiles and row pitch as the
+// plain geometry of the sample width.
+template <class C, int RAWNB>
+dedisp_status execute_pairs(dedisp_plan plan, const PairTables &T, int nbeams, long long nsamps_out,
+                            const uint8_t *in, size_t row_stride, size_t in_beam_stride, void *out,
+                            size_t out_beam_stride, int out_f32, cudaStream_t s, const BitsliceRange &range)
 {
-    using C = Cfg3P;
-    static_assert(C::TILE_WORDS == Cfg2::TILE_WORDS, "pair rows share the tiling of the 2-bit planes");
-    const PairTables &T = plan->pairs;
-    const BitsliceGeom &G = plan->geom[geom_index(2)];
+    static_assert(C::NB == RAWNB + 1, "a pair sum has one more plane than a sample");
+    const BitsliceGeom &G = plan->geom[geom_index(RAWNB)];
     const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
     const long long pitch =
         (((long long)(plan->max_delay >> 5) + ntiles * C::TILE_WORDS + C::WIN_S + 4) + 3) & ~3ll;
     if (ntiles > 0x7fffffff / C::TILE_WORDS || pitch > 0x7fffffff || nbeams > 65535) return DEDISP_ERR_INVALID_ARG;
-    const size_t raw_beam = (size_t)G.nchans_pad * 2 * (size_t)pitch;
+    const size_t raw_beam = (size_t)G.nchans_pad * RAWNB * (size_t)pitch;
     const size_t rows_beam = (size_t)T.nrows * C::NB * (size_t)pitch;
+    if ((unsigned long long)nbeams * T.nrows * C::NB > 0x7fffffffull) return DEDISP_ERR_INVALID_ARG;
     const size_t need_raw = raw_beam * (size_t)nbeams * 4, need_rows = rows_beam * (size_t)nbeams * 4;
     if (plan->planes_bytes < need_raw) {
         cudaFree(plan->d_planes);
@@ -563,9 +567,9 @@ dedisp_status execute_pairs(dedisp_plan plan, int nbeams, long long nsamps_out, 
     DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device));
     if (plan->timing) cudaEventRecord(plan->ev[0], s);
     if (range.prepass) {
-        DEDISP_CUDA_TRY(plan, launch_planes(2, in, in_beam_stride, row_stride, plan->nchans, nbeams, plan->d_planes,
-                                            (int)pitch, G.nchans_pad, s));
-        DEDISP_CUDA_TRY(plan, launch_pair_rows(T, plan->d_planes, raw_beam, G.nchans_pad, plan->d_pair_rows,
+        DEDISP_CUDA_TRY(plan, launch_planes(RAWNB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
+                                            plan->d_planes, (int)pitch, G.nchans_pad, s));
+        DEDISP_CUDA_TRY(plan, launch_pair_rows(T, RAWNB, plan->d_planes, raw_beam, G.nchans_pad, plan->d_pair_rows,
                                                rows_beam, (int)pitch, nbeams, s));
     }
     if (plan->timing) {
@@ -580,7 +584,7 @@ dedisp_status execute_pairs(dedisp_plan plan, int nbeams, long long nsamps_out, 
         if (!enc) return DEDISP_ERR_CUDA;
         const cuuint64_t dims[2] = {(cuuint64_t)pitch, (cuuint64_t)nbeams * T.nrows * C::NB};
         const cuuint64_t strides[1] = {(cuuint64_t)pitch * 4};
-        const cuuint32_t box[2] = {(cuuint32_t)C::plane_words<C::WIN_S>(), (cuuint32_t)C::NB};
+        const cuuint32_t box[2] = {(cuuint32_t)C::template plane_words<C::WIN_S>(), (cuuint32_t)C::NB};
         const cuuint32_t estr[2] = {1, 1};
         if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, plan->d_pair_rows, dims, strides, box, estr,
                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -604,13 +608,20 @@ dedisp_status execute_pairs(dedisp_plan plan, int nbeams, long long nsamps_out, 
     P.g_begin = range.g_begin;
     P.ntiles = (int)ntiles;
     P.nbeams = nbeams;
+    // rows beyond L2: tile-major inside blocks of gblock groups, as in execute_cfg
     P.gblock = 1;
+    if (rows_beam * 4 > (size_t)64 << 20 && RAWNB == 8) {
+        const double spread = (double)(plan->max_delay >> 5) + 1.0;
+        int gb = (int)std::sqrt((double)sms * C::TILE_WORDS * G.ngroups / spread);
+        P.gblock = gb < 1 ? 1 : gb > P.ngroups ? P.ngroups : gb;
+    }
     P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
                (nbeams == 1 || out_beam_stride % 16 == 0);
     const long long nitems = (long long)nbeams * P.ngroups * ntiles;
     const int grid = (int)(nitems < sms ? nitems : sms);
-    // channel blocks as in execute_cfg: a pair sum is at most 6
-    long long cblk = (((1ll << C::NP) - 1) / 6) / CH_PAD * CH_PAD;
+    // channel blocks as in execute_cfg: a pair sum is at most 2 (2^RAWNB - 1)
+    long long cblk = (((1ll << C::NP) - 1) / (2 * ((1ll << RAWNB) - 1))) / CH_PAD * CH_PAD;
+    if (cblk < CH_PAD) return DEDISP_ERR_INVALID_ARG;
     if (cblk > T.npairs_pad) cblk = T.npairs_pad;
     for (long long c0 = 0; c0 < T.npairs_pad; c0 += cblk) {
         const long long c1 = c0 + cblk < T.npairs_pad ? c0 + cblk : T.npairs_pad;
@@ -651,21 +662,25 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     if (rg.g_begin < 0 || rg.g_count < 0 || rg.g_begin + rg.g_count > G.ngroups) return DEDISP_ERR_INVALID_ARG;
     // pair rows: 2-bit samples at full time resolution.  AUTO takes them when the DM list is long enough for
     // the rows (built once per execute, ~max_delay/2 + nchans/2 of them) to pay for themselves.
-    const bool pairs_fit = nbits == 2 && tscrunch == 1 && plan->pairs.usable;
+    const PairTables &PT = nbits == 8 ? plan->pairs8 : plan->pairs;
+    const bool pairs_fit = (nbits == 2 || nbits == 8) && tscrunch == 1 && PT.usable;
     if (plan->want == DEDISP_KERNEL_PAIRS && !pairs_fit) return DEDISP_ERR_INVALID_ARG;
     bool pairs_pay = false;
     if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO) {
-        const PairTables &T = plan->pairs;
-        const long long ntiles = (nsamps_out + Cfg3P::TILE_SAMPS - 1) / Cfg3P::TILE_SAMPS;
-        const unsigned long long bytes = (unsigned long long)T.nrows * Cfg3P::NB * 4ull * (unsigned long long)nbeams *
-                                         (unsigned long long)((plan->max_delay >> 5) + ntiles * Cfg3P::TILE_WORDS + 128);
-        pairs_pay = (long long)PAIRS_GAIN_DEN * G.ngroups * T.npairs_pad >= (long long)PAIRS_GAIN_NUM * T.nrows &&
-                    bytes <= PAIRS_MAX_BYTES;
+        const int tile_words = nbits == 8 ? Cfg9P::TILE_WORDS : Cfg3P::TILE_WORDS;
+        const long long ntiles = (nsamps_out + 32 * tile_words - 1) / (32 * tile_words);
+        const unsigned long long bytes = (unsigned long long)PT.nrows * (nbits + 1) * 4ull * (unsigned long long)nbeams *
+                                         (unsigned long long)((plan->max_delay >> 5) + ntiles * tile_words + 128);
+        pairs_pay = (long long)PAIRS_GAIN_DEN * G.ngroups * PT.npairs_pad >= (long long)PAIRS_GAIN_NUM * PT.nrows &&
+                    bytes <= PAIRS_MAX_BYTES && (nbits == 2 || PAIRS8_AUTO);
     }
     if (pairs_fit && (plan->want == DEDISP_KERNEL_PAIRS || pairs_pay)) {
         plan->bitslice_kind = DEDISP_KERNEL_PAIRS;
-        return execute_pairs(plan, nbeams, nsamps_out, in, row_stride, in_beam_stride, out, out_beam_stride,
-                             out_f32, s, rg);
+        if (nbits == 8)
+            return execute_pairs<Cfg9P, 8>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                           out_beam_stride, out_f32, s, rg);
+        return execute_pairs<Cfg3P, 2>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                       out_beam_stride, out_f32, s, rg);
     }
     plan->bitslice_kind = DEDISP_KERNEL_BITSLICE;
 #define BS_RUN(CFG)                                                                                   \

@@ -62,7 +62,8 @@ struct dedisp_plan_s {
     BitsliceTables tab[2];        // [0] for the 96/224-word windows, [1] for the narrower 8-/6-plane windows
     uint32_t *d_planes = nullptr; // bit-plane copy of the input
     size_t planes_bytes = 0;
-    PairTables pairs;             // pair-row path (2-bit samples)
+    PairTables pairs;             // pair-row path, 2-bit samples (Cfg3P, DM groups of tab[0])
+    PairTables pairs8;            // pair-row path, 8-bit samples (Cfg9P, DM groups of tab[1])
     uint32_t *d_pair_rows = nullptr;
     size_t pair_rows_bytes = 0;
     // dedisp_execute_host staging
@@ -131,7 +132,7 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
 // pair_rows.cu
 dedisp_status pair_prepare(dedisp_plan plan);       // after bitslice_prepare; leaves pairs.usable
 void pair_release(dedisp_plan plan);
-cudaError_t launch_pair_rows(const PairTables &T, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
+cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
                              uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s);
 // DM groups of the plan's bit-sliced geometry for this sample width, or 0 if the kernel cannot serve it
 int bitslice_ngroups(dedisp_plan plan, int nbits);

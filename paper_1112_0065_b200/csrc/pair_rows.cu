@@ -145,11 +145,46 @@ pair_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nc
     *reinterpret_cast<uint4 *>(dst + 2 * (size_t)row_pitch) = s2;
 }
 
+// 8-bit samples: thread = one word of the 9 planes of in[2p][u] + in[2p+1][u + delta] (ripple-carry adder on
+// the bit planes: 8 full adders per word, i.e. per 32 samples).
+__global__ void __launch_bounds__(128)
+pair_rows8_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nchans_pad,
+                  const int32_t *__restrict__ row_pair, const int32_t *__restrict__ row_delta,
+                  uint32_t *__restrict__ rows, size_t rows_beam_pitch, int row_pitch)
+{
+    const int w = blockIdx.y * blockDim.x + threadIdx.x;
+    const int r = blockIdx.x, b = blockIdx.z;
+    if (w >= row_pitch) return;
+    const int p = row_pair[r], delta = row_delta[r];
+    uint32_t s[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) s[k] = 0u;
+    if (2 * p < nchans_pad) {
+        const uint32_t *a = raw + (size_t)b * raw_beam_pitch + (size_t)(2 * p) * 8 * row_pitch;
+        const uint32_t *o = a + 8 * (size_t)row_pitch;
+        const int wo = w + (delta >> 5), sh = delta & 31;
+        const bool in0 = wo < row_pitch, in1 = wo + 1 < row_pitch;
+        uint32_t carry = 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const uint32_t x = a[(size_t)k * row_pitch + w];
+            const uint32_t lo = in0 ? o[(size_t)k * row_pitch + wo] : 0u;
+            const uint32_t hi = in1 ? o[(size_t)k * row_pitch + wo + 1] : 0u;
+            const uint32_t y = __funnelshift_r(lo, hi, sh);
+            s[k] = x ^ y ^ carry;
+            carry = (x & y) | (carry & (x ^ y));
+        }
+        s[8] = carry;
+    }
+    uint32_t *dst = rows + (size_t)b * rows_beam_pitch + (size_t)r * 9 * row_pitch + w;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) dst[(size_t)k * row_pitch] = s[k];
+}
+
 }  // namespace
 
-void pair_release(dedisp_plan p)
+static void release_tables(PairTables &T)
 {
-    PairTables &T = p->pairs;
     cudaFree(T.d_rel);
     cudaFree(T.d_ws);
     cudaFree(T.d_vinfo);
@@ -158,17 +193,20 @@ void pair_release(dedisp_plan p)
     T = PairTables();
 }
 
-// Called after bitslice_prepare: same DM groups (tab[0]) and the 96-word windows of Cfg3P.  A plan the pair
-// rows cannot serve (too few channels or trials to pay for the rows, a group whose trials need more than
-// Cfg3P::NV differences of a pair, offsets beyond the window) leaves pairs.usable false; that is not an error.
-dedisp_status pair_prepare(dedisp_plan p)
+void pair_release(dedisp_plan p)
 {
-    pair_release(p);
-    const BitsliceGeom &G2 = p->geom[2];
-    const BitsliceTables &B = p->tab[0];
+    release_tables(p->pairs);
+    release_tables(p->pairs8);
+}
+
+// Called after bitslice_prepare: same DM groups as the raw geometry (B) and the windows of pair geometry C.  A
+// plan the pair rows cannot serve (a group whose trials need more than C::NV differences of a pair, offsets
+// beyond the window) leaves T.usable false; that is not an error.
+template <class C>
+static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G2, const BitsliceTables &B, PairTables &T)
+{
+    release_tables(T);
     if (!G2.usable || !B.d_order || p->nchans < 2) return DEDISP_OK;
-    using C = Cfg3P;
-    PairTables &T = p->pairs;
     const int npairs_pad = ((G2.nchans_pad / 2) + CH_PAD - 1) / CH_PAD * CH_PAD;
     const int ndm = p->ndm, ngroups = B.ngroups;
     int32_t *d_lo = nullptr, *d_hi = nullptr, *d_row0 = nullptr;
@@ -215,7 +253,7 @@ dedisp_status pair_prepare(dedisp_plan p)
             e = cudaMemcpy(T.d_row_delta, rd.data(), sizeof(int32_t) * (size_t)nrows, cudaMemcpyHostToDevice);
         if (e == cudaSuccess) {
             pair_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, B.d_order, npairs_pad, d_lo, d_row0,
-                                                 C::NV, C::vslot_words<C::WIN_S>() * 4, C::VSKEW * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
+                                                 C::NV, C::template vslot_words<C::WIN_S>() * 4, C::VSKEW * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
             ++g_launch_count;
             e = cudaGetLastError();
         }
@@ -233,19 +271,34 @@ dedisp_status pair_prepare(dedisp_plan p)
     cudaFree(d_flags);
     if (e != cudaSuccess) {
         p->last_cuda_error = (int)e;
-        pair_release(p);
+        release_tables(T);
         return e == cudaErrorMemoryAllocation ? DEDISP_ERR_ALLOC : DEDISP_ERR_CUDA;
     }
-    if (!T.usable) pair_release(p);
+    if (!T.usable) release_tables(T);
     return DEDISP_OK;
 }
 
-cudaError_t launch_pair_rows(const PairTables &T, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
-                             uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s)
+dedisp_status pair_prepare(dedisp_plan p)
 {
-    const dim3 block(128), grid(T.nrows, (row_pitch / 4 + 127) / 128, nbeams);
-    pair_rows_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
-                                            rows_beam_pitch, row_pitch);
+    dedisp_status st = prepare_tables<Cfg3P>(p, p->geom[2], p->tab[0], p->pairs);
+    if (st == DEDISP_OK) st = prepare_tables<Cfg9P>(p, p->geom[8], p->tab[1], p->pairs8);
+    return st;
+}
+
+cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t *raw, size_t raw_beam_pitch,
+                             int nchans_pad, uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams,
+                             cudaStream_t s)
+{
+    const dim3 block(128);
+    if (raw_nbits == 2) {
+        const dim3 grid(T.nrows, (row_pitch / 4 + 127) / 128, nbeams);
+        pair_rows_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
+                                                rows_beam_pitch, row_pitch);
+    } else {
+        const dim3 grid(T.nrows, (row_pitch + 127) / 128, nbeams);
+        pair_rows8_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
+                                                 rows_beam_pitch, row_pitch);
+    }
     ++g_launch_count;
     return cudaGetLastError();
 }

@@ -114,7 +114,7 @@ def test_host_call_leaves_in_dm_group_ranges():
 
 
 def test_plans_the_pair_rows_cannot_serve_are_refused_when_forced():
-    # tiny config: one group of 32 trials spans > 100 delay differences of a pair; 8-bit samples; time scrunch
+    # tiny config: one group of 32 trials spans > 100 delay differences of a pair; 4-bit samples
     w = W.CONFIGS["tiny"]
     delay, md, x = oracle_inputs(w)
     p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
@@ -124,11 +124,47 @@ def test_plans_the_pair_rows_cannot_serve_are_refused_when_forced():
     dd.dedisp_set_kernel(p, dd.DEDISP_KERNEL_AUTO)       # AUTO still serves the plan
     assert np.array_equal(gpu_dedisperse(p, x, 2, w.nsamps_out)[0], oracle.dedisperse(delay, x[0], 2, w.nsamps_out))
     dd.dedisp_destroy(p)
-    w8 = HTRU.scaled(nchans=64, df=-6.0, ndm=40, dm_hi=10.0, nsamps_out=500, nbits=8, kind="gauss8")
-    _, md8, x8 = oracle_inputs(w8)
-    p = make_plan(w8.nchans, w8.dt, w8.f_top, w8.df, w8.dms(), dd.DEDISP_KERNEL_PAIRS)
-    with pytest.raises(dd.DedispError):
-        gpu_dedisperse(p, x8, 8, w8.nsamps_out)
+    w4 = HTRU.scaled(ndm=40, dm_hi=STEP * 39, nsamps_out=500, nbits=4, kind="uniform")
+    _, md4, x4 = oracle_inputs(w4)
+    p = make_plan(w4.nchans, w4.dt, w4.f_top, w4.df, w4.dms(), dd.DEDISP_KERNEL_PAIRS)
+    with pytest.raises(dd.DedispError):      # pair rows exist for 2- and 8-bit samples
+        gpu_dedisperse(p, x4, 4, w4.nsamps_out)
+    dd.dedisp_destroy(p)
+
+
+WIDE8 = W.CONFIGS["wide8"]
+STEP8 = 2000.0 / 2047         # DM step of the wideband list
+
+
+@pytest.mark.parametrize("nchans,dm_lo,ndm,nsamps,od", [
+    (4096, 0.0, 40, 1500, "u32"), (4096, 1950.0, 50, 1409, "f32"), (1001, 900.0, 70, 3000, "u32"),
+    (512, 1200.0, 33, 2817, "f32"), (2, 0.0, 3, 50, "u32"),
+])
+def test_eight_bit_pair_rows(nchans, dm_lo, ndm, nsamps, od):
+    # 9-plane rows (Cfg9P): wideband channelisation, bottom and top of its DM range, odd channel count,
+    # ragged tiles; bit-exact against the oracle
+    w = WIDE8.scaled(nchans=nchans, ndm=ndm, dm_lo=dm_lo, dm_hi=dm_lo + STEP8 * (ndm - 1), nsamps_out=nsamps,
+                     out_dtype=od)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w, md)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    got = gpu_dedisperse(p, x[None], 8, w.nsamps_out, od)[0]
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
+    want = oracle.dedisperse(delay, x, 8, w.nsamps_out)
+    assert np.array_equal(got, want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
+def test_eight_bit_extreme_values_and_beams():
+    # all samples 255: every pair sum is 510 (all carries of the row adder), every output 255 * nchans
+    w = WIDE8.scaled(nchans=4096, ndm=40, dm_hi=STEP8 * 39, nsamps_out=1000, nbeams=2)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = np.full((2, w.nchans, w.nsamps_out + md), 0xFF, dtype=np.uint8)
+    x[1, ::3] = 0x80
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    got = gpu_dedisperse(p, x, 8, w.nsamps_out)
+    assert np.all(got[0] == 255 * w.nchans)
+    assert np.array_equal(got[1], oracle.dedisperse(delay, x[1], 8, w.nsamps_out))
     dd.dedisp_destroy(p)
 
 
