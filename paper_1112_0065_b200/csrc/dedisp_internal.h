@@ -38,8 +38,9 @@ struct PairTables {
     uint32_t *d_rel = nullptr;      // [ngroups][npairs_pad][32] ((variant slot + window offset) bytes << 16) | shift
     int32_t *d_ws = nullptr;        // [ngroups][npairs_pad] window start word (of channel 2p)
     uint32_t *d_vinfo = nullptr;    // [ngroups][npairs_pad] first row | (rows - 1) << 28
-    int32_t *d_row_pair = nullptr;  // [nrows] pair of each row
-    int32_t *d_row_delta = nullptr; // [nrows] delay difference of each row
+    int32_t *d_pair_row0 = nullptr; // [npairs_pad] first row of each pair ...
+    int32_t *d_pair_dlo = nullptr;  // [npairs_pad] ... its delay difference (rows of a pair: consecutive differences)
+    int32_t *d_pair_cnt = nullptr;  // [npairs_pad] rows of the pair
     int nrows = 0;
     int npairs_pad = 0;
     bool usable = false;

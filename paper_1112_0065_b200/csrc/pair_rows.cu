@@ -10,7 +10,8 @@
 //   * pair_range_kernel : the range of delta_p over the whole DM list -> the list of rows to build;
 //   * pair_tables_kernel: per (DM group, pair) the first row the group's trials use, how many consecutive rows
 //     (<= Cfg3P::NV, else the plan stays on the plain path), window start and per-lane offset/shift words;
-//   * pair_rows_kernel  : the rows themselves, once per execute.
+//   * pair_rows_kernel  : the rows themselves, once per execute (a thread writes all rows of its pair for its
+//     four words).
 #include <vector>
 
 #include "bitslice_common.cuh"
@@ -99,86 +100,63 @@ __global__ void pair_tables_kernel(const int32_t *__restrict__ delay, int nchans
     if ((threadIdx.x & 31) == 0) atomicMax(flags, worst);
 }
 
-// Row r = (pair p, difference delta): word w of its 3 planes = planes of in[2p][u] + in[2p+1][u + delta] for the
-// 32 samples u of word w.  Thread = 4 consecutive words (128-bit loads of the even channel and stores; the odd
-// channel is read at a word offset of delta >> 5, funnel-shifted by delta & 31).
-__global__ void __launch_bounds__(128)
+// All rows of pair p (differences lo .. lo + n - 1, consecutive rows from row0): word w of the NB + 1 planes of
+// row (p, delta) = planes of in[2p][u] + in[2p+1][u + delta] for the 32 samples u of word w (a bit-sliced ripple
+// adder: NB full adders per word).  Thread = 4 consecutive words: the even channel is loaded once (128-bit
+// loads), the odd channel's 5 words per plane at word offset delta >> 5 are re-read only when that offset
+// changes and funnel-shifted by delta & 31 for every row, so a row costs its 128-bit stores and nothing else.
+template <int NB>
+__global__ void __launch_bounds__(64)
 pair_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nchans_pad,
-                 const int32_t *__restrict__ row_pair, const int32_t *__restrict__ row_delta,
-                 uint32_t *__restrict__ rows, size_t rows_beam_pitch, int row_pitch)
+                 const int32_t *__restrict__ pair_row0, const int32_t *__restrict__ pair_dlo,
+                 const int32_t *__restrict__ pair_cnt, uint32_t *__restrict__ rows, size_t rows_beam_pitch,
+                 int row_pitch)
 {
     const int w = 4 * (blockIdx.y * blockDim.x + threadIdx.x);
-    const int r = blockIdx.x, b = blockIdx.z;
+    const int p = blockIdx.x, b = blockIdx.z;
     if (w >= row_pitch) return;
-    const int p = row_pair[r], delta = row_delta[r];
-    uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0, s2 = s0;
-    if (2 * p < nchans_pad) {
-        const uint32_t *a = raw + (size_t)b * raw_beam_pitch + (size_t)(2 * p) * 2 * row_pitch;
-        const uint32_t *o = a + 2 * (size_t)row_pitch;   // odd channel (nchans_pad is even)
-        const uint4 a0 = *reinterpret_cast<const uint4 *>(a + w);
-        const uint4 a1 = *reinterpret_cast<const uint4 *>(a + row_pitch + w);
-        const int wo = w + (delta >> 5), sh = delta & 31;
-        uint32_t q0[5], q1[5];
+    const int lo = pair_dlo[p], n = pair_cnt[p];
+    const size_t rstride = (size_t)(NB + 1) * row_pitch;
+    uint32_t *dst = rows + (size_t)b * rows_beam_pitch + (size_t)pair_row0[p] * rstride + w;
+    if (2 * p >= nchans_pad) {
+        for (int i = 0; i < n; ++i, dst += rstride)
 #pragma unroll
-        for (int j = 0; j < 5; ++j) {
-            const bool in = wo + j < row_pitch;
-            q0[j] = in ? o[wo + j] : 0u;
-            q1[j] = in ? o[row_pitch + wo + j] : 0u;
-        }
-        const uint32_t A0[4] = {a0.x, a0.y, a0.z, a0.w}, A1[4] = {a1.x, a1.y, a1.z, a1.w};
-        uint32_t R0[4], R1[4], R2[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t b0 = __funnelshift_r(q0[j], q0[j + 1], sh), b1 = __funnelshift_r(q1[j], q1[j + 1], sh);
-            const uint32_t k = A0[j] & b0;
-            R0[j] = A0[j] ^ b0;
-            R1[j] = A1[j] ^ b1 ^ k;
-            R2[j] = (A1[j] & b1) | (k & (A1[j] ^ b1));
-        }
-        s0 = make_uint4(R0[0], R0[1], R0[2], R0[3]);
-        s1 = make_uint4(R1[0], R1[1], R1[2], R1[3]);
-        s2 = make_uint4(R2[0], R2[1], R2[2], R2[3]);
+            for (int k = 0; k <= NB; ++k) *reinterpret_cast<uint4 *>(dst + (size_t)k * row_pitch) = make_uint4(0, 0, 0, 0);
+        return;
     }
-    uint32_t *dst = rows + (size_t)b * rows_beam_pitch + (size_t)r * 3 * row_pitch + w;
-    *reinterpret_cast<uint4 *>(dst) = s0;
-    *reinterpret_cast<uint4 *>(dst + row_pitch) = s1;
-    *reinterpret_cast<uint4 *>(dst + 2 * (size_t)row_pitch) = s2;
-}
-
-// 8-bit samples: thread = one word of the 9 planes of in[2p][u] + in[2p+1][u + delta] (ripple-carry adder on
-// the bit planes: 8 full adders per word, i.e. per 32 samples).
-__global__ void __launch_bounds__(128)
-pair_rows8_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nchans_pad,
-                  const int32_t *__restrict__ row_pair, const int32_t *__restrict__ row_delta,
-                  uint32_t *__restrict__ rows, size_t rows_beam_pitch, int row_pitch)
-{
-    const int w = blockIdx.y * blockDim.x + threadIdx.x;
-    const int r = blockIdx.x, b = blockIdx.z;
-    if (w >= row_pitch) return;
-    const int p = row_pair[r], delta = row_delta[r];
-    uint32_t s[9];
+    const uint32_t *a = raw + (size_t)b * raw_beam_pitch + (size_t)(2 * p) * NB * row_pitch;
+    const uint32_t *o = a + (size_t)NB * row_pitch;   // odd channel (nchans_pad is even)
+    uint32_t x[NB][4], q[NB][5];
 #pragma unroll
-    for (int k = 0; k < 9; ++k) s[k] = 0u;
-    if (2 * p < nchans_pad) {
-        const uint32_t *a = raw + (size_t)b * raw_beam_pitch + (size_t)(2 * p) * 8 * row_pitch;
-        const uint32_t *o = a + 8 * (size_t)row_pitch;
-        const int wo = w + (delta >> 5), sh = delta & 31;
-        const bool in0 = wo < row_pitch, in1 = wo + 1 < row_pitch;
-        uint32_t carry = 0u;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const uint32_t x = a[(size_t)k * row_pitch + w];
-            const uint32_t lo = in0 ? o[(size_t)k * row_pitch + wo] : 0u;
-            const uint32_t hi = in1 ? o[(size_t)k * row_pitch + wo + 1] : 0u;
-            const uint32_t y = __funnelshift_r(lo, hi, sh);
-            s[k] = x ^ y ^ carry;
-            carry = (x & y) | (carry & (x ^ y));
-        }
-        s[8] = carry;
+    for (int k = 0; k < NB; ++k) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(a + (size_t)k * row_pitch + w);
+        x[k][0] = v.x; x[k][1] = v.y; x[k][2] = v.z; x[k][3] = v.w;
     }
-    uint32_t *dst = rows + (size_t)b * rows_beam_pitch + (size_t)r * 9 * row_pitch + w;
+    int cur = -1;
+    for (int i = 0; i < n; ++i, dst += rstride) {
+        const int delta = lo + i, sh = delta & 31;
+        if ((delta >> 5) != cur) {
+            cur = delta >> 5;
+            const int wo = w + cur;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) dst[(size_t)k * row_pitch] = s[k];
+            for (int k = 0; k < NB; ++k)
+#pragma unroll
+                for (int j = 0; j < 5; ++j) q[k][j] = wo + j < row_pitch ? o[(size_t)k * row_pitch + wo + j] : 0u;
+        }
+        uint32_t c[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+        for (int k = 0; k < NB; ++k) {
+            uint32_t s[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t y = __funnelshift_r(q[k][j], q[k][j + 1], sh);
+                s[j] = x[k][j] ^ y ^ c[j];
+                c[j] = (x[k][j] & y) | (c[j] & (x[k][j] ^ y));
+            }
+            *reinterpret_cast<uint4 *>(dst + (size_t)k * row_pitch) = make_uint4(s[0], s[1], s[2], s[3]);
+        }
+        *reinterpret_cast<uint4 *>(dst + (size_t)NB * row_pitch) = make_uint4(c[0], c[1], c[2], c[3]);
+    }
 }
 
 }  // namespace
@@ -188,8 +166,9 @@ static void release_tables(PairTables &T)
     cudaFree(T.d_rel);
     cudaFree(T.d_ws);
     cudaFree(T.d_vinfo);
-    cudaFree(T.d_row_pair);
-    cudaFree(T.d_row_delta);
+    cudaFree(T.d_pair_row0);
+    cudaFree(T.d_pair_dlo);
+    cudaFree(T.d_pair_cnt);
     T = PairTables();
 }
 
@@ -234,23 +213,19 @@ static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G2, const
         }
     }
     if (e == cudaSuccess && fits) {
-        std::vector<int32_t> rp((size_t)nrows), rd((size_t)nrows);
-        for (int q = 0; q < npairs_pad; ++q)
-            for (int v = 0; v <= hi[q] - lo[q]; ++v) {
-                rp[(size_t)row0[q] + v] = q;
-                rd[(size_t)row0[q] + v] = lo[q] + v;
-            }
-        const size_t ntab = (size_t)ngroups * npairs_pad;
-        e = cudaMemcpy(d_row0, row0.data(), sizeof(int32_t) * npairs_pad, cudaMemcpyHostToDevice);
-        if (e == cudaSuccess) e = cudaMalloc(&T.d_row_pair, sizeof(int32_t) * (size_t)nrows);
-        if (e == cudaSuccess) e = cudaMalloc(&T.d_row_delta, sizeof(int32_t) * (size_t)nrows);
+        std::vector<int32_t> cnt(npairs_pad);
+        for (int q = 0; q < npairs_pad; ++q) cnt[q] = hi[q] - lo[q] + 1;
+        const size_t ntab = (size_t)ngroups * npairs_pad, pbytes = sizeof(int32_t) * npairs_pad;
+        e = cudaMemcpy(d_row0, row0.data(), pbytes, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_pair_row0, pbytes);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_pair_dlo, pbytes);
+        if (e == cudaSuccess) e = cudaMalloc(&T.d_pair_cnt, pbytes);
         if (e == cudaSuccess) e = cudaMalloc(&T.d_ws, sizeof(int32_t) * ntab);
         if (e == cudaSuccess) e = cudaMalloc(&T.d_vinfo, sizeof(uint32_t) * ntab);
         if (e == cudaSuccess) e = cudaMalloc(&T.d_rel, sizeof(uint32_t) * ntab * 32);
-        if (e == cudaSuccess)
-            e = cudaMemcpy(T.d_row_pair, rp.data(), sizeof(int32_t) * (size_t)nrows, cudaMemcpyHostToDevice);
-        if (e == cudaSuccess)
-            e = cudaMemcpy(T.d_row_delta, rd.data(), sizeof(int32_t) * (size_t)nrows, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(T.d_pair_row0, row0.data(), pbytes, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(T.d_pair_dlo, lo.data(), pbytes, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(T.d_pair_cnt, cnt.data(), pbytes, cudaMemcpyHostToDevice);
         if (e == cudaSuccess) {
             pair_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, B.d_order, npairs_pad, d_lo, d_row0,
                                                  C::NV, C::template vslot_words<C::WIN_S>() * 4, C::VSKEW * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
@@ -289,16 +264,13 @@ cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t 
                              int nchans_pad, uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams,
                              cudaStream_t s)
 {
-    const dim3 block(128);
-    if (raw_nbits == 2) {
-        const dim3 grid(T.nrows, (row_pitch / 4 + 127) / 128, nbeams);
-        pair_rows_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
-                                                rows_beam_pitch, row_pitch);
-    } else {
-        const dim3 grid(T.nrows, (row_pitch + 127) / 128, nbeams);
-        pair_rows8_kernel<<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_row_pair, T.d_row_delta, rows,
-                                                 rows_beam_pitch, row_pitch);
-    }
+    const dim3 block(64), grid(T.npairs_pad, (row_pitch / 4 + 63) / 64, nbeams);
+    if (raw_nbits == 2)
+        pair_rows_kernel<2><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,
+                                                   T.d_pair_cnt, rows, rows_beam_pitch, row_pitch);
+    else
+        pair_rows_kernel<8><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,
+                                                   T.d_pair_cnt, rows, rows_beam_pitch, row_pitch);
     ++g_launch_count;
     return cudaGetLastError();
 }
