@@ -39,6 +39,18 @@ def test_htru_shape_low_mid_and_top_of_the_dm_range(dm_lo, ndm, od):
     _check(w, od=od)
 
 
+@pytest.mark.parametrize("od", ["u32", "f32"])
+def test_delay_differences_beyond_one_word(od):
+    # DM 2050 .. 2156 on the HTRU channelisation: pair delay differences reach 66 samples, so the rows of a pair
+    # cross the 32- and 64-sample word boundaries (the row pre-pass re-reads the odd channel at a new word
+    # offset in the middle of a pair's row list) and the lowest pairs start beyond one word
+    w = HTRU.scaled(ndm=128, dm_lo=2050.0, dm_hi=2050.0 + STEP * 127, nsamps_out=4100, out_dtype=od)
+    delay, _ = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    delta = delay[1::2] - delay[0::2]
+    assert delta.max() >= 64 and np.any((delta.min(axis=1) < 32) & (delta.max(axis=1) >= 32))
+    _check(w, od=od)
+
+
 @pytest.mark.parametrize("nchans,df,dm_hi,ndm,nsamps", [
     (2, -100.0, 0.4, 5, 100), (3, -50.0, 0.5, 33, 700), (37, -7.0, 3.0, 40, 1921), (1023, -0.39, 50.0, 64, 1920),
     (130, -2.5, 15.0, 97, 3841), (64, -6.25, 1.8, 32, 4096),
@@ -152,6 +164,20 @@ def test_eight_bit_pair_rows(nchans, dm_lo, ndm, nsamps, od):
     assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
     want = oracle.dedisperse(delay, x, 8, w.nsamps_out)
     assert np.array_equal(got, want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
+def test_eight_bit_delay_differences_beyond_one_word():
+    # DM 4000 .. 4062 on the wideband channelisation: differences up to 39 samples, crossing the word boundary
+    w = WIDE8.scaled(nchans=4096, ndm=64, dm_lo=4000.0, dm_hi=4000.0 + STEP8 * 63, nsamps_out=1500)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    delta = delay[1::2] - delay[0::2]
+    assert np.any((delta.min(axis=1) < 32) & (delta.max(axis=1) >= 32))
+    x = W.generate(w, md)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    got = gpu_dedisperse(p, x[None], 8, w.nsamps_out)[0]
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
+    assert np.array_equal(got, oracle.dedisperse(delay, x, 8, w.nsamps_out))
     dd.dedisp_destroy(p)
 
 
