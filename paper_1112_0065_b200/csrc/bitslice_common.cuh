@@ -154,13 +154,16 @@ using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160, BS6_NSPLIT>;
 #ifndef BS3P_NW
 #define BS3P_NW 15
 #endif
+#ifndef BS3P_W
+#define BS3P_W 4
+#endif
 #ifndef BS3P_TREE_K
 #define BS3P_TREE_K 3
 #endif
 #ifndef BS3P_NSTAGE
 #define BS3P_NSTAGE 3
 #endif
-using Cfg3P = Cfg<3, BS3P_NW, 4, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3>;
+using Cfg3P = Cfg<3, BS3P_NW, BS3P_W, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3>;
 // ... and of two adjacent 8-bit channels: 9-plane rows, three 3-plane adder trees per chunk of 8 pairs, same
 // tile as Cfg8, sums < 2^20 (2048 pairs x 510); a stage is 82 KB, so the ring has two
 #ifndef BS9P_NW
@@ -175,6 +178,18 @@ using Cfg3P = Cfg<3, BS3P_NW, 4, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3>;
 #ifndef BS9P_NSPLIT
 #define BS9P_NSPLIT 3
 #endif
+// ... and of two adjacent 4-bit channels (row f4): 5-plane rows, 8 pairs per stage (a stage is 56 KB), same tile
+// as Cfg4, sums < 2^16 (2048 pairs x 30)
+#ifndef BS5P_NW
+#define BS5P_NW 11
+#endif
+#ifndef BS5P_TREE_K
+#define BS5P_TREE_K 2
+#endif
+#ifndef BS5P_NSTAGE
+#define BS5P_NSTAGE 3
+#endif
+using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, 1, 3>;
 using Cfg9P = Cfg<9, BS9P_NW, 4, BS9P_TREE_K, BS9P_NSTAGE, 20, BS8_WIN_S, BS8_WIN_S, BS9P_NSPLIT, 3>;
 
 constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8

@@ -660,22 +660,25 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     const long long per_chan = (long long)tscrunch * ((1ll << nbits) - 1);
     if (!G.usable || CH_PAD * per_chan >= (1ll << G.nplanes_acc)) return DEDISP_ERR_INVALID_ARG;
     if (rg.g_begin < 0 || rg.g_count < 0 || rg.g_begin + rg.g_count > G.ngroups) return DEDISP_ERR_INVALID_ARG;
-    // pair rows: 2-bit samples at full time resolution.  AUTO takes them when the DM list is long enough for
+    // pair rows: 2-, 4- and 8-bit samples at full time resolution.  AUTO takes them when the DM list is long enough for
     // the rows (built once per execute, ~max_delay/2 + nchans/2 of them) to pay for themselves.
-    const PairTables &PT = nbits == 8 ? plan->pairs8 : plan->pairs;
-    const bool pairs_fit = (nbits == 2 || nbits == 8) && tscrunch == 1 && PT.usable;
+    const PairTables &PT = nbits == 8 ? plan->pairs8 : nbits == 4 ? plan->pairs4 : plan->pairs;
+    const bool pairs_fit = (nbits == 2 || nbits == 4 || nbits == 8) && tscrunch == 1 && PT.usable;
     if (plan->want == DEDISP_KERNEL_PAIRS && !pairs_fit) return DEDISP_ERR_INVALID_ARG;
     bool pairs_pay = false;
     if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO) {
-        const int tile_words = nbits == 8 ? Cfg9P::TILE_WORDS : Cfg3P::TILE_WORDS;
+        const int tile_words = nbits == 8 ? Cfg9P::TILE_WORDS : nbits == 4 ? Cfg5P::TILE_WORDS : Cfg3P::TILE_WORDS;
         const long long ntiles = (nsamps_out + 32 * tile_words - 1) / (32 * tile_words);
         const unsigned long long bytes = (unsigned long long)PT.nrows * (nbits + 1) * 4ull * (unsigned long long)nbeams *
                                          (unsigned long long)((plan->max_delay >> 5) + ntiles * tile_words + 128);
         pairs_pay = (long long)PAIRS_GAIN_DEN * G.ngroups * PT.npairs_pad >= (long long)PAIRS_GAIN_NUM * PT.nrows &&
-                    bytes <= PAIRS_MAX_BYTES && (nbits == 2 || PAIRS8_AUTO);
+                    bytes <= PAIRS_MAX_BYTES && (nbits != 8 || PAIRS8_AUTO);
     }
     if (pairs_fit && (plan->want == DEDISP_KERNEL_PAIRS || pairs_pay)) {
         plan->bitslice_kind = DEDISP_KERNEL_PAIRS;
+        if (nbits == 4)
+            return execute_pairs<Cfg5P, 4>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                           out_beam_stride, out_f32, s, rg);
         if (nbits == 8)
             return execute_pairs<Cfg9P, 8>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
                                            out_beam_stride, out_f32, s, rg);

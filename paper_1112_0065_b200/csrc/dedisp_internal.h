@@ -64,6 +64,7 @@ struct dedisp_plan_s {
     uint32_t *d_planes = nullptr; // bit-plane copy of the input
     size_t planes_bytes = 0;
     PairTables pairs;             // pair-row path, 2-bit samples (Cfg3P, DM groups of tab[0])
+    PairTables pairs4;            // pair-row path, 4-bit samples (Cfg5P, DM groups of tab[0])
     PairTables pairs8;            // pair-row path, 8-bit samples (Cfg9P, DM groups of tab[1])
     uint32_t *d_pair_rows = nullptr;
     size_t pair_rows_bytes = 0;

@@ -175,6 +175,7 @@ static void release_tables(PairTables &T)
 void pair_release(dedisp_plan p)
 {
     release_tables(p->pairs);
+    release_tables(p->pairs4);
     release_tables(p->pairs8);
 }
 
@@ -256,6 +257,7 @@ static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G2, const
 dedisp_status pair_prepare(dedisp_plan p)
 {
     dedisp_status st = prepare_tables<Cfg3P>(p, p->geom[2], p->tab[0], p->pairs);
+    if (st == DEDISP_OK) st = prepare_tables<Cfg5P>(p, p->geom[4], p->tab[0], p->pairs4);
     if (st == DEDISP_OK) st = prepare_tables<Cfg9P>(p, p->geom[8], p->tab[1], p->pairs8);
     return st;
 }
@@ -267,6 +269,9 @@ cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t 
     const dim3 block(64), grid(T.npairs_pad, (row_pitch / 4 + 63) / 64, nbeams);
     if (raw_nbits == 2)
         pair_rows_kernel<2><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,
+                                                   T.d_pair_cnt, rows, rows_beam_pitch, row_pitch);
+    else if (raw_nbits == 4)
+        pair_rows_kernel<4><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,
                                                    T.d_pair_cnt, rows, rows_beam_pitch, row_pitch);
     else
         pair_rows_kernel<8><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,

@@ -126,7 +126,7 @@ def test_host_call_leaves_in_dm_group_ranges():
 
 
 def test_plans_the_pair_rows_cannot_serve_are_refused_when_forced():
-    # tiny config: one group of 32 trials spans > 100 delay differences of a pair; 4-bit samples
+    # tiny config: one group of 32 trials spans > 100 delay differences of a pair; 1-bit samples
     w = W.CONFIGS["tiny"]
     delay, md, x = oracle_inputs(w)
     p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
@@ -136,11 +136,11 @@ def test_plans_the_pair_rows_cannot_serve_are_refused_when_forced():
     dd.dedisp_set_kernel(p, dd.DEDISP_KERNEL_AUTO)       # AUTO still serves the plan
     assert np.array_equal(gpu_dedisperse(p, x, 2, w.nsamps_out)[0], oracle.dedisperse(delay, x[0], 2, w.nsamps_out))
     dd.dedisp_destroy(p)
-    w4 = HTRU.scaled(ndm=40, dm_hi=STEP * 39, nsamps_out=500, nbits=4, kind="uniform")
-    _, md4, x4 = oracle_inputs(w4)
-    p = make_plan(w4.nchans, w4.dt, w4.f_top, w4.df, w4.dms(), dd.DEDISP_KERNEL_PAIRS)
-    with pytest.raises(dd.DedispError):      # pair rows exist for 2- and 8-bit samples
-        gpu_dedisperse(p, x4, 4, w4.nsamps_out)
+    w1 = HTRU.scaled(ndm=40, dm_hi=STEP * 39, nsamps_out=500, nbits=1, kind="uniform")
+    _, md1, x1 = oracle_inputs(w1)
+    p = make_plan(w1.nchans, w1.dt, w1.f_top, w1.df, w1.dms(), dd.DEDISP_KERNEL_PAIRS)
+    with pytest.raises(dd.DedispError):      # pair rows exist for 2-, 4- and 8-bit samples
+        gpu_dedisperse(p, x1, 1, w1.nsamps_out)
     dd.dedisp_destroy(p)
 
 
@@ -204,6 +204,55 @@ def test_full_size_gulp_auto_takes_the_pair_rows_and_equals_the_plain_tiled_kern
     assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
     dd.dedisp_set_kernel(p, dd.DEDISP_KERNEL_BITSLICE)
     b = gpu_dedisperse(p, x, 2, w.nsamps_out)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
+    assert np.array_equal(a, b)
+    dd.dedisp_destroy(p)
+
+
+# ---------------------------------------------------------------- 4-bit samples (row f4): 5-plane rows (Cfg5P)
+HTRU4 = W.CONFIGS["htru_gulp_4bit"]
+
+
+@pytest.mark.parametrize("nchans,dm_lo,ndm,nsamps,od", [
+    (1024, 0.0, 70, 3000, "u32"), (1024, 930.0, 84, 1409, "f32"), (1001, 480.0, 33, 2817, "u32"),
+    (1024, 2050.0, 64, 1500, "u32"), (2, 0.0, 3, 50, "f32"),
+])
+def test_four_bit_pair_rows(nchans, dm_lo, ndm, nsamps, od):
+    # 5-plane rows of two 4-bit channels: bottom, middle and top of the HTRU DM range, beyond it (delay
+    # differences across a word boundary), odd channel count, ragged tiles; bit-exact against the oracle
+    w = HTRU4.scaled(nchans=nchans, ndm=ndm, dm_lo=dm_lo, dm_hi=dm_lo + STEP * (ndm - 1), nsamps_out=nsamps,
+                     out_dtype=od)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w, md)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    got = gpu_dedisperse(p, x[None], 4, w.nsamps_out, od)[0]
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
+    want = oracle.dedisperse(delay, x, 4, w.nsamps_out)
+    assert np.array_equal(got, want if od == "u32" else oracle.to_f32(want))
+    dd.dedisp_destroy(p)
+
+
+def test_four_bit_extreme_values_and_beams():
+    # all samples 15: every pair sum is 30 (all five planes of a row), every output 15 * nchans
+    w = HTRU4.scaled(ndm=40, dm_hi=STEP * 39, nsamps_out=1000, nbeams=2)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = np.full((2, w.nchans, (w.nsamps_out + md + 1) // 2), 0xFF, dtype=np.uint8)
+    x[1, ::3] = 0x8F
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    got = gpu_dedisperse(p, x, 4, w.nsamps_out)
+    assert np.all(got[0] == 15 * w.nchans)
+    assert np.array_equal(got[1], oracle.dedisperse(delay, x[1], 4, w.nsamps_out))
+    dd.dedisp_destroy(p)
+
+
+def test_four_bit_pairs_equal_the_plain_tiled_kernel_at_full_size():
+    w = HTRU4
+    _, md, x = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    a = gpu_dedisperse(p, x, 4, w.nsamps_out)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
+    dd.dedisp_set_kernel(p, dd.DEDISP_KERNEL_BITSLICE)
+    b = gpu_dedisperse(p, x, 4, w.nsamps_out)
     assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
     assert np.array_equal(a, b)
     dd.dedisp_destroy(p)
