@@ -151,6 +151,9 @@ using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160, BS6_NSPLIT>;
 // channels, in[2p][t] + in[2p+1][t + delta], one 3-plane row per delay difference delta that occurs in the
 // DM list; the trials of a group need at most NV = 3 consecutive differences (else the plan stays on Cfg2).
 // Same tile as Cfg2 so that both paths share the DM groups and the row pitch.
+// (sweeps on B200, HTRU gulp, step ms: (NW,W,K,NSTAGE) = (15,4,3,3) 1.03, (15,4,3,2) 1.06 [1.05 at the time],
+//  (15,4,2,4) 1.13, (15,4,2,6) 1.14, (12,5,3,3) 1.13 [13 warps: 4 on one sub-partition, 128 registers, spills],
+//  (10,6,3,3) 1.14, (20,3,3,3) 1.18 [80 registers, spills]; 16 consumers and no producer warp: 1.17)
 #ifndef BS3P_NW
 #define BS3P_NW 15
 #endif
