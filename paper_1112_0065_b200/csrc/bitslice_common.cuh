@@ -181,16 +181,17 @@ using Cfg3P = Cfg<3, BS3P_NW, BS3P_W, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3
 #ifndef BS9P_NSPLIT
 #define BS9P_NSPLIT 3
 #endif
-// ... and of two adjacent 4-bit channels (row f4): 5-plane rows, 8 pairs per stage (a stage is 56 KB), same tile
-// as Cfg4, sums < 2^16 (2048 pairs x 30)
+// ... and of two adjacent 4-bit channels (row f4): 5-plane rows, same tile as Cfg4, sums < 2^16 (2048 pairs x
+// 30); 16 pairs per stage make a stage 110 KB, so the ring has two (sweep on B200, gulp at 4 bits, step ms:
+// (K,NSTAGE) = (3,2) 1.74, (2,3) 1.83, (2,4) 1.84)
 #ifndef BS5P_NW
 #define BS5P_NW 11
 #endif
 #ifndef BS5P_TREE_K
-#define BS5P_TREE_K 2
+#define BS5P_TREE_K 3
 #endif
 #ifndef BS5P_NSTAGE
-#define BS5P_NSTAGE 3
+#define BS5P_NSTAGE 2
 #endif
 using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, 1, 3>;
 using Cfg9P = Cfg<9, BS9P_NW, 4, BS9P_TREE_K, BS9P_NSTAGE, 20, BS8_WIN_S, BS8_WIN_S, BS9P_NSPLIT, 3>;
