@@ -72,7 +72,7 @@ typedef enum {
     DEDISP_KERNEL_DIRECT = 1,   /* one thread per output group, reads packed input from global */
     DEDISP_KERNEL_BITSLICE = 2, /* TMA-staged (DM x time) tiles, bit-plane carry-save adders */
     DEDISP_KERNEL_PAIRS = 3     /* the same tiled kernel on pair rows: in[2p][t] + in[2p+1][t + delta] is formed
-                                   once per delay difference delta of the DM list (3 bit planes) and the tiles
+                                   once per delay difference delta of the DM list (nbits + 1 bit planes) and the tiles
                                    add nchans/2 such rows -- the identical integer sum, re-associated.  2-, 4-
                                    and 8-bit samples; AUTO picks it when the plan fits (see dedisp_get_last_kernel),
                                    BITSLICE forces the plain tiled kernel */

@@ -1,4 +1,4 @@
-// pair_rows.cu -- set-up and pre-pass of the pair-row path of the tiled gather-sum (2-bit samples).
+// pair_rows.cu -- set-up and pre-pass of the pair-row path of the tiled gather-sum (2-, 4- and 8-bit samples).
 //
 //   out[d][t] = sum_c in[c][t + delay[c][d]]                      (BASELINE.json:north_star)
 //             = sum_p S_{p, delta_p(d)}[t + delay[2p][d]],   S_{p,delta}[u] = in[2p][u] + in[2p+1][u + delta],
