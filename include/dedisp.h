@@ -74,7 +74,9 @@ typedef enum {
     DEDISP_KERNEL_PAIRS = 3     /* the same tiled kernel on pair rows: in[2p][t] + in[2p+1][t + delta] is formed
                                    once per delay difference delta of the DM list (nbits + 1 bit planes) and the tiles
                                    add nchans/2 such rows -- the identical integer sum, re-associated.  2-, 4-
-                                   and 8-bit samples; AUTO picks it when the plan fits (see dedisp_get_last_kernel),
+                                   and 8-bit samples; AUTO picks it when the plan fits (see dedisp_get_last_kernel)
+                                   and falls back to the plain tiled kernel when the scratch for the rows
+                                   cannot be allocated (forced PAIRS then returns DEDISP_ERR_ALLOC);
                                    BITSLICE forces the plain tiled kernel */
 } dedisp_kernel;
 

@@ -666,7 +666,8 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     const bool pairs_fit = (nbits == 2 || nbits == 4 || nbits == 8) && tscrunch == 1 && PT.usable;
     if (plan->want == DEDISP_KERNEL_PAIRS && !pairs_fit) return DEDISP_ERR_INVALID_ARG;
     bool pairs_pay = false;
-    if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO) {
+    // (a DM-group range that continues an execute -- no pre-pass of its own -- stays on what the first range ran)
+    if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO && (rg.prepass || plan->bitslice_kind == DEDISP_KERNEL_PAIRS)) {
         const int tile_words = nbits == 8 ? Cfg9P::TILE_WORDS : nbits == 4 ? Cfg5P::TILE_WORDS : Cfg3P::TILE_WORDS;
         const long long ntiles = (nsamps_out + 32 * tile_words - 1) / (32 * tile_words);
         const unsigned long long bytes = (unsigned long long)PT.nrows * (nbits + 1) * 4ull * (unsigned long long)nbeams *
@@ -676,14 +677,16 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
     }
     if (pairs_fit && (plan->want == DEDISP_KERNEL_PAIRS || pairs_pay)) {
         plan->bitslice_kind = DEDISP_KERNEL_PAIRS;
-        if (nbits == 4)
-            return execute_pairs<Cfg5P, 4>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                           out_beam_stride, out_f32, s, rg);
-        if (nbits == 8)
-            return execute_pairs<Cfg9P, 8>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                           out_beam_stride, out_f32, s, rg);
-        return execute_pairs<Cfg3P, 2>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
-                                       out_beam_stride, out_f32, s, rg);
+        const dedisp_status st =
+            nbits == 4   ? execute_pairs<Cfg5P, 4>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                                   out_beam_stride, out_f32, s, rg)
+            : nbits == 8 ? execute_pairs<Cfg9P, 8>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                                   out_beam_stride, out_f32, s, rg)
+                         : execute_pairs<Cfg3P, 2>(plan, PT, nbeams, nsamps_out, in, row_stride, in_beam_stride, out,
+                                                   out_beam_stride, out_f32, s, rg);
+        // AUTO never fails where the plain tiled kernel would not: when the scratch for the rows cannot be
+        // allocated (nothing has been enqueued at that point) the call is served from the planes instead
+        if (st != DEDISP_ERR_ALLOC || plan->want != DEDISP_KERNEL_AUTO) return st;
     }
     plan->bitslice_kind = DEDISP_KERNEL_BITSLICE;
 #define BS_RUN(CFG)                                                                                   \

@@ -256,3 +256,32 @@ def test_four_bit_pairs_equal_the_plain_tiled_kernel_at_full_size():
     assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
     assert np.array_equal(a, b)
     dd.dedisp_destroy(p)
+
+
+def test_auto_falls_back_to_the_planes_when_the_row_scratch_cannot_be_allocated():
+    # the gulp's rows need 373 MB of scratch; with less than that free AUTO must still serve the call (plain tiled
+    # kernel), a forced PAIRS plan reports the failed allocation, and once memory is back AUTO takes the rows again
+    w = HTRU
+    _, md, x = oracle_inputs(w)
+    p = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    q = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_PAIRS)
+    ref = make_plan(w.nchans, w.dt, w.f_top, w.df, w.dms(), dd.DEDISP_KERNEL_BITSLICE)
+    want = gpu_dedisperse(ref, x, 2, w.nsamps_out)
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    filler = torch.empty(free - (700 << 20), dtype=torch.uint8, device="cuda")   # in + out + planes fit, rows do not
+    try:
+        got = gpu_dedisperse(p, x, 2, w.nsamps_out)
+        assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_BITSLICE
+        assert np.array_equal(got, want)
+        with pytest.raises(dd.DedispError) as e:
+            gpu_dedisperse(q, x, 2, w.nsamps_out)
+        assert e.value.status == dd.DEDISP_ERR_ALLOC
+    finally:
+        del filler
+        torch.cuda.empty_cache()
+    got = gpu_dedisperse(p, x, 2, w.nsamps_out)
+    assert dd.dedisp_get_last_kernel(p) == dd.DEDISP_KERNEL_PAIRS
+    assert np.array_equal(got, want)
+    for h in (p, q, ref):
+        dd.dedisp_destroy(h)
