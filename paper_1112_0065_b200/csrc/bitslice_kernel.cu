@@ -2,18 +2,21 @@
 //
 //   out[d][t] = sum_c in[c][t + delay[c][d]]       (BASELINE.json:north_star)
 //
-// B200 design:
-//   * a work item = (beam, group of 32 trial DMs, tile of 2048 output samples);
+// B200 design (the numbers are those of the 2-bit geometry Cfg2, see bitslice_common.cuh):
+//   * a work item = (beam, group of 32 trial DMs, tile of 1920 output samples);
 //     persistent CTAs (one per SM) walk the item list;
-//   * lane  = trial DM, warp = 4 consecutive 32-sample words, 16 consumer warps;
-//   * one producer warp stages, per 16-channel chunk, the window of bit-plane words
+//   * lane  = trial DM, warp = 4 consecutive 32-sample words, 15 consumer warps;
+//   * one producer warp stages, per 32-channel chunk, the window of bit-plane words
 //     the tile needs with 1-D TMA bulk copies (cp.async.bulk + mbarrier tx counts)
-//     into a 4-deep shared-memory ring, so neighbouring DMs reuse one staged window;
+//     into a 3-deep shared-memory ring, so neighbouring DMs reuse one staged window;
 //   * consumers never unpack to integers: a sample stays 2 bit planes, is aligned
 //     with one funnel shift per plane-word and is added with carry-save adders
 //     (2 LOP3 per full adder) into a 12-plane bit-sliced counter held in registers
 //     -- 32 additions per instruction, ~0.2 ALU ops per (channel, DM, sample);
-//   * the counter is un-sliced once per tile and written as uint32 / float32.
+//   * the counter is un-sliced once per tile and written as uint32 / float32;
+//   * pair rows (Cfg3P / Cfg5P / Cfg9P, pair_rows.cu): the same kernel on rows that hold the sum of two
+//     adjacent channels at a fixed delay difference (one more plane, half as many rows per tile), the
+//     1-3 rows a DM group uses of a pair staged as 2-D TMA boxes (cp.async.bulk.tensor.2d).
 #include <cuda.h>
 
 #include <cmath>
