@@ -105,8 +105,21 @@ __global__ void pair_tables_kernel(const int32_t *__restrict__ delay, int nchans
 // adder: NB full adders per word).  Thread = 4 consecutive words: the even channel is loaded once (128-bit
 // loads), the odd channel's 5 words per plane at word offset delta >> 5 are re-read only when that offset
 // changes and funnel-shifted by delta & 31 for every row, so a row costs its 128-bit stores and nothing else.
+// (sweep on B200, pre-pass ms of the HTRU gulp / the 8-bit wideband: block 32 0.097 / 2.00, 64 0.094 / 1.83,
+//  128 0.093 / 1.74, 128 with streaming stores 0.092 / 1.73, 64 with streaming stores 0.094 / 1.83)
+#ifndef PAIR_ROWS_STCS
+#define PAIR_ROWS_STCS 0
+#endif
+#if PAIR_ROWS_STCS
+#define PAIR_ROWS_STORE(p, v) __stcs((p), (v))
+#else
+#define PAIR_ROWS_STORE(p, v) (*(p) = (v))
+#endif
+#ifndef PAIR_ROWS_BLOCK
+#define PAIR_ROWS_BLOCK 128
+#endif
 template <int NB>
-__global__ void __launch_bounds__(64)
+__global__ void __launch_bounds__(PAIR_ROWS_BLOCK)
 pair_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nchans_pad,
                  const int32_t *__restrict__ pair_row0, const int32_t *__restrict__ pair_dlo,
                  const int32_t *__restrict__ pair_cnt, uint32_t *__restrict__ rows, size_t rows_beam_pitch,
@@ -153,9 +166,9 @@ pair_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nc
                 s[j] = x[k][j] ^ y ^ c[j];
                 c[j] = (x[k][j] & y) | (c[j] & (x[k][j] ^ y));
             }
-            *reinterpret_cast<uint4 *>(dst + (size_t)k * row_pitch) = make_uint4(s[0], s[1], s[2], s[3]);
+            PAIR_ROWS_STORE(reinterpret_cast<uint4 *>(dst + (size_t)k * row_pitch), make_uint4(s[0], s[1], s[2], s[3]));
         }
-        *reinterpret_cast<uint4 *>(dst + (size_t)NB * row_pitch) = make_uint4(c[0], c[1], c[2], c[3]);
+        PAIR_ROWS_STORE(reinterpret_cast<uint4 *>(dst + (size_t)NB * row_pitch), make_uint4(c[0], c[1], c[2], c[3]));
     }
 }
 
@@ -266,7 +279,7 @@ cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t 
                              int nchans_pad, uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams,
                              cudaStream_t s)
 {
-    const dim3 block(64), grid(T.npairs_pad, (row_pitch / 4 + 63) / 64, nbeams);
+    const dim3 block(PAIR_ROWS_BLOCK), grid(T.npairs_pad, (row_pitch / 4 + PAIR_ROWS_BLOCK - 1) / PAIR_ROWS_BLOCK, nbeams);
     if (raw_nbits == 2)
         pair_rows_kernel<2><<<grid, block, 0, s>>>(raw, raw_beam_pitch, nchans_pad, T.d_pair_row0, T.d_pair_dlo,
                                                    T.d_pair_cnt, rows, rows_beam_pitch, row_pitch);
