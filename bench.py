@@ -25,7 +25,7 @@ import numpy as np
 ROOT = Path(__file__).resolve().parent
 sys.path.insert(0, str(ROOT))
 from paper_1112_0065_b200 import replicas  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 
 SM_COUNT_NOMINAL = 148
 ADDS_PER_CLK_PER_SM = 128          # FP32/INT32 lane-adds per clock per SM
@@ -274,8 +274,9 @@ def run_ours(args) -> None:
                 "hbm_frac": ((in_bytes + out_bytes) / mm) / hbm_peak,
                 "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
     try:
-        probe = {n: dd.dedisp_probe_alu_rate(i) / 1e12 for i, n in
-                 enumerate(["iadd3", "lop3", "shf", "fadd", "imad", "lop3+imad", "lds32", "lds128", "prmt", "dp4a"])}
+        import bench_probe
+        bench_probe.build()
+        probe = {n: bench_probe.probe_alu_rate(i) / 1e12 for i, n in enumerate(bench_probe.NAMES)}
     except Exception as e:  # noqa: BLE001
         probe = {"error": str(e)}
     cpu = None

@@ -1,10 +1,12 @@
-// probe.cu -- register-only instruction-rate probe (dedisp_probe_alu_rate).
-// The bench uses it to MEASURE the ALU roofline denominator on the device it is
+// probe.cu -- register-only instruction-rate probe (probe_alu_rate), built into its own bench-side
+// library libdedisp_probe.so: it is a micro-benchmark, not part of the product ABI (include/dedisp.h).
+// bench.py uses it to MEASURE the ALU roofline denominator on the device it is
 // running on instead of trusting a spec sheet.
 // Each kernel runs 8 independent dependency chains per thread, 2048 iterations of
 // 8 ops, on 2 CTAs of 1024 threads per SM; results are folded and stored so that
 // nothing is optimised away.
-#include "dedisp_internal.h"
+#include <cuda_runtime.h>
+#include <stdint.h>
 
 #define CHAINS 8
 #define ITERS 2048
@@ -66,16 +68,20 @@ __global__ void __launch_bounds__(1024) probe_kernel(uint32_t *out, uint32_t see
     out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
-extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s)
+// which: 0 = IADD3 (u32 add), 1 = LOP3, 2 = SHF funnel shift, 3 = FADD, 4 = IMAD, 5 = LOP3+IMAD mix,
+// 6 = conflict-free LDS.32 (+ XOR), 7 = conflict-free LDS.128 (+ 4 XOR), 8 = PRMT, 9 = DP4A.
+// Writes lane-operations per second (warp instructions * 32 / s; for 6 and 7: lane-loads of 4 / 16 bytes).
+// Returns 0, or 1 = bad argument, 2 = CUDA error.
+extern "C" int probe_alu_rate(int which, double *lane_ops_per_s)
 {
-    if (!lane_ops_per_s || which < 0 || which > 9) return DEDISP_ERR_INVALID_ARG;
+    if (!lane_ops_per_s || which < 0 || which > 9) return 1;
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return DEDISP_ERR_CUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 2;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-        return DEDISP_ERR_CUDA;
+        return 2;
     const int blocks = 2 * sms, threads = 1024;
     uint32_t *d = nullptr;
-    if (cudaMalloc(&d, (size_t)blocks * threads * 4) != cudaSuccess) return DEDISP_ERR_ALLOC;
+    if (cudaMalloc(&d, (size_t)blocks * threads * 4) != cudaSuccess) return 2;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -94,11 +100,10 @@ extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s
             case 8: probe_kernel<8><<<blocks, threads>>>(d, 12345u + rep); break;
             default: probe_kernel<9><<<blocks, threads>>>(d, 12345u + rep); break;
         }
-        ++g_launch_count;
         cudaEventRecord(e1, 0);
         if (cudaEventSynchronize(e1) != cudaSuccess) {
             cudaFree(d);
-            return DEDISP_ERR_CUDA;
+            return 2;
         }
         float ms = 0;
         cudaEventElapsedTime(&ms, e0, e1);
@@ -109,5 +114,5 @@ extern "C" dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s
     cudaFree(d);
     const double ops = (double)blocks * threads * (double)ITERS * CHAINS;
     *lane_ops_per_s = ops / (best * 1e-3);
-    return DEDISP_OK;
+    return 0;
 }

@@ -338,14 +338,6 @@ unsigned long long dedisp_get_launch_count(void);
 int dedisp_get_last_cuda_error(dedisp_plan plan);
 const char *dedisp_get_error_string(dedisp_status status);
 
-/* Register-only instruction-rate probe used by the bench to MEASURE the ALU
- * roofline denominator on the device it runs on.  which: 0 = IADD3 (u32 add),
- * 1 = LOP3, 2 = SHF funnel shift, 3 = FADD, 4 = IMAD, 5 = LOP3+IMAD mix, 6 = conflict-free
- * LDS.32 (+ XOR), 7 = conflict-free LDS.128 (+ 4 XOR), 8 = PRMT, 9 = DP4A.
- * Writes lane-operations per second (warp instructions * 32 / s; for 6 and 7: lane-loads of 4 / 16
- * bytes) to *lane_ops_per_s. */
-dedisp_status dedisp_probe_alu_rate(int which, double *lane_ops_per_s);
-
 #ifdef __cplusplus
 }
 #endif

@@ -54,7 +54,6 @@ ABI = {
     "dedisp_get_launch_count": (ctypes.c_ulonglong, []),
     "dedisp_get_last_cuda_error": (_i, [_vp]),
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
-    "dedisp_probe_alu_rate": (_i, [_i, ctypes.POINTER(_d)]),
     "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
     "dedisp_matched_filter_rms_workspace_bytes": (_sz, [_ll, _ll, _i]),
     "dedisp_matched_filter_rms": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp, _vp, _vp,
@@ -195,12 +194,6 @@ def dedisp_get_last_kernel(plan: int) -> int:
 
 def dedisp_get_launch_count() -> int:
     return int(lib().dedisp_get_launch_count())
-
-
-def dedisp_probe_alu_rate(which: int) -> float:
-    v = _d()
-    _check(None, lib().dedisp_probe_alu_rate(which, ctypes.byref(v)), "dedisp_probe_alu_rate")
-    return v.value
 
 
 def dedisp_get_last_cuda_error(plan: int) -> int:

@@ -1,22 +1,28 @@
 """Builds libdedisp_b200.so in-tree with nvcc for sm_100a (no JIT cache, no torch).
 
     python -m paper_1112_0065_b200.build [--force] [--verbose]
+
+Every translation unit is compiled to an object file under csrc/build/ (in parallel, re-compiled
+only when it or a header changed) and the objects are linked into the shared library.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libdedisp_b200.so"
+OBJDIR = CSRC / "build"
 SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
-           "pair_rows.cu", "probe.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
+           "pair_rows.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--fmad=false", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "--fmad=false", "-Xptxas", "-v"]
 
 
 def _nvcc() -> str:
@@ -26,30 +32,61 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+def _headers() -> list[Path]:
+    return sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.cuh")) + [INCLUDE / "dedisp.h"]
+
+
 def stale() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    deps = [CSRC / s for s in SOURCES] + list(CSRC.glob("*.h")) + list(CSRC.glob("*.cuh")) \
-        + [INCLUDE / "dedisp.h"]
-    return any(d.stat().st_mtime > t for d in deps)
+    return any(d.stat().st_mtime > t for d in [CSRC / s for s in SOURCES] + _headers())
+
+
+def _compile(src: Path, obj: Path, defs: list[str]) -> tuple[int, str]:
+    cmd = [_nvcc(), *NVCC_FLAGS, *[f"-D{d}" for d in defs], f"-I{INCLUDE}", f"-I{CSRC}", "-c", "-o", str(obj), str(src)]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    return r.returncode, r.stdout + r.stderr
 
 
 def build(force: bool = False, verbose: bool = False, defs: list[str] | None = None,
-          out: Path | None = None) -> Path:
+          out: Path | None = None, sources: list[str] | None = None) -> Path:
     """defs/out: tuning variants for A/B runs (e.g. defs=["BS_NW=20"], out=Path("x.so"))."""
     target = Path(out) if out else LIB
-    if not force and not defs and not out and not stale():
+    defs = list(defs or [])
+    sources = list(sources or SOURCES)
+    if not force and not defs and not out and sources == SOURCES and not stale():
         return LIB
+    tag = hashlib.sha1(" ".join(defs).encode()).hexdigest()[:8] if defs else "default"
+    objdir = OBJDIR / tag
+    objdir.mkdir(parents=True, exist_ok=True)
+    hdr_t = max(h.stat().st_mtime for h in _headers())
+    jobs = []
+    for s in sources:
+        src, obj = CSRC / s, objdir / (Path(s).stem + ".o")
+        if force or not obj.exists() or obj.stat().st_mtime < max(src.stat().st_mtime, hdr_t):
+            jobs.append((src, obj))
+    logs = []
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        for (src, obj), (rc, text) in zip(jobs, ex.map(lambda j: _compile(j[0], j[1], defs), jobs)):
+            logs.append(f"==== {src.name}\n{text}")
+            if verbose or rc != 0:
+                sys.stderr.write(text)
+            if rc != 0:
+                obj.unlink(missing_ok=True)
+                raise RuntimeError(f"nvcc failed compiling {src.name}")
     tmp = target.with_suffix(f".tmp{os.getpid()}.so")
-    cmd = [_nvcc(), *NVCC_FLAGS, *[f"-D{d}" for d in (defs or [])], f"-I{INCLUDE}", f"-I{CSRC}",
-           "-o", str(tmp)] + [str(CSRC / s) for s in SOURCES]
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC", "-o", str(tmp)] + \
+          [str(objdir / (Path(s).stem + ".o")) for s in sources]
     r = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or r.returncode != 0:
-        sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed building libdedisp_b200.so")
-    (target.parent / (target.stem + "_ptxas.log")).write_text(r.stdout + r.stderr)
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError(f"nvcc failed linking {target.name}")
+    logp = target.parent / (target.stem + "_ptxas.log")
+    if jobs:
+        old = logp.read_text() if logp.exists() and not force else ""
+        keep = [blk for blk in old.split("==== ")[1:] if not any(blk.startswith(j[0].name) for j in jobs)]
+        logp.write_text("".join("==== " + b for b in keep) + "".join(logs))
     os.replace(tmp, target)
     return target
 

@@ -5,7 +5,7 @@ import torch
 
 import oracle
 import paper_1112_0065_b200 as dd
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 
 def oracle_inputs(w):

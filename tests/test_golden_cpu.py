@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 SURVEY_GOLDENS = {  # SURVEY.md Sec. 8(d), table "Generator goldens"
     "tiny": dict(in_sha256="7c2cb4eae172d38b5f530334bacd060ab05ae221251e3c999c7fbdcc82eeb8c1",

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 import oracle  # noqa: E402
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs  # noqa: E402
 
 

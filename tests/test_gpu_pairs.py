@@ -9,7 +9,7 @@ import torch
 
 import oracle
 import paper_1112_0065_b200 as dd
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs
 
 pytestmark = pytest.mark.gpu

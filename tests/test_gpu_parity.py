@@ -9,7 +9,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 import oracle  # noqa: E402
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs  # noqa: E402
 
 KERNELS = [dd.DEDISP_KERNEL_AUTO, dd.DEDISP_KERNEL_DIRECT]
@@ -306,7 +306,9 @@ def test_launch_counter_and_probe():
     p = make_plan(8, 64e-6, 1500.0, -10.0, [0.0, 10.0])
     assert dd.dedisp_get_launch_count() > n0
     dd.dedisp_destroy(p)
-    r = dd.dedisp_probe_alu_rate(0)
+    import bench_probe
+    bench_probe.build()
+    r = bench_probe.probe_alu_rate(0)
     assert 1e12 < r < 1e15
 
 

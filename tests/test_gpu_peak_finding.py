@@ -10,7 +10,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 from oracle import peak_finding as PF  # noqa: E402
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 
 
 def gpu_events(z, sigma, nsigma, max_events=None):

@@ -10,7 +10,7 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 from gpu_helpers import make_plan, oracle_inputs  # noqa: E402
 
 

@@ -9,7 +9,7 @@ torch = pytest.importorskip("torch")
 import oracle  # noqa: E402
 from oracle import rfi_mask as RM  # noqa: E402
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs  # noqa: E402
 
 

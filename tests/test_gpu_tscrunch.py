@@ -9,7 +9,7 @@ torch = pytest.importorskip("torch")
 import oracle  # noqa: E402
 from oracle import tscrunch as TS  # noqa: E402
 import paper_1112_0065_b200 as dd  # noqa: E402
-from paper_1112_0065_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 from gpu_helpers import make_plan  # noqa: E402
 
 FAST = [(1, 2), (1, 4), (1, 8), (1, 16), (2, 2), (2, 4), (2, 8), (2, 16), (4, 2), (4, 4), (4, 8)]

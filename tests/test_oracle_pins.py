@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 
 # ----------------------------------------------------------------- helpers

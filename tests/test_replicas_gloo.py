@@ -10,7 +10,7 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 from paper_1112_0065_b200 import replicas
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 
 def _worker(rank, world, port, q):

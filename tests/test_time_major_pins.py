@@ -4,7 +4,7 @@ import pytest
 
 import oracle
 from oracle import time_major as TM
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 
 def test_hand_typed_bytes():

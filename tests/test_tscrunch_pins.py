@@ -4,7 +4,7 @@ import pytest
 
 import oracle
 from oracle import tscrunch as TS
-from paper_1112_0065_b200 import workloads as W
+import workloads as W
 
 # the hand-worked example of SURVEY.md Sec. 8(c) (4 channels, f_top 1500, df -100, DMs 0/10/25),
 # rows of 32 two-bit samples, digits = samples t = 0..31
