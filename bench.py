@@ -108,63 +108,87 @@ def dist_setup(ngpus: int):
     return rank, world, local
 
 
-def cpu_baseline(w: W.Workload, seconds_hint: str = "", tscrunch: int = 1) -> dict:
-    """The oracle as it stands, on this box's host cores, on a bounded sample."""
+def cpu_model() -> str:
+    try:
+        for line in Path("/proc/cpuinfo").read_text().splitlines():
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_baseline(w: W.Workload, tscrunch: int = 1) -> dict:
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the workload: all cores and one
+    thread, best of 3 each (SURVEY.md Sec. 8(d) "CPU baseline timed beside it")."""
     import oracle
     delay, md = oracle.delay_table(w.nchans, tscrunch * w.dt, w.f_top, w.df, w.dms())
     x = W.generate(w.scaled(nbeams=1), tscrunch * (w.nsamps_out + md) - w.nsamps_out)
-    stride = max(1, (w.ndm * w.nsamps_out) // (1200 * 65536))   # ~ one HTRU gulp of work
+    stride = max(1, (w.ndm * w.nsamps_out) // (1200 * 65536))   # ~ one HTRU gulp of work for all cores
+
+    def run(sub, nthreads):
+        best, used = None, 0
+        for _ in range(3):
+            t0 = time.perf_counter()
+            if tscrunch > 1:
+                from oracle import tscrunch as TS
+                _, used = TS.dedisperse_tscrunch_bytes(sub, x, w.nbits, tscrunch, w.nsamps_out, return_threads=True)
+            else:
+                _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, nthreads=nthreads, return_threads=True)
+            dt = time.perf_counter() - t0
+            best = dt if best is None or dt < best else best
+        return best, used
+
     sub = np.ascontiguousarray(delay[:, ::stride])
-    t0 = time.perf_counter()
-    if tscrunch > 1:
-        from oracle import tscrunch as TS
-        _, used = TS.dedisperse_tscrunch_bytes(sub, x, w.nbits, tscrunch, w.nsamps_out, return_threads=True)
-    else:
-        _, used = oracle.dedisperse(sub, x, w.nbits, w.nsamps_out, return_threads=True)
-    dt = time.perf_counter() - t0
+    dt_all, used = run(sub, os.cpu_count() or 1)
     units = sub.shape[1] * w.nsamps_out
-    return {"value": units / dt, "unit": "DM-trial-samples/s", "cores": used, "kind": "oracle",
-            "sample": f"{sub.shape[1]} of {w.ndm} DM trials (every {stride}th) x {w.nsamps_out} samples "
-                      f"x {w.nchans} channels of {w.name}, one pass, {dt:.2f} s",
-            "rtf": (w.nsamps_out * w.dt) / (dt * w.ndm / sub.shape[1])}
+    res = {"value": units / dt_all, "unit": "DM-trial-samples/s", "cores": used, "kind": "oracle",
+           "cpu_model": cpu_model(), "nproc": os.cpu_count(), "best_of": 3, "seconds": dt_all,
+           "sample": f"{sub.shape[1]} of {w.ndm} DM trials (every {stride}th) x {w.nsamps_out} samples "
+                     f"x {w.nchans} channels of {w.name}, best of 3 passes, {dt_all:.2f} s",
+           "rtf": (w.nsamps_out * w.dt) / (dt_all * w.ndm / sub.shape[1])}
+    if tscrunch == 1:
+        sub1 = np.ascontiguousarray(delay[:, ::stride * 8])      # one thread: an eighth of that
+        dt_1, used1 = run(sub1, 1)
+        res["one_thread"] = {"value": sub1.shape[1] * w.nsamps_out / dt_1, "unit": "DM-trial-samples/s", "cores": used1,
+                             "seconds": dt_1, "sample": f"{sub1.shape[1]} of {w.ndm} DM trials (every {stride * 8}th), "
+                                                        f"best of 3 passes, {dt_1:.2f} s"}
+    return res
+
+
+def ncu_traffic(config: str):
+    """(DRAM bytes per launch of the dominant kernel, source file, commit of the capture) from the committed ncu
+    captures (profiles/traffic.csv: config,bytes_per_launch,source,commit), or (None, None, None)."""
+    p = ROOT / "profiles" / "traffic.csv"
+    if not p.exists():
+        return None, None, None
+    for line in p.read_text().splitlines():
+        f = [v.strip() for v in line.split(",")]
+        if len(f) >= 2 and f[0] == config:
+            try:
+                return float(f[1]), (f[2] if len(f) > 2 else None), (f[3] if len(f) > 3 else None)
+            except ValueError:
+                return None, None, None
+    return None, None, None
 
 
 def ncu_traffic_bytes(config: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (or None)."""
-    p = ROOT / "profiles" / "traffic.csv"
-    if not p.exists():
-        return None
-    for line in p.read_text().splitlines():
-        f = line.split(",")
-        if len(f) >= 2 and f[0] == config:
-            try:
-                return float(f[1])
-            except ValueError:
-                return None
-    return None
+    return ncu_traffic(config)[0]
 
 
-def run_ours(args) -> None:
-    import torch
-    import paper_1112_0065_b200 as dd
+KERNEL_NAMES = {1: "direct_kernel", 2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows"}
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
-    rank, world, local = dist_setup(args.gpus)
-    w = W.CONFIGS[args.config]
-    dev = torch.device("cuda", torch.cuda.current_device())
-    props = torch.cuda.get_device_properties(dev)
-    stream = torch.cuda.current_stream()
 
-    k = args.tscrunch   # row f4: blocks of k samples summed, trials dedispersed on the grid k*dt (reading R38)
-    if k > 1 and w.kind == "gauss2_pulses":
-        raise SystemExit("bench.py: --tscrunch is benched on the noise-only configs")
+def measure_dedisperse(torch, dd, w, k, kernel, steps, warmup, rank, world, dev, stream, flush, e2e_steps):
+    """W warm-ups + K timed steps of the hot path on workload w (inputs resident in HBM), CUDA events on the launching
+    stream, L2 flushed between iterations; optionally the end-to-end leg through dedisp_execute_host.  Returns the raw
+    measurements; nothing here is specific to the headline config."""
     plan = dd.dedisp_plan_create(w.nchans, k * w.dt, w.f_top, w.df)
     t0 = time.perf_counter()
     dd.dedisp_set_dm_list(plan, list(w.dms()))
     set_dm_ms = (time.perf_counter() - t0) * 1e3
     dd.dedisp_set_kernel(plan, {"auto": dd.DEDISP_KERNEL_AUTO, "bitslice": dd.DEDISP_KERNEL_BITSLICE,
-                                "pairs": dd.DEDISP_KERNEL_PAIRS}[args.kernel])
+                                "pairs": dd.DEDISP_KERNEL_PAIRS}[kernel])
     md = dd.dedisp_get_max_delay(plan)
     kw = {}
     if w.kind == "gauss2_pulses":   # pulse sweeps from the product's own delay builder
@@ -183,23 +207,16 @@ def run_ours(args) -> None:
     f32 = w.out_dtype == "f32"
     code = dd.DEDISP_OUT_F32 if f32 else dd.DEDISP_OUT_U32
     out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=torch.float32 if f32 else torch.int32, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
     in_bs, out_bs = nch * stride, w.ndm * w.nsamps_out * 4
+    if k == 1:
+        dd.dedisp_reserve(plan, nb, w.nsamps_out, w.nbits)     # the timed steps never allocate
 
     def step():
         dd.dedisp_execute_tscrunch(plan, k, nb, w.nsamps_out, x, in_bs, w.nbits, out, out_bs, code,
                                    stream.cuda_stream)
 
-    def host_step():
-        if k == 1:
-            return dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
-        x.copy_(host_in, non_blocking=True)
-        step()
-        host_out.copy_(out, non_blocking=True)
-        stream.synchronize()
-
     dd.dedisp_set_timing(plan, True)
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
     if world > 1:
@@ -209,8 +226,7 @@ def run_ours(args) -> None:
     sampler.start()
     time.sleep(0.15)
     launches0 = dd.dedisp_get_launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     main_ms, pre_ms = [], []
     torch.cuda.synchronize()
     wall0 = time.perf_counter()
@@ -229,56 +245,127 @@ def run_ours(args) -> None:
     step_ms = [a.elapsed_time(b) for a, b in ev]
     if world > 1:
         dist.barrier()
-    total_ms = replicas.max_over_ranks(sum(step_ms), dev)
-    ms_per_step = total_ms / args.steps
-    units_step = w.dm_trial_samples() * world
-    value = replicas.job_throughput(w.dm_trial_samples(), world, ms_per_step * 1e-3)
+    m = {"plan_md": md, "set_dm_ms": set_dm_ms, "step_ms": step_ms, "main_ms": main_ms, "pre_ms": pre_ms,
+         "launches": launches, "clocks": clocks, "wall": wall, "nb": nb, "in_bytes": nb * in_bs, "out_bytes": nb * out_bs,
+         "kernel_used": dd.dedisp_get_last_kernel(plan), "e2e_s": None, "same": None, "e2e_steps": e2e_steps}
+    if e2e_steps > 0:
+        # ---- end to end through the public host-buffer call (H2D + kernels + D2H inside the timing)
+        host_out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=out.dtype).pin_memory()
+        dd.dedisp_set_timing(plan, False)
 
-    # ---- end to end through the public host-buffer call (H2D + kernels + D2H inside the timing)
-    host_out = torch.empty((nb, w.ndm, w.nsamps_out), dtype=out.dtype).pin_memory()
-    dd.dedisp_set_timing(plan, False)
-    e2e_steps = max(2, min(args.steps, 5))
-    host_step()
-    if world > 1:
-        dist.barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+        def host_step():
+            if k == 1:
+                return dd.dedisp_execute_host(plan, nb, w.nsamps_out, host_in, w.nbits, host_out, code)
+            x.copy_(host_in, non_blocking=True)
+            step()
+            host_out.copy_(out, non_blocking=True)
+            stream.synchronize()
+
         host_step()
-    e2e_s = replicas.max_over_ranks((time.perf_counter() - t0) / e2e_steps, dev)
-    e2e_value = replicas.job_throughput(w.dm_trial_samples(), world, e2e_s)
-    same = bool(torch.equal(host_out.to(dev), out))
-    kernel_used = dd.dedisp_get_last_kernel(plan)
-    dd.dedisp_destroy(plan)
-
-    if rank != 0:
         if world > 1:
-            dist.destroy_process_group()
-        return
-    peaks = measured_peaks()
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            host_step()
+        m["e2e_s"] = (time.perf_counter() - t0) / e2e_steps
+        m["same"] = bool(torch.equal(host_out.to(dev), out))
+        m["kernel_used"] = dd.dedisp_get_last_kernel(plan)
+        del host_out
+    dd.dedisp_destroy(plan)
+    del x, out, host_in
+    torch.cuda.empty_cache()
+    return m
+
+
+def roofline_of(w, k, m, ms_per_step, props, peaks, config_name):
+    """north_star's roofline: the slower of nchans*ndm*nsamps adds at the ALU peak and the compulsory bytes at the HBM
+    bandwidth; `achieved` = adds / the dominant kernel's mean launch time (CUDA events inside the library, live)."""
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = props.multi_processor_count * ADDS_PER_CLK_PER_SM * sm_max_mhz * 1e6   # adds/s
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0)) * 1e9
     adds = w.adds() * k          # every fine sample is added once
-    in_bytes, out_bytes = nb * in_bs, nb * out_bs
-    t_alu, t_hbm = adds / alu_peak, (in_bytes + out_bytes) / hbm_peak
-    mm = statistics.mean(main_ms) * 1e-3
+    t_alu, t_hbm = adds / alu_peak, (m["in_bytes"] + m["out_bytes"]) / hbm_peak
+    mm = statistics.mean(m["main_ms"]) * 1e-3
     achieved = adds / mm
-    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
-                "frac": achieved / alu_peak, "traffic": ncu_traffic_bytes(args.config),
-                "kernel": {2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows"}.get(
-                    kernel_used, "direct_kernel"),
-                "kernel_ms": mm * 1e3, "prepass_ms": statistics.mean(pre_ms),
-                "kernel_share_of_step": mm * 1e3 / ms_per_step,
-                "peak_source": f"{props.multi_processor_count} SMs x {ADDS_PER_CLK_PER_SM} adds/clk x "
-                               f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz); see DESIGN.md",
-                "hbm_frac": ((in_bytes + out_bytes) / mm) / hbm_peak,
-                "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
+    traffic, tsrc, tcommit = ncu_traffic(config_name)
+    return {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
+            "frac": achieved / alu_peak, "traffic": traffic, "traffic_source": tsrc, "traffic_capture_commit": tcommit,
+            "kernel": KERNEL_NAMES.get(m["kernel_used"], "direct_kernel"),
+            "kernel_ms": mm * 1e3, "prepass_ms": statistics.mean(m["pre_ms"]),
+            "kernel_share_of_step": mm * 1e3 / ms_per_step,
+            "peak_source": f"{props.multi_processor_count} SMs x {ADDS_PER_CLK_PER_SM} adds/clk x "
+                           f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz); see DESIGN.md",
+            "algorithmic_bytes": m["in_bytes"] + m["out_bytes"],
+            "hbm_frac": ((m["in_bytes"] + m["out_bytes"]) / mm) / hbm_peak,
+            "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
+
+
+def run_ours(args) -> None:
+    import torch
+    import paper_1112_0065_b200 as dd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    rank, world, local = dist_setup(args.gpus)
+    w = W.CONFIGS[args.config]
+    dev = torch.device("cuda", torch.cuda.current_device())
+    props = torch.cuda.get_device_properties(dev)
+    stream = torch.cuda.current_stream()
+    peaks = measured_peaks()
+
+    k = args.tscrunch   # row f4: blocks of k samples summed, trials dedispersed on the grid k*dt (reading R38)
+    if k > 1 and w.kind == "gauss2_pulses":
+        raise SystemExit("bench.py: --tscrunch is benched on the noise-only configs")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    m = measure_dedisperse(torch, dd, w, k, args.kernel, args.steps, args.warmup, rank, world, dev, stream, flush,
+                           e2e_steps=max(2, min(args.steps, 5)))
+    total_ms = replicas.max_over_ranks(sum(m["step_ms"]), dev)
+    ms_per_step = total_ms / args.steps
+    value = replicas.job_throughput(w.dm_trial_samples(), world, ms_per_step * 1e-3)
+    e2e_s = replicas.max_over_ranks(m["e2e_s"], dev)
+    e2e_value = replicas.job_throughput(w.dm_trial_samples(), world, e2e_s)
+
+    if rank != 0:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+        return
+    roofline = roofline_of(w, k, m, ms_per_step, props, peaks, args.config)
     try:
         import bench_probe
         bench_probe.build()
         probe = {n: bench_probe.probe_alu_rate(i) / 1e12 for i, n in enumerate(bench_probe.NAMES)}
     except Exception as e:  # noqa: BLE001
         probe = {"error": str(e)}
+
+    # ---- the other BASELINE.json configs, timed the same way in the same run (N = 1, default config only)
+    per_config = None
+    if world == 1 and args.per_config and k == 1 and args.kernel == "auto" and args.config == "htru_gulp":
+        per_config = {}
+        for name in W.CONFIG_ORDER:
+            wc = W.CONFIGS[name]
+            if name == args.config:
+                mc, ms_c, rc, nsteps = m, ms_per_step, roofline, args.steps
+            else:
+                nsteps = max(5, min(args.steps, 10))
+                log(f"per_config: {name} ...")
+                mc = measure_dedisperse(torch, dd, wc, 1, "auto", nsteps, max(3, args.warmup), 0, 1, dev, stream, flush,
+                                        e2e_steps=0)
+                ms_c = statistics.mean(mc["step_ms"])
+                rc = roofline_of(wc, 1, mc, ms_c, props, peaks, name)
+            per_config[name] = {
+                "ms_per_step": ms_c, "kernel_ms": rc["kernel_ms"], "prepass_ms": rc["prepass_ms"],
+                "value": wc.dm_trial_samples() / (ms_c * 1e-3), "unit": "DM-trial-samples/s",
+                "real_time_factor": wc.obs_seconds() / (ms_c * 1e-3), "kernel": rc["kernel"],
+                "roofline": {"bound": "alu", "frac": rc["frac"], "achieved": rc["achieved"], "peak": rc["peak"],
+                             "unit": "Tadd/s", "traffic": rc["traffic"], "traffic_source": rc["traffic_source"]},
+                "step_roofline_frac": rc["step_roofline_frac"], "steps": nsteps, "warmup": max(3, args.warmup),
+                "dtype": wc.out_dtype, "gpu_launches": mc["launches"], "clocks": mc["clocks"],
+                "step_ms_min_med_max": [min(mc["step_ms"]), statistics.median(mc["step_ms"]), max(mc["step_ms"])],
+                "config": {"workload": name, "nchans": wc.nchans, "ndm": wc.ndm, "nsamps_out": wc.nsamps_out,
+                           "nbits": wc.nbits, "nbeams": wc.nbeams, "out_dtype": wc.out_dtype, "max_delay": mc["plan_md"]},
+                "note": "3 work items: launch-latency sized, roofline fraction meaningless" if name == "tiny" else None}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w, tscrunch=k)
@@ -287,24 +374,26 @@ def run_ours(args) -> None:
     res = {
         "metric": "DM-trial samples/sec", "value": value, "unit": "DM-trial-samples/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": w.out_dtype,
         "data": "synthetic",
         "config": {"workload": w.name, "nchans": w.nchans, "ndm": w.ndm, "nsamps_out": w.nsamps_out,
                    "nbits": w.nbits, "tscrunch": k, "nbeams_per_gpu": w.nbeams, "out_dtype": w.out_dtype,
-                   "max_delay": md, "l2": "256 MiB flush buffer zeroed between timed iterations",
+                   "max_delay": m["plan_md"], "l2": "256 MiB flush buffer zeroed between timed iterations",
                    "parallelism": f"replicas x{world} (one seeded beam set per GPU, no collective)"},
         "real_time_factor": k * w.obs_seconds() / (ms_per_step * 1e-3),
         "roofline": roofline, "cpu_baseline": cpu,
-        "e2e": {"value": e2e_value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": in_bytes,
-                "d2h_bytes_per_step": out_bytes, "steps": e2e_steps, "matches_device_run": same},
-        "gpu_launches": launches, "clocks": clocks, "alu_probe_Tlaneops": probe,
-        "set_dm_list_ms": set_dm_ms, "wall_s_timed_region": wall,
-        "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
+        "e2e": {"value": e2e_value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": m["in_bytes"],
+                "d2h_bytes_per_step": m["out_bytes"], "steps": m["e2e_steps"], "matches_device_run": m["same"]},
+        "gpu_launches": m["launches"], "clocks": m["clocks"], "alu_probe_Tlaneops": probe,
+        "set_dm_list_ms": m["set_dm_ms"], "wall_s_timed_region": m["wall"],
+        "step_ms_min_med_max": [min(m["step_ms"]), statistics.median(m["step_ms"]), max(m["step_ms"])],
+        "per_config": per_config,
         "paper_context": {"gpu_2011_dm_trial_samples_per_s": 7.5e7, "cpu_dm_trial_samples_per_s": 9.4e6,
                           "source": "PAPER.md:48, unnamed hardware; context, not target"},
     }
     print(json.dumps(res), flush=True)
     if world > 1:
+        import torch.distributed as dist
         dist.destroy_process_group()
 
 
@@ -733,6 +822,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="htru_gulp", choices=W.CONFIG_ORDER + W.EXTRA_CONFIGS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false",
+                    help="skip the per_config block (the other four BASELINE configs, timed in the default run)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "bitslice", "pairs"],
                     help="A/B: force the plain tiled kernel or its pair-row variant (dedisp_set_kernel)")
     ap.add_argument("--tscrunch", type=int, default=1,

@@ -37,7 +37,27 @@
  * library (released by dedisp_destroy).  in/out buffers and the stream belong to
  * the caller.  Host arrays passed in are copied before the call returns.
  *
- * Threading: a plan is not thread-safe; distinct plans are independent.
+ * Threading: a plan is not thread-safe; distinct plans are independent (two host
+ * threads may drive two plans concurrently; the library's only process-wide state, the
+ * launch counter and the per-kernel attribute flags, is atomic).
+ *
+ * Streams and scratch: the execute calls only enqueue work on the caller's stream.  A plan
+ * owns device scratch (bit planes, pair rows) that every execute of that plan re-uses:
+ * executes of ONE plan are therefore ordered -- a call on another stream than the plan's
+ * previous call first waits (cudaStreamWaitEvent) for the event the previous call recorded
+ * behind its kernels, so double-buffered callers stay correct but two executes of one plan
+ * never overlap; use one plan per concurrent stream for overlap.  The scratch is grown on
+ * demand inside execute with cudaFree + cudaMalloc (which synchronises the device);
+ * dedisp_reserve sizes it ahead of time so that the steady state never allocates.  While a
+ * stream is being captured into a CUDA graph the scratch cannot grow (execute returns
+ * DEDISP_ERR_CUDA, last error cudaErrorStreamCaptureUnsupported): call dedisp_reserve before
+ * capturing.  A captured graph holds the scratch pointers of its capture: it is invalidated
+ * when a later, larger execute / dedisp_reserve, or dedisp_set_dm_list, re-allocates them.
+ *
+ * Reads of `in`: only bytes of the caller's rows are read -- the unpack pre-pass uses aligned
+ * 128-bit loads for 16-byte blocks that lie inside [in, in + extent) and byte loads for the
+ * partial first / last block of the buffer, so nothing before `in` or past the last row's end
+ * is touched, whatever the alignment.
  *
  * Errors: every entry point returns a dedisp_status (or a value documented
  * below); nothing throws or aborts across the ABI.
@@ -135,6 +155,12 @@ dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams
 /* ceil(tscrunch * (nsamps_out + max_delay) * in_nbits / 8); 0 on error. */
 size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, long long nsamps_out,
                                                int in_nbits);
+
+/* Grow the plan's scratch to what dedisp_execute_batch(plan, nbeams, nsamps_out, .., in_nbits, ..)
+ * needs with the kernel selection in force (AUTO: pair rows where they pay, else bit planes), so that
+ * later executes of that size or smaller never allocate (see "Streams and scratch").  Synchronises
+ * the device if it has to re-allocate.  Errors: INVALID_ARG, NO_DM_LIST, UNSUPPORTED_NBITS, ALLOC. */
+dedisp_status dedisp_reserve(dedisp_plan plan, int nbeams, long long nsamps_out, int in_nbits);
 
 /* End-to-end convenience with HOST buffers (tight beam strides): copies the
  * packed input host->device, runs dedisp_execute_batch, copies the result back
@@ -330,6 +356,20 @@ dedisp_status dedisp_rfi_mask(const void *x_dev, dedisp_out_dtype x_dtype, int n
  * Only enqueues work on cuda_stream.  Errors: INVALID_ARG, UNSUPPORTED_NBITS, CUDA. */
 dedisp_status dedisp_transpose_time_major(const void *in_dev, int nchans, long long nsamps, int nbits,
                                           void *out_dev, void *cuda_stream);
+
+/* Diagnostics (the hazard evidence of profiles/r2_sanitizer.md; compute-sanitizer is not available on the GPU pool).
+ * dedisp_debug_set_poison: byte_value 0..255 makes every later execute of the plan first fill its scratch (bit planes,
+ * pair rows) with that byte, so a kernel that reads scratch words no pre-pass wrote changes its result with the
+ * byte; -1 (default) switches it off.
+ * dedisp_debug_checks_compiled: 1 when the library was built with -DDEDISP_CHECKS (in-kernel range and pipeline
+ * checks: shared-memory read ranges, the (work item, chunk) a ring stage holds when a consumer reads it, TMA source
+ * ranges, output row ranges), else 0.
+ * dedisp_debug_check_errors: copies the 8 failure counters of such a build to counts_out ([0] = total, [1] =
+ * shared-memory range, [2] = ring stage tag, [3] = TMA source, [4] = output range, [5] = pre-pass range); all zero
+ * in a normal build.  Synchronises the device. */
+int dedisp_debug_checks_compiled(void);
+dedisp_status dedisp_debug_set_poison(dedisp_plan plan, int byte_value);
+dedisp_status dedisp_debug_check_errors(dedisp_plan plan, unsigned long long *counts_out);
 
 /* Number of kernel launches this library has issued in this process (all plans). */
 unsigned long long dedisp_get_launch_count(void);

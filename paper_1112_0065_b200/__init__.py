@@ -41,6 +41,7 @@ ABI = {
     "dedisp_execute_tscrunch": (_i, [_vp, _i, _i, _ll, _vp, _sz, _i, _vp, _sz, _i, _vp]),
     "dedisp_get_in_row_stride_bytes_tscrunch": (_sz, [_vp, _i, _ll, _i]),
     "dedisp_execute_host": (_i, [_vp, _i, _ll, _vp, _i, _vp, _i]),
+    "dedisp_reserve": (_i, [_vp, _i, _ll, _i]),
     "dedisp_destroy": (_i, [_vp]),
     "dedisp_get_max_delay": (_i, [_vp]),
     "dedisp_get_nchans": (_i, [_vp]),
@@ -52,6 +53,9 @@ ABI = {
     "dedisp_set_timing": (_i, [_vp, _i]),
     "dedisp_get_last_kernel_ms": (_i, [_vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
     "dedisp_get_launch_count": (ctypes.c_ulonglong, []),
+    "dedisp_debug_checks_compiled": (_i, []),
+    "dedisp_debug_set_poison": (_i, [_vp, _i]),
+    "dedisp_debug_check_errors": (_i, [_vp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "dedisp_get_last_cuda_error": (_i, [_vp]),
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
     "dedisp_matched_filter": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, _vp, _vp]),
@@ -156,6 +160,10 @@ def dedisp_execute_host(plan: int, nbeams: int, nsamps_out: int, in_host, in_nbi
     _check(plan, st, "dedisp_execute_host")
 
 
+def dedisp_reserve(plan: int, nbeams: int, nsamps_out: int, in_nbits: int) -> None:
+    _check(plan, lib().dedisp_reserve(plan, nbeams, nsamps_out, in_nbits), "dedisp_reserve")
+
+
 def dedisp_destroy(plan: int) -> None:
     lib().dedisp_destroy(plan)
 
@@ -190,6 +198,20 @@ def dedisp_set_kernel(plan: int, which: int) -> None:
 
 def dedisp_get_last_kernel(plan: int) -> int:
     return lib().dedisp_get_last_kernel(plan)
+
+
+def dedisp_debug_checks_compiled() -> bool:
+    return bool(lib().dedisp_debug_checks_compiled())
+
+
+def dedisp_debug_set_poison(plan: int, byte_value: int) -> None:
+    _check(plan, lib().dedisp_debug_set_poison(plan, byte_value), "dedisp_debug_set_poison")
+
+
+def dedisp_debug_check_errors(plan: int) -> list:
+    buf = (ctypes.c_ulonglong * 8)()
+    _check(plan, lib().dedisp_debug_check_errors(plan, buf), "dedisp_debug_check_errors")
+    return list(buf)
 
 
 def dedisp_get_launch_count() -> int:

@@ -20,7 +20,9 @@ INCLUDE = PKG.parent / "include"
 LIB = PKG / "libdedisp_b200.so"
 OBJDIR = CSRC / "build"
 SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
-           "pair_rows.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
+           "bitslice_inst_cfg1.cu", "bitslice_inst_cfg2.cu", "bitslice_inst_cfg3.cu", "bitslice_inst_cfg4.cu",
+           "bitslice_inst_cfg5.cu", "bitslice_inst_cfg6.cu", "bitslice_inst_cfg8.cu", "bitslice_inst_pairs2.cu",
+           "bitslice_inst_pairs4.cu", "bitslice_inst_pairs8.cu", "pair_rows.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=false", "-Xptxas", "-v"]
 
@@ -36,10 +38,11 @@ def _headers() -> list[Path]:
     return sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.cuh")) + [INCLUDE / "dedisp.h"]
 
 
-def stale() -> bool:
-    if not LIB.exists():
+def stale(lib: Path | None = None) -> bool:
+    lib = lib or LIB
+    if not lib.exists():
         return True
-    t = LIB.stat().st_mtime
+    t = lib.stat().st_mtime
     return any(d.stat().st_mtime > t for d in [CSRC / s for s in SOURCES] + _headers())
 
 

@@ -231,4 +231,19 @@ struct BitsliceParams {
     // (vinfo & 0x0fffffff) .. + (vinfo >> 28) of it; rel carries the lane's variant in its byte offset
     const uint32_t *vinfo;     // [ngroups][nchans_pad]
     int vrows;                 // rows per beam
+    // self-checks (library built with -DDEDISP_CHECKS; see dedisp_debug_check_errors): failure counters in device
+    // memory and the extent of the scratch the producer may read
+    unsigned long long *check_errors;   // [DEDISP_NCHECK] or nullptr
+    unsigned long long scratch_words;   // words in `planes`
+    int ndm;
+};
+// what the self-checks count (index into check_errors)
+enum {
+    CHK_TOTAL = 0,          // all failures
+    CHK_LDS_RANGE = 1,      // a consumer's shared-memory reads would leave the stage's data area
+    CHK_STAGE_TAG = 2,      // a consumer found another (work item, chunk) in the stage than the one it waited for
+    CHK_TMA_SRC = 3,        // a bulk copy / tensor box would read outside the scratch (beyond the designed zero-fill margin)
+    CHK_OUT_RANGE = 4,      // the epilogue's output row or sample range is outside out
+    CHK_PREPASS = 5,        // a pre-pass thread would write outside its row
+    DEDISP_NCHECK = 8
 };

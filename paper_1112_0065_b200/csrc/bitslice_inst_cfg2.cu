@@ -1,0 +1,8 @@
+// bitslice_inst_cfg2.cu -- the tiled gather-sum kernel (bitslice_kernel.cuh) instantiated for geometry Cfg2.
+#include "bitslice_kernel.cuh"
+
+dedisp_status bitslice_run_cfg2(const BitsliceCall &c)
+{
+    return bsk::execute_cfg<Cfg2>(c.plan, *c.G, c.nbeams, c.nsamps_out, c.in, c.row_stride, c.in_beam_stride, c.in_nbits,
+                                 c.tscrunch, c.out, c.out_beam_stride, c.out_f32, c.s, c.range, c.reserve_only);
+}

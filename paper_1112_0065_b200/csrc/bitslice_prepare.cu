@@ -46,6 +46,22 @@ __global__ void bitslice_tables_kernel(const int32_t *__restrict__ delay, int nc
 }
 
 // ---- unpack pre-pass -------------------------------------------------------
+// The aligned 16-byte block at a0, restricted to the caller's buffer [vb, ve): one 128-bit load when the block lies
+// inside it, byte loads of the bytes inside it otherwise (only the partial first / last block of the whole buffer
+// takes that path), zero when it lies outside.  Nothing outside the caller's buffer is ever read.
+__device__ __forceinline__ uint4 load_block16(uintptr_t a0, const uint8_t *vb, const uint8_t *ve)
+{
+    if (a0 >= (uintptr_t)vb && a0 + 16 <= (uintptr_t)ve) return __ldg(reinterpret_cast<const uint4 *>(a0));
+    uint32_t w[4] = {0u, 0u, 0u, 0u};
+    if (a0 + 16 > (uintptr_t)vb && a0 < (uintptr_t)ve) {
+        for (int k = 0; k < 16; ++k) {
+            const uintptr_t a = a0 + k;
+            if (a >= (uintptr_t)vb && a < (uintptr_t)ve)
+                w[k >> 2] |= (uint32_t)__ldg(reinterpret_cast<const uint8_t *>(a)) << (8 * (k & 3));
+        }
+    }
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
 __device__ __forceinline__ uint32_t even_bits_to_low16(uint32_t x)
 {
     x &= 0x55555555u;
@@ -73,11 +89,8 @@ planes2_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row
         const uint8_t *a = in + (size_t)b * in_beam_stride + (size_t)c * row_stride + 16u * (size_t)i;
         const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)15;
         const int m = (int)((uintptr_t)a & 15);
-        uint4 lo = make_uint4(0, 0, 0, 0), hi = make_uint4(0, 0, 0, 0);
-        // a 16-byte block is loaded only if it overlaps the caller's buffer
-        if (a0 + 16 > (uintptr_t)valid_begin && a0 < (uintptr_t)valid_end)
-            lo = __ldg(reinterpret_cast<const uint4 *>(a0));
-        if (m && a0 + 16 < (uintptr_t)valid_end) hi = __ldg(reinterpret_cast<const uint4 *>(a0 + 16));
+        const uint4 lo = load_block16(a0, valid_begin, valid_end);
+        const uint4 hi = m ? load_block16(a0 + 16, valid_begin, valid_end) : make_uint4(0, 0, 0, 0);
         const uint32_t v[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
         const int q = m >> 2, sh = (m & 3) * 8;
 #pragma unroll
@@ -125,9 +138,7 @@ planes8_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, size_t row
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             uint4 q = make_uint4(0, 0, 0, 0);
-            const uintptr_t ak = a0 + 16u * k;
-            if ((k < 2 || m) && ak + 16 > (uintptr_t)valid_begin && ak < (uintptr_t)valid_end)
-                q = __ldg(reinterpret_cast<const uint4 *>(ak));
+            if (k < 2 || m) q = load_block16(a0 + 16u * k, valid_begin, valid_end);
             v[4 * k] = q.x; v[4 * k + 1] = q.y; v[4 * k + 2] = q.z; v[4 * k + 3] = q.w;
         }
         const int q4 = m >> 2, sh = (m & 3) * 8;
@@ -163,10 +174,8 @@ __device__ __forceinline__ void load16_aligned(const uint8_t *a, long long nvali
 {
     const uintptr_t a0 = (uintptr_t)a & ~(uintptr_t)15;
     const int m = (int)((uintptr_t)a & 15);
-    uint4 lo = make_uint4(0, 0, 0, 0), hi = make_uint4(0, 0, 0, 0);
-    if (a0 + 16 > (uintptr_t)valid_begin && a0 < (uintptr_t)valid_end)
-        lo = __ldg(reinterpret_cast<const uint4 *>(a0));
-    if (m && a0 + 16 < (uintptr_t)valid_end) hi = __ldg(reinterpret_cast<const uint4 *>(a0 + 16));
+    const uint4 lo = load_block16(a0, valid_begin, valid_end);
+    const uint4 hi = m ? load_block16(a0 + 16, valid_begin, valid_end) : make_uint4(0, 0, 0, 0);
     const uint32_t v[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
     const int q = m >> 2, sh = (m & 3) * 8;
 #pragma unroll
@@ -310,7 +319,15 @@ planes_tscrunch_kernel(const uint8_t *__restrict__ in, size_t in_beam_stride, si
             // an aligned word is loaded only if it overlaps the caller's buffer and the thread's bytes
             const bool need = (q < F || sh) && 4ll * q - (sh >> 3) < nvalid &&
                               aq + 4 > (uintptr_t)valid_begin && aq < (uintptr_t)valid_end;
-            v[q] = need ? __ldg(reinterpret_cast<const uint32_t *>(aq)) : 0u;
+            uint32_t word = 0u;
+            if (need && aq >= (uintptr_t)valid_begin && aq + 4 <= (uintptr_t)valid_end) {
+                word = __ldg(reinterpret_cast<const uint32_t *>(aq));
+            } else if (need) {      // partial first / last word of the caller's buffer: byte loads inside it only
+                for (int k = 0; k < 4; ++k)
+                    if (aq + k >= (uintptr_t)valid_begin && aq + k < (uintptr_t)valid_end)
+                        word |= (uint32_t)__ldg(reinterpret_cast<const uint8_t *>(aq + k)) << (8 * k);
+            }
+            v[q] = word;
         }
 #pragma unroll
         for (int q = 0; q < F; ++q) {

@@ -6,9 +6,10 @@
 #include <cstring>
 #include <new>
 
+#include "bitslice_common.cuh"
 #include "dedisp_internal.h"
 
-unsigned long long g_launch_count = 0;
+std::atomic<unsigned long long> g_launch_count{0};
 
 namespace {
 
@@ -41,6 +42,59 @@ void free_dm_state(dedisp_plan p)
 
 }  // namespace
 
+// ---- plan-owned scratch: growth and cross-stream ordering (dedisp_internal.h) ----
+dedisp_status scratch_reserve_bytes(dedisp_plan plan, void **ptr, size_t *have, size_t need, cudaStream_t s)
+{
+    if (*have >= need) return DEDISP_OK;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (s && cudaStreamIsCapturing(s, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) {
+        // cudaFree / cudaMalloc are not allowed inside a capture (and a graph captured earlier would keep the old
+        // pointer): the caller sizes the scratch with dedisp_reserve before capturing
+        plan->last_cuda_error = (int)cudaErrorStreamCaptureUnsupported;
+        return DEDISP_ERR_CUDA;
+    }
+    cudaFree(*ptr);      // synchronises the device: no kernel in flight still uses the old buffer
+    *ptr = nullptr;
+    *have = 0;
+    const cudaError_t e = cudaMalloc(ptr, need);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        plan->last_cuda_error = (int)e;
+        *ptr = nullptr;
+        return DEDISP_ERR_ALLOC;
+    }
+    *have = need;
+    return DEDISP_OK;
+}
+
+dedisp_status scratch_acquire(dedisp_plan plan, cudaStream_t s)
+{
+    if (!plan->scratch_ev_valid || plan->scratch_stream == s) return DEDISP_OK;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (s) DEDISP_CUDA_TRY(plan, cudaStreamIsCapturing(s, &cap));
+    // (a capturing stream cannot wait on an event recorded outside its capture: see scratch_release)
+    if (cap == cudaStreamCaptureStatusNone) DEDISP_CUDA_TRY(plan, cudaStreamWaitEvent(s, plan->scratch_ev, 0));
+    return DEDISP_OK;
+}
+
+dedisp_status scratch_release(dedisp_plan plan, cudaStream_t s)
+{
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (s) DEDISP_CUDA_TRY(plan, cudaStreamIsCapturing(s, &cap));
+    if (cap != cudaStreamCaptureStatusNone) {
+        // an event recorded inside a capture cannot be waited on from outside it: a plan whose executes are captured
+        // is ordered by the graph's own launch order (dedisp.h "Streams")
+        plan->scratch_ev_valid = false;
+        plan->scratch_stream = s;
+        return DEDISP_OK;
+    }
+    if (!plan->scratch_ev) DEDISP_CUDA_TRY(plan, cudaEventCreateWithFlags(&plan->scratch_ev, cudaEventDisableTiming));
+    DEDISP_CUDA_TRY(plan, cudaEventRecord(plan->scratch_ev, s));
+    plan->scratch_stream = s;
+    plan->scratch_ev_valid = true;
+    return DEDISP_OK;
+}
+
 extern "C" {
 
 dedisp_status dedisp_plan_create(dedisp_plan *plan, int nchans, double dt_s, double f_top_mhz,
@@ -68,6 +122,7 @@ dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int n
     for (int i = 0; i < ndm; ++i)
         if (!std::isfinite(dms_host[i]) || dms_host[i] < 0.0) return DEDISP_ERR_INVALID_ARG;
     DEDISP_CUDA_TRY(plan, cudaGetDevice(&plan->device));
+    DEDISP_CUDA_TRY(plan, cudaDeviceGetAttribute(&plan->sm_count, cudaDevAttrMultiProcessorCount, plan->device));
     free_dm_state(plan);
     plan->dms.assign(dms_host, dms_host + ndm);
 
@@ -104,6 +159,12 @@ dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int n
     }
     plan->ndm = ndm;
     plan->max_delay = flags[0];
+#ifdef DEDISP_CHECKS
+    if (!plan->d_check_errors) {
+        DEDISP_CUDA_TRY(plan, cudaMalloc(&plan->d_check_errors, sizeof(unsigned long long) * DEDISP_NCHECK));
+        DEDISP_CUDA_TRY(plan, cudaMemset(plan->d_check_errors, 0, sizeof(unsigned long long) * DEDISP_NCHECK));
+    }
+#endif
     dedisp_status st = bitslice_prepare(plan);
     if (st == DEDISP_OK) st = pair_prepare(plan);
     if (st != DEDISP_OK) free_dm_state(plan);
@@ -140,21 +201,16 @@ dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams
     int direct_nbits = in_nbits;
     size_t direct_beam_stride = in_beam_stride_bytes;
     size_t direct_row_stride = row_stride;
+    bool uses_scratch = false;
     if (tscrunch > 1) {
         // block sums as one byte each in the plan's scratch, then the DIRECT kernel on 8-bit samples
         const long long n_scr = nsamps_out + plan->max_delay;
         const size_t need = (size_t)nbeams * plan->nchans * (size_t)n_scr;
-        if (plan->planes_bytes < need) {
-            cudaFree(plan->d_planes);
-            plan->d_planes = nullptr;
-            plan->planes_bytes = 0;
-            if (cudaMalloc(&plan->d_planes, need) != cudaSuccess) {
-                cudaGetLastError();
-                return DEDISP_ERR_ALLOC;
-            }
-            plan->planes_bytes = need;
-        }
         if (nbeams > 65535 || plan->nchans > 65535) return DEDISP_ERR_INVALID_ARG;
+        st = scratch_reserve(plan, &plan->d_planes, &plan->planes_bytes, need, s);
+        if (st == DEDISP_OK) st = scratch_acquire(plan, s);
+        if (st != DEDISP_OK) return st;
+        uses_scratch = true;
         DEDISP_CUDA_TRY(plan, launch_tscrunch_bytes(in_nbits, tscrunch, in, in_beam_stride_bytes, row_stride,
                                                     plan->nchans, nbeams, n_scr, (uint8_t *)plan->d_planes, s));
         in = (const uint8_t *)plan->d_planes;
@@ -178,7 +234,7 @@ dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams
         plan->timing_has_prepass = false;
     }
     plan->last_kernel = DEDISP_KERNEL_DIRECT;
-    return DEDISP_OK;
+    return uses_scratch ? scratch_release(plan, s) : DEDISP_OK;
 }
 
 dedisp_status dedisp_execute_batch(dedisp_plan plan, int nbeams, long long nsamps_out,
@@ -198,6 +254,19 @@ dedisp_status dedisp_execute(dedisp_plan plan, long long nsamps_out, const void 
                                 cuda_stream);
 }
 
+dedisp_status dedisp_reserve(dedisp_plan plan, int nbeams, long long nsamps_out, int in_nbits)
+{
+    if (!plan || nbeams < 1 || nsamps_out < 1) return DEDISP_ERR_INVALID_ARG;
+    if (plan->ndm < 1 || !plan->d_delay) return DEDISP_ERR_NO_DM_LIST;
+    if (!nbits_ok(in_nbits)) return DEDISP_ERR_UNSUPPORTED_NBITS;
+    if (plan->want == DEDISP_KERNEL_DIRECT) return DEDISP_OK;       // the DIRECT kernel has no scratch
+    const size_t row_stride = dedisp_get_in_row_stride_bytes(plan, nsamps_out, in_nbits);
+    const dedisp_status st = bitslice_execute(plan, nbeams, nsamps_out, (const uint8_t *)nullptr, row_stride, 0, in_nbits,
+                                              1, nullptr, 0, 0, nullptr, nullptr, true);
+    // INVALID_ARG: the plan does not fit the tiled kernel; AUTO then runs DIRECT, which needs nothing
+    return (st == DEDISP_ERR_INVALID_ARG && plan->want == DEDISP_KERNEL_AUTO) ? DEDISP_OK : st;
+}
+
 dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps_out,
                                   const void *in_host, int in_nbits, void *out_host,
                                   dedisp_out_dtype out_dtype)
@@ -211,21 +280,10 @@ dedisp_status dedisp_execute_host(dedisp_plan plan, int nbeams, long long nsamps
     const size_t in_bytes = in_beam * nbeams, out_bytes = out_beam * nbeams;
     if (!plan->host_stream)
         DEDISP_CUDA_TRY(plan, cudaStreamCreateWithFlags(&plan->host_stream, cudaStreamNonBlocking));
-    if (plan->in_stage_bytes < in_bytes) {
-        cudaFree(plan->d_in_stage);
-        plan->d_in_stage = nullptr;
-        plan->in_stage_bytes = 0;
-        if (cudaMalloc(&plan->d_in_stage, in_bytes) != cudaSuccess) return DEDISP_ERR_ALLOC;
-        plan->in_stage_bytes = in_bytes;
-    }
-    if (plan->out_stage_bytes < out_bytes) {
-        cudaFree(plan->d_out_stage);
-        plan->d_out_stage = nullptr;
-        plan->out_stage_bytes = 0;
-        if (cudaMalloc(&plan->d_out_stage, out_bytes) != cudaSuccess) return DEDISP_ERR_ALLOC;
-        plan->out_stage_bytes = out_bytes;
-    }
     cudaStream_t s = plan->host_stream;
+    dedisp_status sst = scratch_reserve(plan, &plan->d_in_stage, &plan->in_stage_bytes, in_bytes, s);
+    if (sst == DEDISP_OK) sst = scratch_reserve(plan, &plan->d_out_stage, &plan->out_stage_bytes, out_bytes, s);
+    if (sst != DEDISP_OK) return sst;      // (the failed cudaMalloc is cleared and recorded in last_cuda_error)
     DEDISP_CUDA_TRY(plan, cudaMemcpyAsync(plan->d_in_stage, in_host, in_bytes, cudaMemcpyHostToDevice, s));
     // The result (out_bytes) dominates the transfer time, so it leaves in pieces while the kernel is
     // still running: one beam at a time, or -- single beam, trial DMs given in ascending order, so that
@@ -294,6 +352,7 @@ dedisp_status dedisp_destroy(dedisp_plan plan)
     if (!plan) return DEDISP_OK;
     free_dm_state(plan);
     cudaFree(plan->d_pair_rows);
+    cudaFree(plan->d_check_errors);
     cudaFree(plan->d_planes);
     cudaFree(plan->d_in_stage);
     cudaFree(plan->d_out_stage);
@@ -303,6 +362,7 @@ dedisp_status dedisp_destroy(dedisp_plan plan)
         if (e) cudaEventDestroy(e);
     for (int i = 0; i < 4; ++i)
         if (plan->ev[i]) cudaEventDestroy(plan->ev[i]);
+    if (plan->scratch_ev) cudaEventDestroy(plan->scratch_ev);
     delete plan;
     return DEDISP_OK;
 }
@@ -365,8 +425,34 @@ dedisp_status dedisp_get_last_kernel_ms(dedisp_plan plan, float *prepass_ms, flo
     return DEDISP_OK;
 }
 
+int dedisp_debug_checks_compiled(void)
+{
+#ifdef DEDISP_CHECKS
+    return 1;
+#else
+    return 0;
+#endif
+}
+
+dedisp_status dedisp_debug_set_poison(dedisp_plan plan, int byte_value)
+{
+    if (!plan || byte_value < -1 || byte_value > 255) return DEDISP_ERR_INVALID_ARG;
+    plan->poison = byte_value;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_debug_check_errors(dedisp_plan plan, unsigned long long *counts_out)
+{
+    if (!plan || !counts_out) return DEDISP_ERR_INVALID_ARG;
+    for (int i = 0; i < DEDISP_NCHECK; ++i) counts_out[i] = 0;
+    if (plan->d_check_errors)      // (synchronises with the kernels that may still be counting)
+        DEDISP_CUDA_TRY(plan, cudaMemcpy(counts_out, plan->d_check_errors, sizeof(unsigned long long) * DEDISP_NCHECK,
+                                         cudaMemcpyDeviceToHost));
+    return DEDISP_OK;
+}
+
 int dedisp_get_last_kernel(dedisp_plan plan) { return plan ? plan->last_kernel : 0; }
-unsigned long long dedisp_get_launch_count(void) { return g_launch_count; }
+unsigned long long dedisp_get_launch_count(void) { return g_launch_count.load(); }
 int dedisp_get_last_cuda_error(dedisp_plan plan) { return plan ? plan->last_cuda_error : 0; }
 
 const char *dedisp_get_error_string(dedisp_status s)

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <vector>
 
 #include "dedisp.h"
@@ -46,6 +47,15 @@ struct PairTables {
     bool usable = false;
 };
 
+// The encoded 2-D tensor map of the pair rows (cuTensorMapEncodeTiled), kept until the scratch moves or the shape changes.
+struct TensorMapCache {
+    alignas(64) unsigned char map[128] = {};
+    bool valid = false;
+    void *base = nullptr;
+    long long pitch = 0;
+    unsigned long long lines = 0;
+};
+
 struct dedisp_plan_s {
     int nchans = 0;
     double dt = 0, f_top = 0, df = 0;
@@ -68,6 +78,16 @@ struct dedisp_plan_s {
     PairTables pairs8;            // pair-row path, 8-bit samples (Cfg9P, DM groups of tab[1])
     uint32_t *d_pair_rows = nullptr;
     size_t pair_rows_bytes = 0;
+    TensorMapCache tmap[3];       // pair rows of 2-, 4- and 8-bit samples
+    // diagnostics (dedisp_debug_set_poison / dedisp_debug_check_errors)
+    int poison = -1;                               // >= 0: every execute first fills the scratch with this byte
+    unsigned long long *d_check_errors = nullptr;  // [DEDISP_NCHECK] failure counters of a -DDEDISP_CHECKS build
+    int sm_count = 0;             // multiprocessors of `device` (set_dm_list)
+    // ordering of the plan-owned scratch between executes on different streams: the stream and an event after the
+    // last kernels that touched it (scratch_acquire / scratch_release, dedisp_api.cu)
+    cudaStream_t scratch_stream = nullptr;
+    cudaEvent_t scratch_ev = nullptr;
+    bool scratch_ev_valid = false;
     // dedisp_execute_host staging
     void *d_in_stage = nullptr;
     size_t in_stage_bytes = 0;
@@ -84,7 +104,7 @@ struct dedisp_plan_s {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
-extern unsigned long long g_launch_count;
+extern std::atomic<unsigned long long> g_launch_count;
 
 #define DEDISP_CUDA_TRY(plan, expr)                         \
     do {                                                    \
@@ -130,7 +150,48 @@ struct BitsliceRange {
 dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_out,
                                const uint8_t *in, size_t row_stride, size_t in_beam_stride,
                                int nbits, int tscrunch, void *out, size_t out_beam_stride, int out_f32,
-                               cudaStream_t s, const BitsliceRange *range = nullptr);
+                               cudaStream_t s, const BitsliceRange *range = nullptr, bool reserve_only = false);
+
+// One call of the tiled kernel in a given geometry; the geometries are instantiated by one translation unit each
+// (bitslice_inst_*.cu) so that they compile in parallel.
+struct BitsliceCall {
+    dedisp_plan plan;
+    const BitsliceGeom *G;
+    int nbeams;
+    long long nsamps_out;
+    const uint8_t *in;
+    size_t row_stride, in_beam_stride;
+    int in_nbits, tscrunch;
+    void *out;
+    size_t out_beam_stride;
+    int out_f32;
+    cudaStream_t s;
+    BitsliceRange range;
+    bool reserve_only;        // grow the scratch for this call and return (dedisp_reserve)
+};
+dedisp_status bitslice_run_cfg1(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg2(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg3(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg4(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg5(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg6(const BitsliceCall &c);
+dedisp_status bitslice_run_cfg8(const BitsliceCall &c);
+dedisp_status bitslice_run_pairs2(const BitsliceCall &c);
+dedisp_status bitslice_run_pairs4(const BitsliceCall &c);
+dedisp_status bitslice_run_pairs8(const BitsliceCall &c);
+
+// Plan-owned scratch (dedisp_api.cu).  reserve: grow *ptr to `need` bytes (cudaFree + cudaMalloc: synchronises the
+// device, so nothing in flight still reads the old buffer; refused with DEDISP_ERR_CUDA while `s` is being captured
+// into a graph -- call dedisp_reserve before capturing).  acquire / release bracket the kernels of one execute:
+// an execute on another stream than the previous one first waits for the event the previous one recorded.
+dedisp_status scratch_reserve_bytes(dedisp_plan plan, void **ptr, size_t *have, size_t need, cudaStream_t s);
+template <class T>
+inline dedisp_status scratch_reserve(dedisp_plan plan, T **ptr, size_t *have, size_t need, cudaStream_t s)
+{
+    return scratch_reserve_bytes(plan, reinterpret_cast<void **>(ptr), have, need, s);
+}
+dedisp_status scratch_acquire(dedisp_plan plan, cudaStream_t s);
+dedisp_status scratch_release(dedisp_plan plan, cudaStream_t s);
 // pair_rows.cu
 dedisp_status pair_prepare(dedisp_plan plan);       // after bitslice_prepare; leaves pairs.usable
 void pair_release(dedisp_plan plan);

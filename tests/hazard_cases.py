@@ -1,17 +1,27 @@
-"""Small invocations of every hazard-prone kernel path, for compute-sanitizer (SURVEY.md Sec. 4 tier T3,
-Sec. 5 "race detection": "compute-sanitizer racecheck on the smem pipeline (mbarrier phases are the risk)").
+"""Small invocations of every hazard-prone kernel path (SURVEY.md Sec. 4 tier T3, Sec. 5 "race detection":
+"compute-sanitizer racecheck on the smem pipeline (mbarrier phases are the risk)").
 
-    compute-sanitizer --tool memcheck|racecheck|initcheck|synccheck python tests/sanitizer_cases.py [case ...]
+    python tests/hazard_cases.py [case ...]                       # parity + guard zones + scratch poisoning
+    DEDISP_B200_LIB=paper_1112_0065_b200/libdedisp_b200_checks.so python tests/hazard_cases.py   # + in-kernel checks
+    compute-sanitizer --tool memcheck|racecheck|initcheck|synccheck python tests/hazard_cases.py  # where the tool exists
 
-Each case runs the CUDA path through the C ABI on a shape chosen to reach one hazard and checks the result
-against the oracle (so a sanitizer run is also a parity run).  tests/test_gpu_sanitizer.py runs the four tools
-over all cases; profiles/r2_sanitizer.md keeps the summaries.  Cases:
+compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md), so the hazards it would look for are
+checked by the library's own instrumentation instead.  Each case runs the CUDA path through the C ABI on a shape
+chosen to reach one hazard and compares the result with the oracle, and in every case
+  * the input sits at a byte offset inside a buffer of random bytes (a read outside the caller's rows changes sums),
+  * the output sits between two canary zones that must come back untouched (out-of-bounds writes),
+  * the plan's scratch is pre-filled with 0x00, 0xFF and 0xA5 in turn (dedisp_debug_set_poison): a kernel that
+    consumes scratch words no pre-pass wrote (initcheck's job) cannot give the oracle's result for all three,
+  * with the -DDEDISP_CHECKS build the in-kernel counters must stay zero: shared-memory read ranges, the
+    (work item, chunk) tag of a ring stage before and after it is consumed (producer/consumer phase errors,
+    racecheck's job), TMA source ranges, output row ranges.
+tests/test_gpu_selfcheck.py runs both builds over all cases.  Cases:
   tiny_auto / tiny_direct   BASELINE configs[0] through the tiled kernel (plain planes, 1-D TMA) / the DIRECT kernel
   pairs3     cut-down HTRU shape at the top of the DM range: pair rows, 3 variants per slot, negative-x TMA boxes
   pairs8     8-bit wideband channelisation on 9-plane pair rows (Cfg9P)
   blocks     4100 channels of 2-bit samples: channel blocks, the epilogue reads `out` back (accumulate)
   unaligned  input base pointer at odd byte offsets: the guarded 128-bit straddling loads of the unpack pre-pass
-  multi      one plan, several persistent work items per CTA and a ragged last tile, float32 output
+  multi      several persistent work items per CTA (the ring wraps many times) and a ragged last tile
   search     dedisp_matched_filter_rms + dedisp_find_events_hinted (rows f1 + f2)
 """
 import sys
@@ -31,24 +41,40 @@ STEP = 1000.0 / 1199
 STEP8 = 2000.0 / 2047
 
 
+POISONS = (0x00, 0xFF, 0xA5)
+GUARD = 4096          # canary words on either side of the output
+CANARY = -1234567
+
+
 def _run(w, kernel, nbits, od="u32", offset=0, expect=None):
     delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
     x = W.generate(w, md)
     want = oracle.dedisperse(delay, x, nbits, w.nsamps_out)
+    f32 = od == "f32"
+    want = oracle.to_f32(want) if f32 else want
     p = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
     dd.dedisp_set_dm_list(p, list(w.dms()))
     dd.dedisp_set_kernel(p, kernel)
-    buf = torch.zeros(x.size + 32, dtype=torch.uint8, device="cuda")
+    # input: at `offset` inside random bytes
+    g = torch.Generator(device="cuda").manual_seed(7 + offset)
+    buf = torch.randint(0, 256, (x.size + 64,), dtype=torch.uint8, device="cuda", generator=g)
     buf[offset: offset + x.size] = torch.from_numpy(x.ravel()).cuda()
-    f32 = od == "f32"
-    out = torch.zeros((w.ndm, w.nsamps_out), dtype=torch.float32 if f32 else torch.int32, device="cuda")
-    dd.dedisp_execute(p, w.nsamps_out, buf.data_ptr() + offset, nbits, out,
-                      dd.DEDISP_OUT_F32 if f32 else dd.DEDISP_OUT_U32, torch.cuda.current_stream().cuda_stream)
-    torch.cuda.synchronize()
-    got = out.cpu().numpy()
-    assert np.array_equal(got if f32 else got.view(np.uint32), oracle.to_f32(want) if f32 else want)
+    n = w.ndm * w.nsamps_out
+    for poison in POISONS:
+        dd.dedisp_debug_set_poison(p, poison)
+        whole = torch.full((n + 2 * GUARD,), CANARY, dtype=torch.int32, device="cuda")
+        out = whole[GUARD: GUARD + n]
+        dd.dedisp_execute(p, w.nsamps_out, buf.data_ptr() + offset, nbits, out.data_ptr(),
+                          dd.DEDISP_OUT_F32 if f32 else dd.DEDISP_OUT_U32, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        h = whole.cpu().numpy()
+        assert (h[:GUARD] == CANARY).all() and (h[GUARD + n:] == CANARY).all(), "write outside out"
+        got = h[GUARD: GUARD + n].reshape(w.ndm, w.nsamps_out)
+        assert np.array_equal(got.view(np.float32) if f32 else got.view(np.uint32), want), f"poison {poison:#x}"
     if expect is not None:
         assert dd.dedisp_get_last_kernel(p) == expect, dd.dedisp_get_last_kernel(p)
+    errs = dd.dedisp_debug_check_errors(p)
+    assert errs[0] == 0, f"in-kernel checks failed: {errs}"
     dd.dedisp_destroy(p)
 
 
@@ -88,7 +114,8 @@ def multi():
     # persistent CTAs wrap the ring many times (producer/consumer phase parity across work items)
     w = HTRU.scaled(nchans=96, df=-4.0, ndm=300, dm_hi=60.0, nsamps_out=1920 * 4 + 77, kind="uniform2")
     _run(w, dd.DEDISP_KERNEL_BITSLICE, 2, od="f32")
-    _run(w, dd.DEDISP_KERNEL_PAIRS, 2, od="u32")
+    w = HTRU.scaled(nchans=96, df=-0.4, ndm=300, dm_hi=STEP * 299, nsamps_out=1920 * 4 + 77)
+    _run(w, dd.DEDISP_KERNEL_PAIRS, 2, od="u32", expect=dd.DEDISP_KERNEL_PAIRS)
 
 
 def search():
@@ -130,8 +157,9 @@ def main(argv):
     names = argv or list(CASES)
     for n in names:
         CASES[n]()
-        print(f"case {n}: ok (bit-exact vs oracle)", flush=True)
-    print(f"sanitizer_cases: {len(names)} cases ok; launches={dd.dedisp_get_launch_count()}", flush=True)
+        print(f"case {n}: ok (bit-exact vs oracle, guards intact, 3 scratch poisons, 0 check failures)", flush=True)
+    print(f"hazard_cases: {len(names)} cases ok; in-kernel checks compiled: {dd.dedisp_debug_checks_compiled()}; "
+          f"launches={dd.dedisp_get_launch_count()}", flush=True)
 
 
 if __name__ == "__main__":
