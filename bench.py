@@ -422,7 +422,8 @@ def run_matched_filter(args) -> None:
     widths = [1, 2, 4, 8, 16, 32, 64]
     radius = min(int(round(1.0 / w.dt)), (w.nsamps_out - 1) // 2)   # 2 s window (R21)
     x_max = w.nchans * ((1 << w.nbits) - 1)
-    z = torch.empty((len(widths), w.ndm, w.nsamps_out), dtype=torch.float32, device=dev)
+    z = None if (args.op == "search" and args.search_mode == "fused") else \
+        torch.empty((len(widths), w.ndm, w.nsamps_out), dtype=torch.float32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step():
@@ -578,29 +579,45 @@ def _bench_find_events(args, dd, torch, w, widths, z, make_z, flush, stream) -> 
 
 
 def _bench_search(args, dd, torch, w, widths, radius, x_max, x, z, flush, stream) -> None:
-    """--op search: rows f1 + f2 chained on the dedispersed output of --config.  A step =
-    dedisp_matched_filter_rms (z, the RMS of every filtered series and the block maxima of z in one pass
-    over x) + dedisp_find_events_hinted at 6 sigma (reads only the chunks of z whose block maxima exceed the
-    threshold).  Algorithmic bytes: x read once, z written once, the bit mask written and read."""
+    """--op search: rows f1 + f2 chained on the dedispersed output of --config, one call:
+    dedisp_search_events (RMS + block maxima of z in one pass over x without writing z, the blocks above the threshold
+    re-computed into a compact z, sigma-cut + grouping on that) at 6 sigma.  Algorithmic bytes: x read once.
+    --search-mode dense times the round-1 chain instead (dedisp_matched_filter_rms writing all of z +
+    dedisp_find_events_hinted).  The end-to-end leg starts from the PACKED filterbank in pinned host memory:
+    H2D (22 MB) -> dedisp_execute -> dedisp_search_events -> event list D2H."""
     dev = x.device
-    nw, nrows, n = z.shape
+    nw, nrows, n = len(widths), x.shape[0], x.shape[1]
     ns = nw * nrows
     nsigma, cap = 6.0, 1 << 20
-    wsb = dd.dedisp_find_events_workspace_bytes(ns, n)
-    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
-    mwb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, nw)
-    mws = torch.empty(mwb, dtype=torch.uint8, device=dev)
+    dense = args.search_mode == "dense"
     rms = torch.empty(ns, dtype=torch.float32, device=dev)
     ev = torch.empty((cap, 5), dtype=torch.int32, device=dev)
-    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
-    nblk, hblock, hoff = dd.dedisp_matched_filter_hint_blocks(n, widths)
-    hint = torch.empty((ns, nblk), dtype=torch.int32, device=dev)
+    cnt = torch.zeros(2, dtype=torch.int64, device=dev)
+    if dense:
+        wsb = dd.dedisp_find_events_workspace_bytes(ns, n)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        mwb = dd.dedisp_matched_filter_rms_workspace_bytes(nrows, n, nw)
+        mws = torch.empty(mwb, dtype=torch.uint8, device=dev)
+        nblk, hblock, hoff = dd.dedisp_matched_filter_hint_blocks(n, widths)
+        hint = torch.empty((ns, nblk), dtype=torch.int32, device=dev)
 
-    def step():
-        dd.dedisp_matched_filter_rms(x, dd.DEDISP_OUT_U32, nrows, n, radius, widths, x_max, z, rms, mws, mwb,
-                                     stream.cuda_stream, blockmax_ptr=hint)
-        dd.dedisp_find_events_hinted(z, ns, n, rms, nsigma, hint, hblock, hoff, ws, wsb, ev, cap, cnt,
-                                     stream.cuda_stream)
+        def step():
+            dd.dedisp_matched_filter_rms(x, dd.DEDISP_OUT_U32, nrows, n, radius, widths, x_max, z, rms, mws, mwb,
+                                         stream.cuda_stream, blockmax_ptr=hint)
+            dd.dedisp_find_events_hinted(z, ns, n, rms, nsigma, hint, hblock, hoff, ws, wsb, ev, cap, cnt,
+                                         stream.cuda_stream)
+        alg_bytes = x.numel() * 4 + z.numel() * 4 + 2 * (z.numel() // 8)
+        what, kern = "matched_filter_rms + find_events_hinted (dense z)", "matched_filter_kernel + sigma_cut_kernel (+ 4 small kernels)"
+    else:
+        max_blocks = 1 << 14      # 128 MiB of compact z: 6 sigma on noise flags a few dozen blocks
+        wsb = dd.dedisp_search_events_workspace_bytes(nrows, n, widths, max_blocks)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+
+        def step():
+            dd.dedisp_search_events(x, dd.DEDISP_OUT_U32, nrows, n, radius, widths, x_max, nsigma, rms, max_blocks,
+                                    ws, wsb, ev, cap, cnt, stream.cuda_stream)
+        alg_bytes = x.numel() * 4
+        what, kern = "search_events (no z written)", "matched_filter_kernel<RMS, no z> (+ sparse re-computation, 6 small kernels)"
 
     sampler = ClockSampler(0)
     sampler.start()
@@ -610,19 +627,37 @@ def _bench_search(args, dd, torch, w, widths, radius, x_max, x, z, flush, stream
     launches = (dd.dedisp_get_launch_count() - launches0) * args.steps // (args.steps + args.warmup)
     clocks = sampler.stop()
     ms = statistics.mean(step_ms)
-    found = int(cnt.item())
-    hx = x.cpu().pin_memory()
+    found, flagged = int(cnt[0].item()), int(cnt[1].item())
+    # end to end from the packed filterbank in pinned host memory to the event list in host memory
+    plan = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+    dd.dedisp_set_dm_list(plan, list(w.dms()))
+    md = dd.dedisp_get_max_delay(plan)
+    host_in = torch.from_numpy(W.generate(w, md)).pin_memory()
+    xin = torch.empty_like(host_in, device=dev)
     hev = torch.empty((cap, 5), dtype=torch.int32).pin_memory()
+    hcnt = torch.zeros(2, dtype=torch.int64).pin_memory()
+    dd.dedisp_reserve(plan, 1, n, w.nbits)
+
+    def e2e():
+        xin.copy_(host_in, non_blocking=True)
+        dd.dedisp_execute(plan, n, xin, w.nbits, x, dd.DEDISP_OUT_U32, stream.cuda_stream)
+        step()
+        hcnt.copy_(cnt, non_blocking=True)
+        stream.synchronize()
+        k = min(int(hcnt[0].item()), cap)
+        hev[:k].copy_(ev[:k], non_blocking=True)
+        stream.synchronize()
+        return k
+
+    e2e()
+    e2e_steps = 3
     t0 = time.perf_counter()
-    x.copy_(hx, non_blocking=True)
-    step()
-    k = min(int(cnt.item()), cap)
-    hev[:k].copy_(ev[:k], non_blocking=True)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
+    for _ in range(e2e_steps):
+        k = e2e()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    dd.dedisp_destroy(plan)
     peaks = measured_peaks()
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    alg_bytes = x.numel() * 4 + z.numel() * 4 + 2 * (z.numel() // 8)
     cpu = None
     if not args.no_cpu_baseline:
         from oracle import matched_filter as MF, peak_finding as PF
@@ -634,20 +669,23 @@ def _bench_search(args, dd, torch, w, widths, radius, x_max, x, z, flush, stream
         cpu = {"value": zz.size / dt, "unit": "searched samples/s", "cores": 1, "kind": "oracle",
                "sample": f"{rows.shape[0]} of {nrows} rows x {n} samples x {nw} widths "
                          f"(matched filter + rms + find_events), {dt:.2f} s"}
+    traffic, tsrc, tcommit = ncu_traffic(("search_dense_" if dense else "search_") + w.name)
     res = {"metric": "filtered and searched samples/sec", "value": ns * n / (ms * 1e-3), "unit": "searched samples/s",
            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "exact int -> f32",
            "data": "synthetic",
-           "config": {"workload": f"matched_filter_rms + find_events_hinted on dedispersed {w.name}", "nrows": nrows,
+           "config": {"workload": f"{what} on dedispersed {w.name}", "nrows": nrows,
                       "nsamps": n, "widths": widths, "radius": radius, "nsigma": nsigma, "events_found": found,
-                      "l2": "256 MiB flush buffer zeroed between timed iterations"},
+                      "blocks_recomputed": flagged, "l2": "256 MiB flush buffer zeroed between timed iterations"},
            "roofline": {"bound": "hbm", "achieved": alg_bytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                        "frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": ncu_traffic_bytes("search_" + w.name),
-                        "kernel": "matched_filter_kernel + sigma_cut_kernel (+ 4 small kernels)", "kernel_ms": ms,
+                        "frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": traffic, "traffic_source": tsrc,
+                        "traffic_capture_commit": tcommit, "algorithmic_bytes": alg_bytes,
+                        "kernel": kern, "kernel_ms": ms,
                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
            "cpu_baseline": cpu,
-           "e2e": {"value": ns * n / e2e_s, "unit": "searched samples/s", "h2d_bytes_per_step": x.numel() * 4,
-                   "d2h_bytes_per_step": k * 20 + 8, "steps": 1},
+           "e2e": {"value": ns * n / e2e_s, "unit": "searched samples/s", "h2d_bytes_per_step": host_in.numel(),
+                   "d2h_bytes_per_step": k * 20 + 16, "steps": e2e_steps, "ms_per_step": e2e_s * 1e3,
+                   "path": "packed host input -> H2D -> dedisp_execute -> search -> event list D2H"},
            "gpu_launches": launches, "clocks": clocks,
            "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)]}
     print(json.dumps(res), flush=True)
@@ -826,6 +864,8 @@ def main():
                     help="skip the per_config block (the other four BASELINE configs, timed in the default run)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "bitslice", "pairs"],
                     help="A/B: force the plain tiled kernel or its pair-row variant (dedisp_set_kernel)")
+    ap.add_argument("--search-mode", default="fused", choices=["fused", "dense"],
+                    help="--op search: dedisp_search_events (no z written; default) or the dense two-call chain")
     ap.add_argument("--tscrunch", type=int, default=1,
                     help="--op dedisperse only: sum blocks of K input samples and dedisperse on the grid K*dt "
                          "(row f4; the input then holds K x as many samples per output sample)")

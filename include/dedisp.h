@@ -252,6 +252,8 @@ dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dtype x_dtype,
  *                  one 2048-sample step of the kernel, gathered with warp maxima and atomicMax.
  *   workspace_dev  DEVICE scratch, 8-byte aligned, >= dedisp_matched_filter_rms_workspace_bytes();
  *                  owned by the caller, free to reuse once the call's work has completed.
+ *   z_dev          may be NULL here: rms_dev (and blockmax_dev) are computed and z is not written at all
+ *                  (what dedisp_search_events does in its first pass).
  * Other arguments, layouts and errors as dedisp_matched_filter; a null rms_dev, a null, misaligned
  * or too small workspace: INVALID_ARG.  Only enqueues work on cuda_stream (2 kernels, 1 memset). */
 size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths);
@@ -315,6 +317,32 @@ dedisp_status dedisp_find_events_hinted(const float *z_dev, long long nseries, l
                                         int hint_block, int hint_offset, void *workspace_dev,
                                         size_t workspace_bytes, dedisp_event *events_dev,
                                         long long max_events, long long *count_dev, void *cuda_stream);
+
+/* Rows f1 + f2 chained WITHOUT materialising z ("fusing the S/N search would remove that
+ * write"; Sec. 2.3): baseline removal + boxcar filters + RMS + sigma-cut + event grouping from the
+ * dedispersed series x straight to the event list.  Same definitions as dedisp_matched_filter_rms followed by
+ * dedisp_find_events_hinted at threshold nsigma * rms, and the same result: the event list is identical, field by
+ * field.  How: pass 1 runs the filter kernel for the RMS of every filtered series and the maxima of z over blocks of
+ * 2048 outputs and stores no z; the blocks whose maximum exceeds the series' threshold (a handful at 6 sigma on
+ * noise) are then re-computed by the same kernel into a compact z of max_blocks blocks (exact integer numerators, so
+ * every value is bit-identical to what the dense pass writes); the sigma-cut and the grouping run on that.
+ *   x_dev .. x_max   as for dedisp_matched_filter;  series index = width index * nrows + row
+ *   rms_dev          float32 [nwidths * nrows] out: sqrt(mean z^2) of every filtered series
+ *   max_blocks       capacity of the compact z (blocks of 2048 outputs, 8 KiB each)
+ *   workspace_dev    dedisp_search_events_workspace_bytes(...) bytes, 256-byte aligned, caller-owned
+ *   events_dev, max_events   as for dedisp_find_events
+ *   count_dev        int64 [2] out: [0] = events found (all of them, also beyond max_events), [1] = blocks that
+ *                    exceeded the threshold; the event list is complete iff count[1] <= max_blocks (else call again
+ *                    with a larger max_blocks: events of the blocks that did not fit are missing)
+ * Algorithmic bytes: x read once (+ 130 KB per flagged block); nothing of the size of z is written or read.
+ * Only enqueues work on cuda_stream.  Errors: INVALID_ARG, UNSUPPORTED_DTYPE, OVERFLOW, CUDA. */
+size_t dedisp_search_events_workspace_bytes(long long nrows, long long nsamps, const int *widths_host, int nwidths,
+                                            long long max_blocks);
+dedisp_status dedisp_search_events(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps,
+                                   int radius, const int *widths_host, int nwidths, unsigned int x_max, float nsigma,
+                                   float *rms_dev, long long max_blocks, void *workspace_dev, size_t workspace_bytes,
+                                   dedisp_event *events_dev, long long max_events, long long *count_dev,
+                                   void *cuda_stream);
 
 /* rms_dev[s] = float32( sqrt( (1/nsamps) * sum_t z[s][t]^2 ) ), accumulated in float64: the
  * noise estimate of a baseline-removed (zero-mean) series, offered as sigma for the

@@ -65,6 +65,9 @@ ABI = {
     "dedisp_matched_filter_hint_blocks": (_ll, [_ll, ctypes.POINTER(_i), _i, ctypes.POINTER(_i), ctypes.POINTER(_i)]),
     "dedisp_find_events_hinted": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _i, _i, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_find_events_workspace_bytes": (_sz, [_ll, _ll]),
+    "dedisp_search_events_workspace_bytes": (_sz, [_ll, _ll, ctypes.POINTER(_i), _i, _ll]),
+    "dedisp_search_events": (_i, [_vp, _i, _ll, _ll, _i, ctypes.POINTER(_i), _i, ctypes.c_uint, ctypes.c_float, _vp, _ll,
+                                  _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_find_events": (_i, [_vp, _ll, _ll, _vp, ctypes.c_float, _vp, _sz, _vp, _ll, _vp, _vp]),
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
     "dedisp_transpose_time_major": (_i, [_vp, _i, _ll, _i, _vp, _vp]),
@@ -243,7 +246,7 @@ def dedisp_matched_filter(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: 
     """Baseline removal + boxcar matched filters (include/dedisp.h)."""
     w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
     st = lib().dedisp_matched_filter(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths),
-                                     x_max, _ptr(z_ptr), stream or None)
+                                     x_max, _ptr(z_ptr) if z_ptr is not None else None, stream or None)
     _check(None, st, "dedisp_matched_filter")
 
 
@@ -258,11 +261,29 @@ def dedisp_matched_filter_rms(x_ptr, x_dtype: int, nrows: int, nsamps: int, radi
     dedisp_find_events_hinted uses) in the same pass (include/dedisp.h)."""
     w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
     st = lib().dedisp_matched_filter_rms(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths), x_max,
-                                         _ptr(z_ptr), _ptr(rms_ptr) if rms_ptr is not None else None,
+                                         _ptr(z_ptr) if z_ptr is not None else None,
+                                         _ptr(rms_ptr) if rms_ptr is not None else None,
                                          _ptr(blockmax_ptr) if blockmax_ptr is not None else None,
                                          _ptr(workspace_ptr) if workspace_ptr is not None else None,
                                          workspace_bytes, stream or None)
     _check(None, st, "dedisp_matched_filter_rms")
+
+
+def dedisp_search_events_workspace_bytes(nrows: int, nsamps: int, widths, max_blocks: int) -> int:
+    w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
+    return int(lib().dedisp_search_events_workspace_bytes(nrows, nsamps, w, len(widths), max_blocks))
+
+
+def dedisp_search_events(x_ptr, x_dtype: int, nrows: int, nsamps: int, radius: int, widths, x_max: int,
+                         nsigma: float, rms_ptr, max_blocks: int, workspace_ptr, workspace_bytes: int, events_ptr,
+                         max_events: int, count_ptr, stream: int = 0) -> None:
+    """Rows f1 + f2 chained without materialising z: x -> event list (include/dedisp.h)."""
+    w = (ctypes.c_int * len(widths))(*[int(v) for v in widths])
+    st = lib().dedisp_search_events(_ptr(x_ptr), x_dtype, nrows, nsamps, radius, w, len(widths), x_max, nsigma,
+                                    _ptr(rms_ptr), max_blocks, _ptr(workspace_ptr), workspace_bytes,
+                                    _ptr(events_ptr) if events_ptr is not None else None, max_events,
+                                    _ptr(count_ptr), stream or None)
+    _check(None, st, "dedisp_search_events")
 
 
 def dedisp_matched_filter_hint_blocks(nsamps: int, widths) -> tuple[int, int, int]:

@@ -86,11 +86,20 @@ struct Cfg {
     static constexpr int NB = NB_, NW = NW_, W = W_, K = K_, NSTAGE = NSTAGE_, NP = NP_, NV = NV_;
     static constexpr int NSPLIT = NSPLIT_, NBS = NB_ / NSPLIT_;
     // variant windows (NV > 1) are fetched as 2-D TMA boxes of NB plane lines x (WIN + VSKEW) words; the box of
-    // an odd variant starts VSKEW = 16 words early, so its window sits 16 banks away from an even variant's:
-    // two lanes at the same window offset in neighbouring variants do not collide (offsets differ by less than
-    // 16 words in all but the widest groups; the outer two of three variants belong to the low and the high
-    // lanes of a group, whose offsets differ)
+    // an odd variant starts VSKEW = 16 words early, so its window sits 16 banks away from an even variant's: two
+    // lanes of neighbouring variants collide on a bank only when their window offsets differ by exactly 16 words
+    // (the offsets of a group span <= 17 words for the HTRU list, <= 24 for the 8-bit wideband one).  The variant
+    // of a lane is NOT monotone in the lane -- delay[2p+1] - delay[2p] is a difference of two roundings and
+    // toggles between neighbouring values from trial to trial -- so lanes of different variants interleave and a
+    // small skew collides often: BS_VSKEW_UNIT=4 (variant v skewed by 4 v banks) measured 1.040 ms instead of
+    // 0.935 ms on the HTRU gulp and 39.0 instead of 34.1 ms on the wideband (profiles/r2_wide8.md).
+#ifdef BS_VSKEW_UNIT
+    static constexpr int VSKEW = BS_VSKEW_UNIT * (NV_ - 1);
+    static __host__ __device__ constexpr int vskew(int v) { return BS_VSKEW_UNIT * v; }
+#else
     static constexpr int VSKEW = NV_ > 1 ? 16 : 0;
+    static __host__ __device__ constexpr int vskew(int v) { return (v & 1) * VSKEW; }
+#endif
     template <int WIN> static constexpr int plane_words() { return WIN + VSKEW; }
     template <int WIN> static constexpr int vslot_words()
     {
@@ -194,7 +203,13 @@ using Cfg3P = Cfg<3, BS3P_NW, BS3P_W, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3
 #define BS5P_NSTAGE 2
 #endif
 using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, 1, 3>;
-using Cfg9P = Cfg<9, BS9P_NW, 4, BS9P_TREE_K, BS9P_NSTAGE, 20, BS8_WIN_S, BS8_WIN_S, BS9P_NSPLIT, 3>;
+#ifndef BS9P_W
+#define BS9P_W 4
+#endif
+#ifndef BS9P_WIN
+#define BS9P_WIN BS8_WIN_S
+#endif
+using Cfg9P = Cfg<9, BS9P_NW, BS9P_W, BS9P_TREE_K, BS9P_NSTAGE, 20, BS9P_WIN, BS9P_WIN, BS9P_NSPLIT, 3>;
 
 constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8
 constexpr int geom_index(int nplanes) { return nplanes; }

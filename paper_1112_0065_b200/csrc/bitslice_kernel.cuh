@@ -118,12 +118,28 @@ __device__ __forceinline__ void check_fail(unsigned long long *errs, int code)
 
 // Load the W+1 words of every plane of channel CI that this thread's W output words
 // need, and align them to the output time axis (one funnel shift per plane-word).
+// Geometries with many plane subsets (NSPLIT > 2) visit every channel slot once per subset: they keep the slot's
+// rel word and window address in registers for the whole chunk (SlotCache) instead of re-deriving them per subset.
+template <class C>
+struct SlotCache {
+    static constexpr bool ON = C::NSPLIT > 2;
+    uint32_t r[ON ? C::CH : 1];
+    const uint32_t *wp[ON ? C::CH : 1];
+};
+
 template <class C, int CI, int WIN, int P0>
-__device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *relp,
+__device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *relp, const SlotCache<C> &sc,
                                              uint32_t (&x)[C::NBS][C::W])
 {
-    const uint32_t r = relp[CI * LANES];
-    const uint32_t *wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (Stage<C, WIN>::CPITCH / 4) + P0 * Stage<C, WIN>::PLW;
+    uint32_t r;
+    const uint32_t *wp;
+    if constexpr (SlotCache<C>::ON) {
+        r = sc.r[CI];
+        wp = sc.wp[CI] + P0 * Stage<C, WIN>::PLW;
+    } else {
+        r = relp[CI * LANES];
+        wp = reinterpret_cast<const uint32_t *>(tb + (r >> 16)) + CI * (Stage<C, WIN>::CPITCH / 4) + P0 * Stage<C, WIN>::PLW;
+    }
 #pragma unroll
     for (int p = 0; p < C::NBS; ++p) {
         uint32_t w[C::W + 1];
@@ -139,11 +155,11 @@ __device__ __forceinline__ void load_aligned(const uint8_t *tb, const uint32_t *
 template <class C, int K, int C0, int WIN, int P0>
 struct Tree {
     static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&e)[C::NBS][C::W])
+                                               const uint32_t *relp, const SlotCache<C> &sc, uint32_t (&e)[C::NBS][C::W])
     {
         uint32_t e1[C::NBS][C::W], e2[C::NBS][C::W];
-        Tree<C, K - 1, C0, WIN, P0>::run(A, tb, relp, e1);
-        Tree<C, K - 1, C0 + (1 << K), WIN, P0>::run(A, tb, relp, e2);
+        Tree<C, K - 1, C0, WIN, P0>::run(A, tb, relp, sc, e1);
+        Tree<C, K - 1, C0 + (1 << K), WIN, P0>::run(A, tb, relp, sc, e2);
 #pragma unroll
         for (int i = 0; i < C::NBS; ++i)
 #pragma unroll
@@ -153,11 +169,11 @@ struct Tree {
 template <class C, int C0, int WIN, int P0>
 struct Tree<C, 0, C0, WIN, P0> {
     static __device__ __forceinline__ void run(uint32_t (&A)[C::NP][C::W], const uint8_t *tb,
-                                               const uint32_t *relp, uint32_t (&e)[C::NBS][C::W])
+                                               const uint32_t *relp, const SlotCache<C> &sc, uint32_t (&e)[C::NBS][C::W])
     {
         uint32_t x0[C::NBS][C::W], x1[C::NBS][C::W];
-        load_aligned<C, C0, WIN, P0>(tb, relp, x0);
-        load_aligned<C, C0 + 1, WIN, P0>(tb, relp, x1);
+        load_aligned<C, C0, WIN, P0>(tb, relp, sc, x0);
+        load_aligned<C, C0 + 1, WIN, P0>(tb, relp, sc, x1);
 #pragma unroll
         for (int i = 0; i < C::NBS; ++i)   // bit P0 + i of both channels
 #pragma unroll
@@ -172,11 +188,11 @@ struct Tree<C, 0, C0, WIN, P0> {
 // 81 instructions per chunk and word, profiles/r2_wide8.md); only the last subset ripples into the top planes.
 template <class C, int WIN, int S>
 __device__ __forceinline__ void add_chunk(uint32_t (&A)[C::NP][C::W], const uint8_t *tb, const uint32_t *relp,
-                                          uint32_t (&c)[C::W])
+                                          const SlotCache<C> &sc, uint32_t (&c)[C::W])
 {
     constexpr int P0 = S * C::NBS, B = P0 + C::K + 1, NBS = C::NBS, NP = C::NP, W = C::W;
     uint32_t e[NBS][W];
-    Tree<C, C::K, 0, WIN, P0>::run(A, tb, relp, e);
+    Tree<C, C::K, 0, WIN, P0>::run(A, tb, relp, sc, e);
 #pragma unroll
     for (int j = 0; j < W; ++j) {
         if constexpr (S == 0) {
@@ -189,7 +205,7 @@ __device__ __forceinline__ void add_chunk(uint32_t (&A)[C::NP][C::W], const uint
         for (int i = 1; i < NBS; ++i) c[j] = full_add(A[B + i][j], e[i][j], c[j]);
     }
     if constexpr (S + 1 < C::NSPLIT) {
-        add_chunk<C, WIN, S + 1>(A, tb, relp, c);
+        add_chunk<C, WIN, S + 1>(A, tb, relp, sc, c);
     } else {
 #pragma unroll
         for (int j = 0; j < W; ++j) {
@@ -370,9 +386,9 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                         const int cl = i / C::NV, v = i % C::NV;
                         const uint32_t info = P.vinfo[c0 + cl];
                         if (v <= (int)(info >> 28)) {
-                            const int x = P.ws[c0 + cl] + tile * C::TILE_WORDS - (v & 1) * C::VSKEW;
+                            const int x = P.ws[c0 + cl] + tile * C::TILE_WORDS - C::vskew(v);
                             const int y = (beam * P.vrows + (int)(info & 0x0fffffffu) + v) * NB;
-                            // (x < 0 only by the designed skew of odd variants: those words are zero-filled and never read)
+                            // (x < 0 only by the designed skew of the variants: those words are zero-filled and never read)
                             BS_CHECK(x >= -C::VSKEW && x + S::PLW <= P.row_pitch && y >= 0 &&
                                          (unsigned long long)(y + NB) * P.row_pitch <= P.scratch_words && (x & 3) == 0, CHK_TMA_SRC);
                             tma_box_g2s(sb + cl * S::CPITCH + v * S::VSLOT, &tmap, x, y, fb);
@@ -411,7 +427,15 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
             }
 #endif
             uint32_t carry[W];
-            add_chunk<C, WIN, 0>(A, tb, relp, carry);
+            SlotCache<C> sc;
+            if constexpr (SlotCache<C>::ON) {
+#pragma unroll
+                for (int ci = 0; ci < CH; ++ci) {
+                    sc.r[ci] = relp[ci * LANES];
+                    sc.wp[ci] = reinterpret_cast<const uint32_t *>(tb + (sc.r[ci] >> 16)) + ci * (S::CPITCH / 4);
+                }
+            }
+            add_chunk<C, WIN, 0>(A, tb, relp, sc, carry);
 #ifdef DEDISP_CHECKS
             BS_CHECK(tags[stage] == item * nchunks + chunk, CHK_STAGE_TAG);   // not overwritten while it was being read
 #endif
@@ -610,7 +634,7 @@ dedisp_status execute_pairs(dedisp_plan plan, const PairTables &T, int nbeams, l
         cudaEventRecord(plan->ev[2], s);
     }
     // the rows as a 2-D tensor [nbeams * nrows * NB lines][pitch words]; a box = the NB plane lines of one row x
-    // one window (words outside the tensor read as zero: odd variants start VSKEW words early)
+    // one window (words outside the tensor read as zero: variant v starts vskew(v) words early)
     // (encoded once and kept in the plan: re-encoded only when the scratch pointer, the pitch or the line count change)
     TensorMapCache &tc = plan->tmap[RAWNB == 2 ? 0 : RAWNB == 4 ? 1 : 2];
     const unsigned long long lines = (unsigned long long)nbeams * T.nrows * C::NB;

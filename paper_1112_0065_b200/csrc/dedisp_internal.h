@@ -199,3 +199,10 @@ cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t 
                              uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s);
 // DM groups of the plan's bit-sliced geometry for this sample width, or 0 if the kernel cannot serve it
 int bitslice_ngroups(dedisp_plan plan, int nbits);
+
+// matched_filter.cu: the dense pass (z and / or RMS + block maxima) or, with sparse_list, the re-computation of listed
+// blocks into a compact z (dedisp_search_events, peak_finding.cu)
+dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps, int radius,
+                     const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
+                     int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
+                     const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks);

@@ -53,7 +53,7 @@ __global__ void pair_range_kernel(const int32_t *__restrict__ delay, int nchans,
 __global__ void pair_tables_kernel(const int32_t *__restrict__ delay, int nchans, int ndm,
                                    const int32_t *__restrict__ sorted, int npairs_pad,
                                    const int32_t *__restrict__ dlo, const int32_t *__restrict__ row0, int nv,
-                                   int slot_bytes, int skew_bytes, int32_t *__restrict__ ws, uint32_t *__restrict__ rel,
+                                   int slot_bytes, int skew_unit_bytes, int skew_odd_bytes, int32_t *__restrict__ ws, uint32_t *__restrict__ rel,
                                    uint32_t *__restrict__ vinfo, int *flags)
 {
     const int g = blockIdx.x;
@@ -93,7 +93,7 @@ __global__ void pair_tables_kernel(const int32_t *__restrict__ delay, int nchans
             v = v > nv - 1 ? nv - 1 : v;
             const int off = (dv >> 5) - w0;
             worst = max(worst, off);
-            rel[row * 32 + l] = ((uint32_t)(off * 4 + v * slot_bytes + (v & 1) * skew_bytes) << 16) | (uint32_t)(dv & 31);
+            rel[row * 32 + l] = ((uint32_t)(off * 4 + v * slot_bytes + v * skew_unit_bytes + (v & 1) * skew_odd_bytes) << 16) | (uint32_t)(dv & 31);
         }
     }
     for (int o = 16; o > 0; o >>= 1) worst = max(worst, __shfl_xor_sync(0xffffffffu, worst, o));
@@ -242,7 +242,8 @@ static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G2, const
         if (e == cudaSuccess) e = cudaMemcpy(T.d_pair_cnt, cnt.data(), pbytes, cudaMemcpyHostToDevice);
         if (e == cudaSuccess) {
             pair_tables_kernel<<<ngroups, 256>>>(p->d_delay, p->nchans, ndm, B.d_order, npairs_pad, d_lo, d_row0,
-                                                 C::NV, C::template vslot_words<C::WIN_S>() * 4, C::VSKEW * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
+                                                 C::NV, C::template vslot_words<C::WIN_S>() * 4, (C::vskew(2) - 2 * C::vskew(1) == 0 ? C::vskew(1) : 0) * 4,
+                                                 (C::vskew(2) == 0 ? C::vskew(1) : 0) * 4, T.d_ws, T.d_rel, T.d_vinfo, d_flags);
             ++g_launch_count;
             e = cudaGetLastError();
         }

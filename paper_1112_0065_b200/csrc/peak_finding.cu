@@ -46,6 +46,32 @@ PFLayout make_layout(long long nseries, long long nsamps)
     return L;
 }
 
+// Where the kernels read z.  DenseZ: the full [nseries][n] array.  CompactZ (dedisp_search_events): only the blocks of
+// hblock outputs whose maximum exceeds the threshold exist, re-computed into zc[index][hblock]; map[s][b] is the index
+// of block b of series s (block b holds t with b*hblock - hoff <= t < (b+1)*hblock - hoff) or -1, and a sample of a
+// block that does not exist is at or below the threshold by construction: it reads as -infinity.
+struct DenseZ {
+    const float *z;
+    long long n;
+    static constexpr bool DENSE = true;
+    __device__ __forceinline__ float at(long long s, long long t) const { return __ldcs(z + s * n + t); }
+    __device__ __forceinline__ const float *row(long long s) const { return z + s * n; }
+};
+struct CompactZ {
+    const float *zc;
+    const int *map;
+    long long nblk;
+    int hblock, hoff;
+    static constexpr bool DENSE = false;
+    __device__ __forceinline__ float at(long long s, long long t) const
+    {
+        const long long u = t + hoff, b = u / hblock;
+        const int idx = __ldg(map + s * nblk + b);
+        return idx < 0 ? -INFINITY : __ldg(zc + (size_t)idx * hblock + (u - b * hblock));
+    }
+    __device__ __forceinline__ const float *row(long long) const { return nullptr; }
+};
+
 // run starts of a mask word: set bits whose predecessor (previous bit, or the top bit of the
 // previous word for bit 0) is clear
 __device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
@@ -54,14 +80,21 @@ __device__ __forceinline__ uint32_t run_starts(uint32_t m, uint32_t prev_word)
 }
 
 // ---- transform of one (series, chunk) by one warp ----
-__device__ __forceinline__ void cut_chunk(const float *__restrict__ z, long long n, long long nchunks, long long s,
+template <class ZA>
+__device__ __forceinline__ void cut_chunk(const ZA za, long long n, long long nchunks, long long s,
                                           long long c, float thr, uint32_t *__restrict__ mask,
                                           uint32_t *__restrict__ counts, int vec_ok, int lane)
 {
-    const float *zr = z + s * n;
+    const float *zr = za.row(s);
     const long long t0 = c * CHUNK;
     uint32_t mine = 0;
-    if (vec_ok && t0 + CHUNK <= n) {
+    if (!ZA::DENSE) {
+        for (int w = 0; w < CHUNK_WORDS; ++w) {
+            const long long t = t0 + w * 32 + lane;
+            const uint32_t b = __ballot_sync(0xffffffffu, t < n && za.at(s, t) > thr);
+            if (lane == w) mine = b;
+        }
+    } else if (vec_ok && t0 + CHUNK <= n) {
         // 128-bit loads: lane l of pass i holds samples 128 i + 4 l .. + 3 -> a nibble of word
         // 4 i + l/8; three OR-shuffles assemble the word in its 8-lane group, one more hands word
         // L to lane L
@@ -93,7 +126,7 @@ __device__ __forceinline__ void cut_chunk(const float *__restrict__ z, long long
     }
     // top bit of the word before: previous lane, or the sample before the chunk
     uint32_t prev = __shfl_up_sync(0xffffffffu, mine, 1);
-    if (lane == 0) prev = (t0 > 0 && __ldg(zr + t0 - 1) > thr) ? 0x80000000u : 0u;
+    if (lane == 0) prev = (t0 > 0 && za.at(s, t0 - 1) > thr) ? 0x80000000u : 0u;
     int cnt = __popc(run_starts(mine, prev));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
@@ -103,7 +136,7 @@ __device__ __forceinline__ void cut_chunk(const float *__restrict__ z, long long
 
 // one warp per (series, chunk)
 __global__ void __launch_bounds__(WARPS * 32)
-sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+sigma_cut_kernel(const DenseZ z, long long nseries, long long n, long long nchunks,
                  const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
                  uint32_t *__restrict__ counts, int vec_ok)
 {
@@ -118,8 +151,9 @@ sigma_cut_kernel(const float *__restrict__ z, long long nseries, long long n, lo
 // and transforms only those the hint does not rule out.  hint[s][b] bounds (order-preserving int image of
 // the float) every z[s][t] with b*hint_block - hint_offset <= t < (b+1)*hint_block - hint_offset from
 // above: a chunk all of whose blocks stay at or below the threshold holds no sample above it.
+template <class ZA>
 __global__ void __launch_bounds__(WARPS * 32)
-sigma_cut_hinted_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+sigma_cut_hinted_kernel(const ZA z, long long nseries, long long n, long long nchunks,
                         const float *__restrict__ sigma, float nsigma, uint32_t *__restrict__ mask,
                         uint32_t *__restrict__ counts, int vec_ok, const int *__restrict__ hint, int hint_block,
                         int hint_offset, long long hint_nblocks)
@@ -211,7 +245,8 @@ series_scan_kernel(const uint32_t *__restrict__ series_tot, long long nseries,
 
 // ---- reduce by key: a warp takes 32 (series, chunk) items at a time, skips those in which no
 // run starts (their count is 0) and handles the others one by one, lane = mask word ----
-__device__ __forceinline__ void group_chunk(const float *__restrict__ z, long long n, long long nchunks,
+template <class ZA>
+__device__ __forceinline__ void group_chunk(const ZA za, long long n, long long nchunks,
                                             const uint32_t *__restrict__ mask,
                                             const uint32_t *__restrict__ chunk_off,
                                             const unsigned long long *__restrict__ series_base,
@@ -234,7 +269,6 @@ __device__ __forceinline__ void group_chunk(const float *__restrict__ z, long lo
         if (lane >= o) inc += u;
     }
     unsigned long long slot = series_base[s] + chunk_off[s * nchunks + c] + (unsigned)(inc - cnt);
-    const float *zr = z + s * n;
     while (st) {
         const int b = __ffs(st) - 1;
         st &= st - 1;
@@ -255,10 +289,10 @@ __device__ __forceinline__ void group_chunk(const float *__restrict__ z, long lo
             }
         }
         if ((long long)slot < max_events) {
-            float peak = zr[t_start];
+            float peak = za.at(s, t_start);
             long long tp = t_start;
             for (long long t = t_start + 1; t < t_start + len; ++t) {
-                const float v = zr[t];
+                const float v = za.at(s, t);
                 if (v > peak) {
                     peak = v;
                     tp = t;
@@ -276,8 +310,9 @@ __device__ __forceinline__ void group_chunk(const float *__restrict__ z, long lo
     }
 }
 
+template <class ZA>
 __global__ void __launch_bounds__(WARPS * 32)
-group_events_kernel(const float *__restrict__ z, long long nseries, long long n, long long nchunks,
+group_events_kernel(const ZA z, long long nseries, long long n, long long nchunks,
                     const uint32_t *__restrict__ mask, const uint32_t *__restrict__ counts,
                     const uint32_t *__restrict__ chunk_off,
                     const unsigned long long *__restrict__ series_base,
@@ -345,6 +380,54 @@ size_t dedisp_find_events_workspace_bytes(long long nseries, long long nsamps)
     return make_layout(nseries, nsamps).total;
 }
 
+}  // extern "C"
+
+// The four kernels of the event search over the z the accessor ZA presents (dense array, or compact blocks).
+template <class ZA>
+static dedisp_status find_events_launch(const ZA za, bool vec_ok, long long nseries, long long nsamps,
+                                        const float *sigma_dev, float nsigma, const int *hint_dev, int hint_block,
+                                        int hint_offset, void *workspace_dev, size_t workspace_bytes,
+                                        dedisp_event *events_dev, long long max_events, long long *count_dev,
+                                        cudaStream_t s)
+{
+    const PFLayout L = make_layout(nseries, nsamps);
+    if (workspace_bytes < L.total) return DEDISP_ERR_INVALID_ARG;
+    uint8_t *ws = (uint8_t *)workspace_dev;
+    uint32_t *mask = (uint32_t *)ws;
+    uint32_t *counts = (uint32_t *)(ws + L.off_counts);
+    uint32_t *chunk_off = (uint32_t *)(ws + L.off_chunk_off);
+    uint32_t *series_tot = (uint32_t *)(ws + L.off_series_tot);
+    unsigned long long *series_base = (unsigned long long *)(ws + L.off_series_base);
+    const long long items = nseries * L.nchunks;
+    const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
+    if (hint_dev) {
+        // mask and counts (adjacent in the workspace) start at zero; only the chunks the hint cannot rule out
+        // are transformed
+        if (cudaMemsetAsync(mask, 0, L.off_chunk_off, s) != cudaSuccess) return DEDISP_ERR_CUDA;
+        const unsigned hgrid = (unsigned)((items + 32 * WARPS - 1) / (32 * WARPS));
+        sigma_cut_hinted_kernel<ZA><<<hgrid, WARPS * 32, 0, s>>>(za, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
+                                                                 mask, counts, vec_ok, hint_dev, hint_block, hint_offset,
+                                                                 (nsamps + hint_offset + hint_block - 1) / hint_block);
+    } else {
+        if constexpr (ZA::DENSE)
+            sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(za, nseries, nsamps, L.nchunks, sigma_dev, nsigma, mask, counts,
+                                                         vec_ok);
+        else
+            return DEDISP_ERR_INVALID_ARG;
+    }
+    chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
+                                                                    chunk_off, series_tot);
+    series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
+    int sms = 148, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long gwant = (items + WARPS * 32 - 1) / (WARPS * 32);
+    const unsigned ggrid = (unsigned)(gwant < 8ll * sms ? gwant : 8ll * sms);
+    group_events_kernel<ZA><<<ggrid, WARPS * 32, 0, s>>>(za, nseries, nsamps, L.nchunks, mask, counts,
+                                                         chunk_off, series_base, events_dev, max_events);
+    g_launch_count += 4;
+    return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
+}
+
 static dedisp_status find_events_run(const float *z_dev, long long nseries, long long nsamps,
                                      const float *sigma_dev, float nsigma, const int *hint_dev, int hint_block,
                                      int hint_offset, void *workspace_dev, size_t workspace_bytes,
@@ -358,41 +441,119 @@ static dedisp_status find_events_run(const float *z_dev, long long nseries, long
     if (((uintptr_t)z_dev & 3u) || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)events_dev & 3u) ||
         ((uintptr_t)count_dev & 7u))
         return DEDISP_ERR_INVALID_ARG;
-    const PFLayout L = make_layout(nseries, nsamps);
-    if (workspace_bytes < L.total) return DEDISP_ERR_INVALID_ARG;
-    uint8_t *ws = (uint8_t *)workspace_dev;
-    uint32_t *mask = (uint32_t *)ws;
-    uint32_t *counts = (uint32_t *)(ws + L.off_counts);
-    uint32_t *chunk_off = (uint32_t *)(ws + L.off_chunk_off);
-    uint32_t *series_tot = (uint32_t *)(ws + L.off_series_tot);
-    unsigned long long *series_base = (unsigned long long *)(ws + L.off_series_base);
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    const long long items = nseries * L.nchunks;
-    const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
-    const int vec_ok = (((uintptr_t)z_dev & 15u) == 0) && (nsamps % 4 == 0);
-    if (hint_dev) {
-        // mask and counts (adjacent in the workspace) start at zero; only the chunks the hint cannot rule out
-        // are transformed
-        if (cudaMemsetAsync(mask, 0, L.off_chunk_off, s) != cudaSuccess) return DEDISP_ERR_CUDA;
-        const unsigned hgrid = (unsigned)((items + 32 * WARPS - 1) / (32 * WARPS));
-        sigma_cut_hinted_kernel<<<hgrid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
-                                                             mask, counts, vec_ok, hint_dev, hint_block, hint_offset,
-                                                             (nsamps + hint_offset + hint_block - 1) / hint_block);
-    } else {
-        sigma_cut_kernel<<<grid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, sigma_dev, nsigma,
-                                                     mask, counts, vec_ok);
+    const bool vec_ok = (((uintptr_t)z_dev & 15u) == 0) && (nsamps % 4 == 0);
+    return find_events_launch(DenseZ{z_dev, nsamps}, vec_ok, nseries, nsamps, sigma_dev, nsigma, hint_dev, hint_block,
+                              hint_offset, workspace_dev, workspace_bytes, events_dev, max_events, count_dev,
+                              (cudaStream_t)cuda_stream);
+}
+
+// ---- dedisp_search_events: rows f1 + f2 without materialising z ----
+// One thread per (series, block): blocks whose maximum exceeds the series' threshold get a slot in the compact z
+// (first come first served: the slot order is irrelevant, the event list is ordered by the scans) and are listed for
+// the sparse re-computation; count[0] = number of such blocks (all of them, also beyond the capacity).
+__global__ void __launch_bounds__(256)
+flag_blocks_kernel(const int *__restrict__ blockmax, const float *__restrict__ sigma, float nsigma, long long nseries,
+                   long long nblk, int max_blocks, int *__restrict__ map, int2 *__restrict__ list, int *count)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nseries * nblk) return;
+    const long long s = i / nblk;
+    const float thr = __fmul_rn(nsigma, __ldg(sigma + s));
+    const int ti = __float_as_int(thr);
+    const bool look = !(thr == thr) || blockmax[i] > (ti >= 0 ? ti : ti ^ 0x7fffffff);
+    int slot = -1;
+    if (look) {
+        slot = atomicAdd(count, 1);
+        if (slot < max_blocks) list[slot] = make_int2((int)s, (int)(i - s * nblk));
+        else slot = -1;
     }
-    chunk_scan_kernel<<<(unsigned)((nseries + 7) / 8), 256, 0, s>>>(counts, nseries, L.nchunks,
-                                                                    chunk_off, series_tot);
-    series_scan_kernel<<<1, 1024, 0, s>>>(series_tot, nseries, series_base, count_dev);
-    int sms = 148, dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long gwant = (items + WARPS * 32 - 1) / (WARPS * 32);
-    const unsigned ggrid = (unsigned)(gwant < 8ll * sms ? gwant : 8ll * sms);
-    group_events_kernel<<<ggrid, WARPS * 32, 0, s>>>(z_dev, nseries, nsamps, L.nchunks, mask, counts,
-                                                     chunk_off, series_base, events_dev, max_events);
-    g_launch_count += 4;
-    return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ERR_CUDA;
+    map[i] = slot;
+}
+
+// count_out[1] = blocks flagged; count[0] (the sparse kernel's CTA count) = min(flagged, max_blocks)
+__global__ void clamp_block_count_kernel(int *count, int max_blocks, long long *count_out)
+{
+    count_out[1] = *count;
+    if (*count > max_blocks) *count = max_blocks;
+}
+
+struct SearchLayout {
+    size_t off_partial, off_blockmax, off_map, off_list, off_count, off_zc, off_pf, total;
+    long long nblk;
+    int hblock, hoff;
+};
+
+static bool search_layout(long long nrows, long long nsamps, const int *widths_host, int nwidths, long long max_blocks,
+                          SearchLayout &L)
+{
+    if (nrows < 1 || nsamps < 1 || nwidths < 1 || max_blocks < 1 || max_blocks > 0x7fffffffll) return false;
+    const long long nseries = nrows * nwidths;
+    if (!pf_sizes_ok(nseries, nsamps)) return false;
+    L.nblk = dedisp_matched_filter_hint_blocks(nsamps, widths_host, nwidths, &L.hblock, &L.hoff);
+    if (L.nblk < 1) return false;
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    size_t o = 0;
+    L.off_partial = o;  o = up(o + dedisp_matched_filter_rms_workspace_bytes(nrows, nsamps, nwidths));
+    L.off_blockmax = o; o = up(o + (size_t)nseries * L.nblk * 4);
+    L.off_map = o;      o = up(o + (size_t)nseries * L.nblk * 4);
+    L.off_list = o;     o = up(o + (size_t)max_blocks * 8);
+    L.off_count = o;    o = up(o + 8);
+    L.off_zc = o;       o = up(o + (size_t)max_blocks * L.hblock * 4);
+    L.off_pf = o;       o = up(o + dedisp_find_events_workspace_bytes(nseries, nsamps));
+    L.total = o;
+    return true;
+}
+
+extern "C" {
+
+size_t dedisp_search_events_workspace_bytes(long long nrows, long long nsamps, const int *widths_host, int nwidths,
+                                            long long max_blocks)
+{
+    SearchLayout L;
+    return (widths_host && search_layout(nrows, nsamps, widths_host, nwidths, max_blocks, L)) ? L.total : 0;
+}
+
+dedisp_status dedisp_search_events(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps,
+                                   int radius, const int *widths_host, int nwidths, unsigned int x_max, float nsigma,
+                                   float *rms_dev, long long max_blocks, void *workspace_dev, size_t workspace_bytes,
+                                   dedisp_event *events_dev, long long max_events, long long *count_dev,
+                                   void *cuda_stream)
+{
+    if (!x_dev || !widths_host || !rms_dev || !workspace_dev || !count_dev || max_events < 0 ||
+        (max_events > 0 && !events_dev))
+        return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)workspace_dev & 255u) || ((uintptr_t)events_dev & 3u) || ((uintptr_t)count_dev & 7u))
+        return DEDISP_ERR_INVALID_ARG;
+    SearchLayout L;
+    if (!search_layout(nrows, nsamps, widths_host, nwidths, max_blocks, L) || workspace_bytes < L.total)
+        return DEDISP_ERR_INVALID_ARG;
+    uint8_t *ws = (uint8_t *)workspace_dev;
+    int *blockmax = (int *)(ws + L.off_blockmax), *map = (int *)(ws + L.off_map), *count = (int *)(ws + L.off_count);
+    int2 *list = (int2 *)(ws + L.off_list);
+    float *zc = (float *)(ws + L.off_zc);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const long long nseries = nrows * nwidths;
+    // pass 1: the RMS of every filtered series and the block maxima of z; z itself is not written
+    dedisp_status st = mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, nullptr, rms_dev,
+                              blockmax, ws + L.off_partial, L.off_blockmax - L.off_partial, cuda_stream, nullptr, nullptr,
+                              nullptr, 0);
+    if (st != DEDISP_OK) return st;
+    // pass 2: the few blocks that can hold a sample above the threshold, re-computed (bit-identical: same kernel,
+    // same exact integer sums) into the compact z
+    if (cudaMemsetAsync(count, 0, 8, s) != cudaSuccess) return DEDISP_ERR_CUDA;
+    const long long nb = nseries * L.nblk;
+    flag_blocks_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, s>>>(blockmax, rms_dev, nsigma, nseries, L.nblk,
+                                                                    (int)max_blocks, map, list, count);
+    clamp_block_count_kernel<<<1, 1, 0, s>>>(count, (int)max_blocks, count_dev);
+    g_launch_count += 2;
+    if (cudaGetLastError() != cudaSuccess) return DEDISP_ERR_CUDA;
+    st = mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, nullptr, nullptr, nullptr, nullptr, 0,
+                cuda_stream, list, count, zc, max_blocks);
+    if (st != DEDISP_OK) return st;
+    // pass 3: sigma-cut and grouping over the compact z (chunks the block maxima rule out are skipped as before)
+    const CompactZ za{zc, map, L.nblk, L.hblock, L.hoff};
+    return find_events_launch(za, false, nseries, nsamps, rms_dev, nsigma, blockmax, L.hblock, L.hoff, ws + L.off_pf,
+                              L.total - L.off_pf, events_dev, max_events, count_dev, s);
 }
 
 dedisp_status dedisp_find_events(const float *z_dev, long long nseries, long long nsamps,
