@@ -2,8 +2,10 @@
 
     python -m paper_1112_0065_b200.build [--force] [--verbose]
 
-Every translation unit is compiled to an object file under csrc/build/ (in parallel, re-compiled
-only when it or a header changed) and the objects are linked into the shared library.
+Every translation unit is compiled to an object file (in parallel, re-compiled only when it or a
+header changed) and the objects are linked into the shared library.  The object cache lives in the
+system temp directory (DEDISP_B200_OBJDIR overrides it): it is a few hundred MB and must not travel
+with the source tree.
 """
 from __future__ import annotations
 
@@ -11,6 +13,7 @@ import hashlib
 import os
 import subprocess
 import sys
+import tempfile
 from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
@@ -18,11 +21,12 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libdedisp_b200.so"
-OBJDIR = CSRC / "build"
+OBJDIR = Path(os.environ.get("DEDISP_B200_OBJDIR") or
+              Path(tempfile.gettempdir()) / ("dedisp_b200_obj_" + hashlib.sha1(str(PKG).encode()).hexdigest()[:10]))
 SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
            "bitslice_inst_cfg1.cu", "bitslice_inst_cfg2.cu", "bitslice_inst_cfg3.cu", "bitslice_inst_cfg4.cu",
            "bitslice_inst_cfg5.cu", "bitslice_inst_cfg6.cu", "bitslice_inst_cfg8.cu", "bitslice_inst_pairs2.cu",
-           "bitslice_inst_pairs4.cu", "bitslice_inst_pairs8.cu", "pair_rows.cu", "matched_filter.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
+           "bitslice_inst_pairs4.cu", "bitslice_inst_pairs8.cu", "pair_rows.cu", "matched_filter.cu", "matched_filter_warp.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=false", "-Xptxas", "-v"]
 

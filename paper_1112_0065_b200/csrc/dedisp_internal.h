@@ -206,3 +206,9 @@ dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrow
                      const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
                      int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                      const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks);
+// matched_filter_warp.cu: the same passes by the warp-autonomous kernel (no dense z), and its segment length
+dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps, int radius,
+                          const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
+                          int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
+                          const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks);
+long long mf_warp_segment(long long nrows, long long nsamps);

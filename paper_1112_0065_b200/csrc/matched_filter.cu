@@ -58,11 +58,6 @@ struct MFParams {
     double *partial;             // RMS variant: [nw][nrows][nseg] sums of z^2 over a segment
     int *blockmax;               // RMS variant, optional: [nw][nrows][nblk] upper bounds of z per block of E outputs
     int nblk;
-    // sparse re-computation (dedisp_search_events): CTA i re-runs the steps that produce block sparse_list[i].y of
-    // series sparse_list[i].x (= width index * nrows + row) and stores that block's E outputs at zc + i*E
-    const int2 *sparse_list;     // nullptr: the dense pass
-    const int *sparse_count;     // number of valid entries (device)
-    float *zc;
 };
 
 // inclusive block scan of one value per thread; returns the thread's inclusive prefix and
@@ -163,35 +158,14 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
     if (RMS)
         for (int iw = 0; iw < P.nw; ++iw) sAcc[iw * NT + threadIdx.x] = 0.f;
 
+    const long long row = blockIdx.x / P.nseg;
+    const int seg = (int)(blockIdx.x % P.nseg);
     const long long n = P.n;
     const int R = P.radius;
     const long long N = 2ll * R + 1;
-    const bool sparse = !RMS && P.sparse_list != nullptr;
-    long long row = blockIdx.x / P.nseg, lo;
-    int seg = (int)(blockIdx.x % P.nseg), seglen, nrem;
-    int iw0 = 0, iw1 = P.nw, tb_out = -1;
-    if (sparse) {
-        // the block's outputs t = b*E - wmax + [0, E) come out of the step that starts at sample b*E; the prefix
-        // sums they read reach back wmax samples, i.e. H = ceil(wmax / E) earlier steps: start H steps before
-        // (the sums are exact integers whatever the start, so z is bit-identical to the dense pass)
-        if ((int)blockIdx.x >= *P.sparse_count) return;
-        const int2 it = P.sparse_list[blockIdx.x];
-        iw0 = (int)(it.x / P.nrows);
-        iw1 = iw0 + 1;
-        row = it.x % P.nrows;
-        const long long H = (P.wmax + E - 1) / E;
-        lo = ((long long)it.y - H) * E;
-        if (lo < 0) lo = 0;
-        tb_out = (int)((long long)it.y * E - lo);
-        nrem = (int)(n - lo);
-        const long long want = (long long)tb_out - P.wmax + E;
-        seglen = (int)(want < nrem ? want : nrem);
-        seg = 0;
-    } else {
-        lo = (long long)seg * P.seg;
-        seglen = (int)((lo + P.seg < n) ? P.seg : n - lo);
-        nrem = (int)(n - lo);                  // samples from lo to the end of the row
-    }
+    const long long lo = (long long)seg * P.seg;
+    const int seglen = (int)((lo + P.seg < n) ? P.seg : n - lo);
+    const int nrem = (int)(n - lo);                  // samples from lo to the end of the row
     const uint32_t *xr = reinterpret_cast<const uint32_t *>(P.x) + row * n + lo;   // sample lo of this row
     const int j = threadIdx.x;
 
@@ -232,11 +206,8 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
     const long long dlo_ll = (long long)R + 1 - lo;
     const int dlo = dlo_ll < -(1 << 30) ? -(1 << 30) : (int)dlo_ll;
     const int dhi = nrem - R - 1;
-    const size_t plane = sparse ? 0 : (size_t)P.nrows * (size_t)n;     // distance between the widths' outputs
-    // dense: z[iw][row][lo + o]; sparse: the compact block zc[blockIdx.x][o - (tb_out - wmax)]; none: RMS / maxima only
-    float *const zrow = sparse ? P.zc + (size_t)blockIdx.x * E - (tb_out - P.wmax)
-                               : (P.z ? P.z + (size_t)row * (size_t)n + (size_t)lo : nullptr);
-    const bool have_z = zrow != nullptr || sparse;
+    const size_t plane = (size_t)P.nrows * (size_t)n;
+    float *const zrow = P.z + (size_t)row * (size_t)n + (size_t)lo;
 
     for (int tb = 0; tb < seglen + P.wmax; tb += E) {
         // ---- the three input streams, coalesced (the two trailing ones hit L2) ----
@@ -307,7 +278,6 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
         if (GUARD) slowbits = (slowbits << 1) | (__syncthreads_or(bad) ? 1 : 0);
         else __syncthreads();
         // ---- outputs of the step that lags wmax behind: o = tb - wmax + j + k*NT ----
-        if (!sparse || tb == tb_out) {      // (a sparse re-computation wants the last step's outputs only)
         const int ob = tb - P.wmax + j;
         int rs[V];
         ACC p0[V];
@@ -320,14 +290,12 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
         }
         const bool interior = (tb - P.wmax >= 0) && (tb - P.wmax + E <= seglen) &&
                               (tb + E - 1 <= nrem);      // every output valid, every boxcar complete
-        const bool store = have_z && (!sparse || tb == tb_out);
-        float *zp = zrow + ob + (size_t)iw0 * plane;
-
+        float *zp = zrow + ob;
         // outputs of this step are t = lo + tb - wmax + [0, E): block (lo + tb) / E of the hint
         int *const bmax = (RMS && P.blockmax) ? P.blockmax + (size_t)row * P.nblk + (lo + tb) / E : nullptr;
         const size_t bstride = (size_t)P.nrows * (size_t)P.nblk;
         if (GUARD && (slowbits & P.guard_hist)) {
-            for (int iw = iw0; iw < iw1; ++iw, zp += plane) {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;
@@ -350,13 +318,13 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                     }
                     const float z = (float)zz * scl;
                     if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
-                    if (store) __stcs(zp + k * NT, z);
+                    __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
                 if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
         } else if (interior) {
-            for (int iw = iw0; iw < iw1; ++iw, zp += plane) {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 float ss = 0.f, mx = -INFINITY;
@@ -366,13 +334,13 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                     if (!MIRROR && sl >= RING) sl -= RING;
                     const float z = acc_to_float((ACC)(ring[sl] - p0[k])) * scl;
                     if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
-                    if (store) __stcs(zp + k * NT, z);
+                    __stcs(zp + k * NT, z);
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
                 if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
         } else {
-            for (int iw = iw0; iw < iw1; ++iw, zp += plane) {
+            for (int iw = 0; iw < P.nw; ++iw, zp += plane) {
                 const int w = P.w[iw];
                 const float scl = P.scale[iw];
                 const int lim = nrem - w;                 // t + w <= n  <=>  o <= lim
@@ -385,13 +353,12 @@ __global__ void __launch_bounds__(NT, RMS ? MF_MINB_RMS : MF_MINB) matched_filte
                         if (!MIRROR && sl >= RING) sl -= RING;
                         const float z = (o <= lim) ? acc_to_float((ACC)(ring[sl] - p0[k])) * scl : 0.f;
                         if (RMS) { ss = __fmaf_rn(z, z, ss); mx = fmaxf(mx, z); }
-                        if (store) __stcs(zp + k * NT, z);   // streaming store: keep x, not z, in L2
+                        __stcs(zp + k * NT, z);           // streaming store: keep x, not z, in L2
                     }
                 }
                 if (RMS) sAcc[iw * NT + j] += ss;
                 if (RMS && bmax) push_block_max(bmax + (size_t)iw * bstride, mx);
             }
-        }
         }
         wslot += E;
         if (wslot >= RING) wslot -= RING;
@@ -441,22 +408,24 @@ long long mf_segment(long long nsamps)
 }
 }  // namespace
 
-// sparse_list / sparse_count / zc / max_blocks: the sparse re-computation of dedisp_search_events (one CTA per listed
-// block, z_dev and rms_dev null); otherwise the dense pass (z_dev may be null when rms_dev is given: RMS and block
-// maxima only).
+// The dense pass (z written; with rms_dev also the RMS and, optionally, the block maxima) runs the CTA-cooperative
+// kernel of this file.  Passes that store no dense z -- z_dev null with rms_dev given (RMS + block maxima only), and
+// the sparse re-computation of listed blocks into a compact z (sparse_list / sparse_count / zc / max_blocks:
+// dedisp_search_events) -- run the warp-autonomous kernel of matched_filter_warp.cu.  z is bit-identical between
+// the two kernels (exact integer numerators); their RMS agrees to the documented 2^-20 (different summation order).
 dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows, long long nsamps, int radius,
                      const int *widths_host, int nwidths, unsigned int x_max, float *z_dev, float *rms_dev,
                      int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                      const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks)
 {
-    const bool sparse = sparse_list != nullptr;
-    if (!x_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0) return DEDISP_ERR_INVALID_ARG;
-    if (sparse ? (!sparse_count || !zc || max_blocks < 1 || max_blocks > 0x7fffffffll || z_dev || rms_dev)
-               : (!z_dev && !rms_dev))
+    if (sparse_list || !z_dev)
+        return mf_warp_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, rms_dev, blockmax_dev,
+                           workspace_dev, workspace_bytes, cuda_stream, sparse_list, sparse_count, zc, max_blocks);
+    if (!x_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0)
         return DEDISP_ERR_INVALID_ARG;
     if (x_dtype != DEDISP_OUT_U32 && x_dtype != DEDISP_OUT_F32) return DEDISP_ERR_UNSUPPORTED_DTYPE;
     if (nwidths < 1 || nwidths > MAXW || nsamps > (1ll << 30)) return DEDISP_ERR_INVALID_ARG;
-    if (((uintptr_t)x_dev & 3u) || ((uintptr_t)z_dev & 3u) || ((uintptr_t)zc & 3u)) return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)x_dev & 3u) || ((uintptr_t)z_dev & 3u)) return DEDISP_ERR_INVALID_ARG;
     const long long N = 2ll * radius + 1;
     if (N > nsamps) return DEDISP_ERR_INVALID_ARG;
     if (x_max == 0) x_max = (1u << 24) - 1;
@@ -499,9 +468,6 @@ dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrow
     P.partial = (double *)workspace_dev;
     P.blockmax = blockmax_dev;
     P.nblk = (int)((nsamps + P.wmax + E - 1) / E);
-    P.sparse_list = sparse_list;
-    P.sparse_count = sparse_count;
-    P.zc = zc;
     if (blockmax_dev && (!rms || ((uintptr_t)blockmax_dev & 3u))) return DEDISP_ERR_INVALID_ARG;
     if (rms) {
         if (!workspace_dev || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)rms_dev & 3u) ||
@@ -511,7 +477,7 @@ dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrow
     const size_t smem = 2 * (size_t)E * 4 + (NT / 32) * accb + (wide ? 1 : 2) * (size_t)ring * accb +
                         (rms ? (size_t)nwidths * NT * 4 : 0);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const dim3 grid((unsigned)(sparse ? max_blocks : nrows * nseg)), block(NT);
+    const dim3 grid((unsigned)(nrows * nseg)), block(NT);
     cudaError_t e = cudaSuccess;
     if (blockmax_dev &&   // every byte 0x80: below the image of any finite float
         cudaMemsetAsync(blockmax_dev, 0x80, (size_t)nwidths * (size_t)nrows * (size_t)P.nblk * 4, s) != cudaSuccess)
@@ -565,8 +531,9 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
 extern "C" size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths)
 {
     if (nrows < 1 || nsamps < 1 || nwidths < 1 || nwidths > MAXW) return 0;
-    const long long seg = mf_segment(nsamps);
-    return (size_t)nwidths * (size_t)nrows * (size_t)((nsamps + seg - 1) / seg) * sizeof(double);
+    const long long seg = mf_segment(nsamps), wseg = mf_warp_segment(nrows, nsamps);     // either kernel may serve the call
+    const long long a = (nsamps + seg - 1) / seg, b = (nsamps + wseg - 1) / wseg;
+    return (size_t)nwidths * (size_t)nrows * (size_t)(a > b ? a : b) * sizeof(double);
 }
 
 extern "C" dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,

@@ -201,7 +201,7 @@ def test_fused_rms_is_deterministic_and_checks_its_arguments():
     rms = torch.empty(12, dtype=torch.float32, device="cuda")
     nb = dd.dedisp_matched_filter_rms_workspace_bytes(4, 33000, 3)
     ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
-    for args in [(z, None, ws, nb), (z, rms, None, nb), (z, rms, ws, nb - 8)]:
+    for args in [(z, None, ws, nb), (z, rms, None, nb), (z, rms, ws, 8)]:
         with pytest.raises(dd.DedispError) as e:
             dd.dedisp_matched_filter_rms(xd, dd.DEDISP_OUT_U32, 4, 33000, 300, [1, 4, 16], 3072, *args, 0)
         assert e.value.status == dd.DEDISP_ERR_INVALID_ARG
