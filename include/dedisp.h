@@ -371,6 +371,32 @@ dedisp_status dedisp_rfi_mask(const void *x_dev, dedisp_out_dtype x_dtype, int n
                               const float *mean_dev, const float *sigma_dev, float nsigma,
                               int min_beams, unsigned char *mask_dev, void *cuda_stream);
 
+/* The same test when the beams live on several GPUs (the paper's deployment is one beam per GPU, and
+ * the coincidence test needs all 13): every rank counts its own beams,
+ *     counts[s][t] = number of LOCAL beams b with above[b][s][t]            (uint8, nbeams <= 255)
+ * the counts are summed across ranks -- the path's one real exchange step: an all-reduce(SUM) of nseries*nsamps
+ * bytes, done by the caller with NCCL (paper_1112_0065_b200.replicas.allreduce_beam_counts; the total number of
+ * beams must stay <= 255) -- and thresholded:
+ *     mask[s][t] = counts[s][t] >= min_beams.
+ * dedisp_rfi_beam_counts followed by dedisp_rfi_mask_from_counts on one GPU equals dedisp_rfi_mask.
+ * counts_dev / mask_dev: DEVICE uint8 [nseries][nsamps].  Errors as dedisp_rfi_mask. */
+dedisp_status dedisp_rfi_beam_counts(const void *x_dev, dedisp_out_dtype x_dtype, int nbeams,
+                                     long long nseries, long long nsamps, size_t beam_stride_bytes,
+                                     const float *mean_dev, const float *sigma_dev, float nsigma,
+                                     unsigned char *counts_dev, void *cuda_stream);
+dedisp_status dedisp_rfi_mask_from_counts(const unsigned char *counts_dev, long long nseries, long long nsamps,
+                                          int min_beams, unsigned char *mask_dev, void *cuda_stream);
+
+/* A consumer of the mask (reading R39; the paper says only that the mask is "written"):
+ * events whose PEAK sample is flagged are vetoed.  mask_dev is ONE series of the mask, uint8 [nsamps] (e.g. the
+ * coincidence mask of the DM-0 series of all beams); an event i < min(*count_dev, max_events) with
+ * mask[t_peak] != 0 gets series = -1 - series (in place, order kept, so the original index is recoverable);
+ * *kept_dev (int64) = number of events left.  Events vetoed by an earlier call stay vetoed and are not counted.
+ * Only enqueues work on cuda_stream.  Errors: INVALID_ARG, CUDA. */
+dedisp_status dedisp_veto_events(dedisp_event *events_dev, const long long *count_dev, long long max_events,
+                                 const unsigned char *mask_dev, long long nsamps, long long *kept_dev,
+                                 void *cuda_stream);
+
 /* ---- input-format variant: telescope-order stream ---- */
 
 /* Re-lay a time-major filterbank stream (for every time sample all channels next to

@@ -48,3 +48,20 @@ def beam_count(x, mean, sigma, nsigma) -> np.ndarray:
 def coincidence_mask(x, mean, sigma, nsigma, min_beams) -> np.ndarray:
     """uint8 [nseries, n]: 1 where at least min_beams beams exceed their threshold."""
     return (beam_count(x, mean, sigma, nsigma) >= int(min_beams)).astype(np.uint8)
+
+
+def veto_events(events: np.ndarray, mask_row: np.ndarray) -> tuple[np.ndarray, int]:
+    """A consumer of the mask (reading R39): an event whose PEAK sample is flagged in ``mask_row``
+    (uint8 [n], one series of the mask) is vetoed -- its ``series`` becomes ``-1 - series`` (order kept).
+    Returns (events with vetoes marked, number of events kept).  Events already vetoed stay so and are not counted."""
+    out = events.copy()
+    kept = 0
+    for i in range(len(out)):
+        s = int(out["series"][i])
+        if s < 0:
+            continue
+        if mask_row[int(out["t_peak"][i])]:
+            out["series"][i] = -1 - s
+        else:
+            kept += 1
+    return out, kept

@@ -72,6 +72,9 @@ ABI = {
     "dedisp_series_rms": (_i, [_vp, _ll, _ll, _vp, _vp]),
     "dedisp_transpose_time_major": (_i, [_vp, _i, _ll, _i, _vp, _vp]),
     "dedisp_rfi_mask": (_i, [_vp, _i, _i, _ll, _ll, _sz, _vp, _vp, ctypes.c_float, _i, _vp, _vp]),
+    "dedisp_rfi_beam_counts": (_i, [_vp, _i, _i, _ll, _ll, _sz, _vp, _vp, ctypes.c_float, _vp, _vp]),
+    "dedisp_rfi_mask_from_counts": (_i, [_vp, _ll, _ll, _i, _vp, _vp]),
+    "dedisp_veto_events": (_i, [_vp, _vp, _ll, _vp, _ll, _vp, _vp]),
 }
 DEDISP_MF_MAX_WIDTH = 8192
 DEDISP_EVENT_BYTES = 20      # struct dedisp_event {int series, t_start, length, t_peak; float peak;}
@@ -333,6 +336,26 @@ def dedisp_rfi_mask(x_ptr, x_dtype: int, nbeams: int, nseries: int, nsamps: int,
                                _ptr(mean_ptr), _ptr(sigma_ptr), nsigma, min_beams, _ptr(mask_ptr),
                                stream or None)
     _check(None, st, "dedisp_rfi_mask")
+
+
+def dedisp_rfi_beam_counts(x_ptr, x_dtype: int, nbeams: int, nseries: int, nsamps: int, beam_stride_bytes: int,
+                           mean_ptr, sigma_ptr, nsigma: float, counts_ptr, stream: int = 0) -> None:
+    """Per-sample number of LOCAL beams above threshold (uint8): the per-GPU half of the coincidence test."""
+    st = lib().dedisp_rfi_beam_counts(_ptr(x_ptr), x_dtype, nbeams, nseries, nsamps, beam_stride_bytes,
+                                      _ptr(mean_ptr), _ptr(sigma_ptr), nsigma, _ptr(counts_ptr), stream or None)
+    _check(None, st, "dedisp_rfi_beam_counts")
+
+
+def dedisp_rfi_mask_from_counts(counts_ptr, nseries: int, nsamps: int, min_beams: int, mask_ptr, stream: int = 0) -> None:
+    st = lib().dedisp_rfi_mask_from_counts(_ptr(counts_ptr), nseries, nsamps, min_beams, _ptr(mask_ptr), stream or None)
+    _check(None, st, "dedisp_rfi_mask_from_counts")
+
+
+def dedisp_veto_events(events_ptr, count_ptr, max_events: int, mask_ptr, nsamps: int, kept_ptr, stream: int = 0) -> None:
+    """Events whose peak sample is masked get series = -1 - series; *kept = events left (include/dedisp.h)."""
+    st = lib().dedisp_veto_events(_ptr(events_ptr) if events_ptr is not None else None, _ptr(count_ptr), max_events,
+                                  _ptr(mask_ptr), nsamps, _ptr(kept_ptr), stream or None)
+    _check(None, st, "dedisp_veto_events")
 
 
 def dedisp_transpose_time_major(in_ptr, nchans: int, nsamps: int, nbits: int, out_ptr, stream: int = 0) -> None:

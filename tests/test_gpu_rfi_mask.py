@@ -105,3 +105,58 @@ def test_argument_errors():
     assert st(x, 1, 2, 1, 64, 100, ms, ms, 3.0, 1, m) == dd.DEDISP_ERR_INVALID_ARG     # stride < beam
     assert st(x, 9, 2, 1, 64, 256, ms, ms, 3.0, 1, m) == dd.DEDISP_ERR_UNSUPPORTED_DTYPE
     assert st(0, 1, 2, 1, 64, 256, ms, ms, 3.0, 1, m) == dd.DEDISP_ERR_INVALID_ARG
+
+
+def test_beam_counts_of_subsets_summed_equal_the_mask():
+    # the multi-GPU form on one GPU: counts of two disjoint beam subsets, summed (what the all-reduce does), thresholded
+    rng = np.random.default_rng(31)
+    nb, ns, n = 13, 2, 5003                      # odd length: scalar tail
+    x = rng.standard_normal((nb, ns, n)).astype(np.float32)
+    x[:, 0, 100:110] += 6.0
+    mean = rng.normal(0, 0.1, (nb, ns)).astype(np.float32)
+    sigma = rng.uniform(0.8, 1.2, (nb, ns)).astype(np.float32)
+    s = torch.cuda.current_stream().cuda_stream
+    tot = torch.zeros((ns, n), dtype=torch.uint8, device="cuda")
+    for a, b in ((0, 7), (7, 13)):
+        xd = torch.from_numpy(np.ascontiguousarray(x[a:b])).cuda()
+        c = torch.full((ns, n), 99, dtype=torch.uint8, device="cuda")
+        dd.dedisp_rfi_beam_counts(xd, dd.DEDISP_OUT_F32, b - a, ns, n, ns * n * 4, torch.from_numpy(mean[a:b]).cuda(),
+                                  torch.from_numpy(sigma[a:b]).cuda(), 2.0, c, s)
+        torch.cuda.synchronize()
+        assert np.array_equal(c.cpu().numpy(), RM.beam_count(x[a:b], mean[a:b], sigma[a:b], 2.0).astype(np.uint8))
+        tot += c
+    for k in (1, 4, 13, 14, 0):
+        m = torch.full((ns, n), 7, dtype=torch.uint8, device="cuda")
+        dd.dedisp_rfi_mask_from_counts(tot, ns, n, k, m, s)
+        torch.cuda.synchronize()
+        assert np.array_equal(m.cpu().numpy(), RM.coincidence_mask(x, mean, sigma, 2.0, k)), k
+    with pytest.raises(dd.DedispError):
+        dd.dedisp_rfi_beam_counts(tot, dd.DEDISP_OUT_F32, 256, ns, n, ns * n * 4, tot, tot, 2.0, tot, s)
+
+
+def test_veto_events_marks_events_with_a_masked_peak():
+    from oracle import peak_finding as PF
+    z = W.filtered_like(9, 5, 6000, npulses=6).astype(np.float32)
+    sigma = PF.series_rms(z).astype(np.float32)
+    want = PF.find_events(z, sigma, 3.0)
+    assert len(want) > 20
+    rng = np.random.default_rng(2)
+    mask = (rng.random(6000) < 0.3).astype(np.uint8)
+    zd, sd = torch.from_numpy(z).cuda(), torch.from_numpy(sigma).cuda()
+    wsb = dd.dedisp_find_events_workspace_bytes(5, 6000)
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    cap = 1 << 16
+    ev = torch.zeros((cap, 5), dtype=torch.int32, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    kept = torch.full((1,), -5, dtype=torch.int64, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    dd.dedisp_find_events(zd, 5, 6000, sd, 3.0, ws, wsb, ev, cap, cnt, s)
+    dd.dedisp_veto_events(ev, cnt, cap, torch.from_numpy(mask).cuda(), 6000, kept, s)
+    torch.cuda.synchronize()
+    exp, nkept = RM.veto_events(want, mask)
+    got = ev[: int(cnt.item())].cpu().numpy()
+    assert int(kept.item()) == nkept and 0 < nkept < len(want)
+    assert np.array_equal(got[:, 0], exp["series"]) and np.array_equal(got[:, 3], exp["t_peak"])
+    dd.dedisp_veto_events(ev, cnt, cap, torch.ones(6000, dtype=torch.uint8, device="cuda"), 6000, kept, s)   # again
+    torch.cuda.synchronize()
+    assert int(kept.item()) == 0 and (ev[: int(cnt.item()), 0] < 0).all()

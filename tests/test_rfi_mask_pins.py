@@ -86,3 +86,30 @@ def test_monotone_in_min_beams_and_limits():
     assert np.all(RM.coincidence_mask(x, z, o, 0.5, 14) == 0)
     np.testing.assert_array_equal(RM.coincidence_mask(x, z, o, 0.5, 1), (x > 0.5).any(axis=0))
     np.testing.assert_array_equal(RM.coincidence_mask(x, z, o, 0.5, 13), (x > 0.5).all(axis=0))
+
+
+def test_veto_events_hand_worked():
+    # reading R39: an event is vetoed when its PEAK sample is masked; series -> -1 - series, order kept
+    from oracle import peak_finding as PF
+    ev = np.zeros(4, dtype=PF.EVENT_DTYPE)
+    ev["series"] = [0, 0, 3, 5]
+    ev["t_start"] = [2, 10, 4, 7]
+    ev["length"] = [3, 1, 4, 2]
+    ev["t_peak"] = [3, 10, 7, 8]
+    mask = np.zeros(12, np.uint8)
+    mask[[2, 7, 10]] = 1                     # t_start of event 0 is masked, its peak (3) is not
+    out, kept = RM.veto_events(ev, mask)
+    assert kept == 2 and out["series"].tolist() == [0, -1, -4, 5]
+    assert np.array_equal(out["t_peak"], ev["t_peak"]) and ev["series"].tolist() == [0, 0, 3, 5]
+    out2, kept2 = RM.veto_events(out, np.ones(12, np.uint8))      # vetoed events stay vetoed, are not counted
+    assert kept2 == 0 and out2["series"].tolist() == [-1, -1, -4, -6]
+
+
+def test_counts_of_beam_subsets_add_up_to_the_coincidence_mask():
+    # the multi-GPU form: counts of disjoint beam subsets summed, then thresholded == the mask over all beams
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal((13, 2, 500)).astype(np.float32)
+    mean, sigma = rng.normal(0, 0.1, (13, 2)).astype(np.float32), rng.uniform(0.8, 1.2, (13, 2)).astype(np.float32)
+    total = sum(RM.beam_count(x[a:b], mean[a:b], sigma[a:b], 1.0) for a, b in ((0, 4), (4, 9), (9, 13)))
+    assert np.array_equal(total, RM.beam_count(x, mean, sigma, 1.0))
+    assert np.array_equal((total >= 4).astype(np.uint8), RM.coincidence_mask(x, mean, sigma, 1.0, 4))
