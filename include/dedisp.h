@@ -420,8 +420,12 @@ dedisp_status dedisp_transpose_time_major(const void *in_dev, int nchans, long l
  * ranges, output row ranges), else 0.
  * dedisp_debug_check_errors: copies the 8 failure counters of such a build to counts_out ([0] = total, [1] =
  * shared-memory range, [2] = ring stage tag, [3] = TMA source, [4] = output range, [5] = pre-pass range); all zero
- * in a normal build.  Synchronises the device. */
+ * in a normal build.  Synchronises the device.
+ * dedisp_debug_inject_fault: kind 1 makes the producer warp of a -DDEDISP_CHECKS build stamp a wrong tag on the
+ * first ring stage every CTA fills (the data is still right), so that the stage-tag check must count failures --
+ * the test that the checks can fail at all; kind 0 switches it off; no effect in a normal build. */
 int dedisp_debug_checks_compiled(void);
+dedisp_status dedisp_debug_inject_fault(dedisp_plan plan, int kind);
 dedisp_status dedisp_debug_set_poison(dedisp_plan plan, int byte_value);
 dedisp_status dedisp_debug_check_errors(dedisp_plan plan, unsigned long long *counts_out);
 

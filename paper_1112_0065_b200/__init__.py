@@ -55,6 +55,7 @@ ABI = {
     "dedisp_get_launch_count": (ctypes.c_ulonglong, []),
     "dedisp_debug_checks_compiled": (_i, []),
     "dedisp_debug_set_poison": (_i, [_vp, _i]),
+    "dedisp_debug_inject_fault": (_i, [_vp, _i]),
     "dedisp_debug_check_errors": (_i, [_vp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "dedisp_get_last_cuda_error": (_i, [_vp]),
     "dedisp_get_error_string": (ctypes.c_char_p, [_i]),
@@ -212,6 +213,10 @@ def dedisp_debug_checks_compiled() -> bool:
 
 def dedisp_debug_set_poison(plan: int, byte_value: int) -> None:
     _check(plan, lib().dedisp_debug_set_poison(plan, byte_value), "dedisp_debug_set_poison")
+
+
+def dedisp_debug_inject_fault(plan: int, kind: int) -> None:
+    _check(plan, lib().dedisp_debug_inject_fault(plan, kind), "dedisp_debug_inject_fault")
 
 
 def dedisp_debug_check_errors(plan: int) -> list:

@@ -251,6 +251,7 @@ struct BitsliceParams {
     unsigned long long *check_errors;   // [DEDISP_NCHECK] or nullptr
     unsigned long long scratch_words;   // words in `planes`
     int ndm;
+    int inject_fault;                   // dedisp_debug_inject_fault: 1 = stamp a wrong tag on one ring stage
 };
 // what the self-checks count (index into check_errors)
 enum {

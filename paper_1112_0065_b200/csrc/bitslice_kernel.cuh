@@ -358,7 +358,8 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                 const uint32_t sb = smem_u32(smem) + stage * S::BYTES;
                 const uint32_t fb = full0 + 8 * stage;
 #ifdef DEDISP_CHECKS
-                if (lane == 0) tags[stage] = item * nchunks + chunk;   // ordered before the arrive on full[] below
+                if (lane == 0)      // ordered before the arrive on full[] below
+                    tags[stage] = (P.inject_fault == 1 && item == blockIdx.x && chunk == 0) ? -1 : item * nchunks + chunk;
                 __syncwarp();
 #endif
                 if constexpr (C::NV == 1) {
@@ -516,6 +517,7 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     BitsliceParams P;
     P.planes = plan->d_planes;
     P.check_errors = plan->d_check_errors;
+    P.inject_fault = plan->inject_fault;
     P.scratch_words = plan->planes_bytes / 4;
     P.ndm = plan->ndm;
     P.vinfo = nullptr;
@@ -659,6 +661,7 @@ dedisp_status execute_pairs(dedisp_plan plan, const PairTables &T, int nbeams, l
     BitsliceParams P;
     P.planes = plan->d_pair_rows;
     P.check_errors = plan->d_check_errors;
+    P.inject_fault = plan->inject_fault;
     P.scratch_words = plan->pair_rows_bytes / 4;
     P.ndm = plan->ndm;
     P.vrows = T.nrows;

@@ -441,6 +441,13 @@ dedisp_status dedisp_debug_set_poison(dedisp_plan plan, int byte_value)
     return DEDISP_OK;
 }
 
+dedisp_status dedisp_debug_inject_fault(dedisp_plan plan, int kind)
+{
+    if (!plan || kind < 0 || kind > 1) return DEDISP_ERR_INVALID_ARG;
+    plan->inject_fault = kind;
+    return DEDISP_OK;
+}
+
 dedisp_status dedisp_debug_check_errors(dedisp_plan plan, unsigned long long *counts_out)
 {
     if (!plan || !counts_out) return DEDISP_ERR_INVALID_ARG;

@@ -81,6 +81,7 @@ struct dedisp_plan_s {
     TensorMapCache tmap[3];       // pair rows of 2-, 4- and 8-bit samples
     // diagnostics (dedisp_debug_set_poison / dedisp_debug_check_errors)
     int poison = -1;                               // >= 0: every execute first fills the scratch with this byte
+    int inject_fault = 0;                          // -DDEDISP_CHECKS builds: a deliberate fault the checks must count
     unsigned long long *d_check_errors = nullptr;  // [DEDISP_NCHECK] failure counters of a -DDEDISP_CHECKS build
     int sm_count = 0;             // multiprocessors of `device` (set_dm_list)
     // ordering of the plan-owned scratch between executes on different streams: the stream and an event after the

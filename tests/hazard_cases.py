@@ -23,6 +23,7 @@ tests/test_gpu_selfcheck.py runs both builds over all cases.  Cases:
   unaligned  input base pointer at odd byte offsets: the guarded 128-bit straddling loads of the unpack pre-pass
   multi      several persistent work items per CTA (the ring wraps many times) and a ragged last tile
   search     dedisp_matched_filter_rms + dedisp_find_events_hinted (rows f1 + f2)
+  fault_injection   a deliberately wrong ring-stage tag must be counted by the checks build (the checks can fail)
 """
 import sys
 from pathlib import Path
@@ -149,15 +150,45 @@ def search():
     assert np.array_equal(got[:, 1], want["t_start"]) and np.array_equal(got[:, 3], want["t_peak"])
 
 
-CASES = {f.__name__: f for f in (tiny_auto, tiny_direct, pairs3, pairs8, blocks, unaligned, multi, search)}
+def fault_injection():
+    """The checks can fail: with a wrong tag stamped on one ring stage per CTA (dedisp_debug_inject_fault) the
+    -DDEDISP_CHECKS build counts stage-tag failures -- and nothing else, the data being right the result still
+    equals the oracle.  A product build has no checks compiled in and counts nothing."""
+    w = HTRU.scaled(ndm=84, dm_lo=930.0, dm_hi=930.0 + STEP * 83, nsamps_out=4100)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    x = W.generate(w, md)
+    want = oracle.dedisperse(delay, x, 2, w.nsamps_out)
+    counted = []
+    for kernel in (dd.DEDISP_KERNEL_PAIRS, dd.DEDISP_KERNEL_BITSLICE):
+        p = dd.dedisp_plan_create(w.nchans, w.dt, w.f_top, w.df)
+        dd.dedisp_set_dm_list(p, list(w.dms()))
+        dd.dedisp_set_kernel(p, kernel)
+        dd.dedisp_debug_inject_fault(p, 1)
+        out = torch.zeros((w.ndm, w.nsamps_out), dtype=torch.int32, device="cuda")
+        dd.dedisp_execute(p, w.nsamps_out, torch.from_numpy(x).cuda(), 2, out, dd.DEDISP_OUT_U32,
+                          torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), want)
+        errs = dd.dedisp_debug_check_errors(p)
+        if dd.dedisp_debug_checks_compiled():
+            assert errs[2] > 0 and errs[0] == errs[2], errs        # CHK_STAGE_TAG only
+        else:
+            assert errs[0] == 0, errs
+        counted.append(errs[2])
+        dd.dedisp_destroy(p)
+    return f"bit-exact vs oracle; injected wrong stage tags counted by the checks: {counted} (pair rows, planes)"
+
+
+CASES = {f.__name__: f for f in (tiny_auto, tiny_direct, pairs3, pairs8, blocks, unaligned, multi, search, fault_injection)}
 
 
 def main(argv):
     assert torch.cuda.is_available(), "needs a CUDA device (there is no CPU fallback)"
     names = argv or list(CASES)
     for n in names:
-        CASES[n]()
-        print(f"case {n}: ok (bit-exact vs oracle, guards intact, 3 scratch poisons, 0 check failures)", flush=True)
+        note = CASES[n]()
+        print(f"case {n}: ok ({note or 'bit-exact vs oracle, guards intact, 3 scratch poisons, 0 check failures'})",
+              flush=True)
     print(f"hazard_cases: {len(names)} cases ok; in-kernel checks compiled: {dd.dedisp_debug_checks_compiled()}; "
           f"launches={dd.dedisp_get_launch_count()}", flush=True)
 
