@@ -177,6 +177,14 @@ def ncu_traffic_bytes(config: str):
 
 
 KERNEL_NAMES = {1: "direct_kernel", 2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows"}
+# ALU-pipe (LOP3 / SHF / LEA: 64 lanes per clock and SM) instructions per addition of the dominant kernel's hot loop,
+# counted on the SASS / the ncu source page: (kernel, nbits) -> (lane-instructions per add, where it was counted)
+ALU_PIPE_INSTR_PER_ADD = {
+    (3, 2): (626.0 / 4096.0, "profiles/r2_sass_cfg3p.txt: 626 ALU-pipe of 918 instructions per 4096 adds"),
+    (3, 8): (0.455, "profiles/r2_wide8.md: ncu source page, LOP3 + SHF share of 23.97 G instructions"),
+    (2, 2): (0.21, "DESIGN.md Sec. 6 C: 62 full adders + ripple + 64 SHF per 32 channels and word"),
+}
+ALU_PIPE_LANES_PER_CLK_PER_SM = 64
 
 
 def measure_dedisperse(torch, dd, w, k, kernel, steps, warmup, rank, world, dev, stream, flush, e2e_steps):
@@ -277,6 +285,19 @@ def measure_dedisperse(torch, dd, w, k, kernel, steps, warmup, rank, world, dev,
     return m
 
 
+def instr_bound(w, m, achieved_adds_per_s, props, sm_max_mhz):
+    """Fraction of the 64-lane ALU pipe the dominant kernel's hot loop keeps busy, from its counted ALU-pipe
+    instructions per addition (None where no count is committed)."""
+    ent = ALU_PIPE_INSTR_PER_ADD.get((m["kernel_used"], w.nbits))
+    if ent is None:
+        return None
+    per_add, src = ent
+    pipe_peak = props.multi_processor_count * ALU_PIPE_LANES_PER_CLK_PER_SM * sm_max_mhz * 1e6
+    return {"bound": "alu_pipe", "alu_pipe_instr_per_add": per_add, "achieved": per_add * achieved_adds_per_s / 1e12,
+            "peak": pipe_peak / 1e12, "unit": "T lane-instr/s", "frac": per_add * achieved_adds_per_s / pipe_peak,
+            "source": src}
+
+
 def roofline_of(w, k, m, ms_per_step, props, peaks, config_name):
     """north_star's roofline: the slower of nchans*ndm*nsamps adds at the ALU peak and the compulsory bytes at the HBM
     bandwidth; `achieved` = adds / the dominant kernel's mean launch time (CUDA events inside the library, live)."""
@@ -297,7 +318,10 @@ def roofline_of(w, k, m, ms_per_step, props, peaks, config_name):
                            f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz); see DESIGN.md",
             "algorithmic_bytes": m["in_bytes"] + m["out_bytes"],
             "hbm_frac": ((m["in_bytes"] + m["out_bytes"]) / mm) / hbm_peak,
-            "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3)}
+            "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3),
+            "frac_note": "north_star's fraction counts one add per lane-op; a bit-sliced LOP3 pair adds 32 samples and "
+                         "pair rows share two-channel sums, so it can exceed 1 -- instr_bound is the physical limiter",
+            "instr_bound": instr_bound(w, m, achieved, props, sm_max_mhz)}
 
 
 def run_ours(args) -> None:
