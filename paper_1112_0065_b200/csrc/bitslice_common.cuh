@@ -48,8 +48,9 @@
 #define BS8_NSTAGE 3
 #endif
 #ifndef BS8_NSPLIT
-#define BS8_NSPLIT 2
-#endif
+#define BS8_NSPLIT 8      // round 2: one plane per tree -- with the carries chained across the subsets (add_chunk) more
+#endif                    // subsets cost nothing and the 160-byte spill of NSPLIT = 2 is gone: wide8 on the plain kernel
+                          // 57.1 -> 55.4 ms (NSPLIT 4: 55.6), profiles/r2_wide8.md
 #ifndef BS8_WIN_S
 #define BS8_WIN_S 80
 #endif
@@ -116,8 +117,8 @@ struct Cfg {
 };
 // 2-bit samples: 15 x 4 words = 1920-sample tiles, 32-channel trees, sums < 4096
 using Cfg2 = Cfg<2, BS_NW, BS_W, BS_TREE_K, BS_NSTAGE, 12, 96, 224, BS_NSPLIT>;
-// 8-bit samples: 11 x 4 words = 1408-sample tiles, 16-channel trees run once per nibble (NSPLIT = 2:
-// the temporaries of a 4-plane tree leave room for 11 consumer warps at 168 registers), sums < 2^20
+// 8-bit samples: 11 x 4 words = 1408-sample tiles, 16-channel trees run once per plane subset (round 1: NSPLIT = 2,
+// the temporaries of a 4-plane tree leave room for 11 consumer warps at 168 registers; round 2: NSPLIT = 8), sums < 2^20
 // (sweeps on B200, wide8, kernel ms.  One 8-plane tree, (NW,W,K,NSTAGE): (14,2,2,3) 81.6, (7,4,2,3) 75.0,
 //  (6,4,2,3) 85.8, (12,2,3,3) 91.5, (10,2,3,3) 101.9, (7,4,3,3) 74.5 [ALU pipe 69 % busy: 2 warps per
 //  sub-partition], (6,4,3,3) 84.9.  Split trees, (NSPLIT,NW,K,NSTAGE): (2,7,3,3) 73.7, (2,11,3,3) 60.7,
@@ -153,7 +154,10 @@ using Cfg4 = Cfg<4, BS4_NW, BS4_W, BS4_TREE_K, BS4_NSTAGE, 16, 96, 224, BS4_NSPL
 #define BS6_TREE_K 3
 #endif
 using Cfg3 = Cfg<3, BS3_NW, 4, BS3_TREE_K, 3, 13, 96, 224>;
-using Cfg5 = Cfg<5, BS5_NW, 4, BS5_TREE_K, 3, 16, 96, 224>;
+#ifndef BS5_NSPLIT
+#define BS5_NSPLIT 5      // (one plane per tree: no spill; 8 x scrunched gulp 2.99 -> 2.90 ms)
+#endif
+using Cfg5 = Cfg<5, BS5_NW, 4, BS5_TREE_K, 3, 16, 96, 224, BS5_NSPLIT>;
 using Cfg6 = Cfg<6, BS6_NW, 4, BS6_TREE_K, 3, 16, 96, 160, BS6_NSPLIT>;
 
 // Pair sums: a virtual channel is the exact sum of two adjacent 2-bit
@@ -202,7 +206,10 @@ using Cfg3P = Cfg<3, BS3P_NW, BS3P_W, BS3P_TREE_K, BS3P_NSTAGE, 13, 96, 96, 1, 3
 #ifndef BS5P_NSTAGE
 #define BS5P_NSTAGE 2
 #endif
-using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, 1, 3>;
+#ifndef BS5P_NSPLIT
+#define BS5P_NSPLIT 5     // (one plane per tree: the 36-44 byte spill is gone; gulp at 4 bits, kernel 1.567 -> 1.512 ms)
+#endif
+using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, BS5P_NSPLIT, 3>;
 #ifndef BS9P_W
 #define BS9P_W 4
 #endif

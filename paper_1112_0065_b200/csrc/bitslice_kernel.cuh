@@ -195,29 +195,28 @@ __device__ __forceinline__ void add_chunk(uint32_t (&A)[C::NP][C::W], const uint
     Tree<C, C::K, 0, WIN, P0>::run(A, tb, relp, sc, e);
 #pragma unroll
     for (int j = 0; j < W; ++j) {
+        uint32_t cj;
         if constexpr (S == 0) {
-            c[j] = A[B][j] & e[0][j];
+            cj = A[B][j] & e[0][j];
             A[B][j] ^= e[0][j];
         } else {
-            c[j] = full_add(A[B][j], e[0][j], c[j]);   // c: weight 2^B, handed over by subset S - 1
+            cj = full_add(A[B][j], e[0][j], c[j]);   // c: weight 2^B, handed over by subset S - 1
         }
 #pragma unroll
-        for (int i = 1; i < NBS; ++i) c[j] = full_add(A[B + i][j], e[i][j], c[j]);
-    }
-    if constexpr (S + 1 < C::NSPLIT) {
-        add_chunk<C, WIN, S + 1>(A, tb, relp, sc, c);
-    } else {
-#pragma unroll
-        for (int j = 0; j < W; ++j) {
-#pragma unroll
+        for (int i = 1; i < NBS; ++i) cj = full_add(A[B + i][j], e[i][j], cj);
+        if constexpr (S + 1 < C::NSPLIT) {
+            c[j] = cj;                               // carry in of the next subset
+        } else {                                     // last subset: ripple into the top planes (word by word: one
+#pragma unroll                                       // live carry register, as before the subsets were chained)
             for (int p = B + NBS; p < NP - 1; ++p) {
-                const uint32_t t = A[p][j] & c[j];
-                A[p][j] ^= c[j];
-                c[j] = t;
+                const uint32_t t = A[p][j] & cj;
+                A[p][j] ^= cj;
+                cj = t;
             }
-            if (B + NBS < NP) A[NP - 1][j] ^= c[j];
+            if (B + NBS < NP) A[NP - 1][j] ^= cj;
         }
     }
+    if constexpr (S + 1 < C::NSPLIT) add_chunk<C, WIN, S + 1>(A, tb, relp, sc, c);
 }
 
 // Work-item order (P.gblock): blocks of gblock DM groups; inside a block consecutive items are the
