@@ -81,7 +81,8 @@ typedef enum {
     DEDISP_ERR_UNSUPPORTED_DTYPE = 4, /* out_dtype not U32/F32 */
     DEDISP_ERR_OVERFLOW = 5,          /* nchans*(2^nbits-1) >= 2^24, or a delay beyond int32 */
     DEDISP_ERR_ALLOC = 6,             /* host or device allocation failed */
-    DEDISP_ERR_CUDA = 7               /* CUDA runtime error; see dedisp_get_last_cuda_error */
+    DEDISP_ERR_CUDA = 7,              /* CUDA runtime error; see dedisp_get_last_cuda_error */
+    DEDISP_ERR_SCRATCH_LIMIT = 8      /* dedisp_execute_static: the problem needs more than the fixed static scratch */
 } dedisp_status;
 
 typedef enum { DEDISP_OUT_U32 = 0, DEDISP_OUT_F32 = 1 } dedisp_out_dtype;
@@ -161,6 +162,30 @@ size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, l
  * later executes of that size or smaller never allocate (see "Streams and scratch").  Synchronises
  * the device if it has to re-allocate.  Errors: INVALID_ARG, NO_DM_LIST, UNSUPPORTED_NBITS, ALLOC. */
 dedisp_status dedisp_reserve(dedisp_plan plan, int nbeams, long long nsamps_out, int in_nbits);
+
+/* dedisp_execute for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): one beam through the plain tiled kernel (what DEDISP_KERNEL_BITSLICE runs: unpack
+ * pre-pass -> bit planes -> TMA-staged gather-sum), with the bit planes in a file-scope device array of
+ * DEDISP_STATIC_SCRATCH_BYTES (32 MiB) instead of the plan's cudaMalloc'ed scratch.  The call -- the first one
+ * included -- calls no cudaMalloc / cudaFree and no allocating library routine; the first call on a device looks the
+ * array's device address up (cudaGetSymbolAddress; CUDA loads modules lazily, so this is also when the driver
+ * reserves the 32 MiB) and sets the kernel's shared-memory attribute, and a plan's first call outside a capture
+ * creates the plan's ordering event: make one call outside a capture first.  Same arguments, layouts and result (bit for bit) as dedisp_execute; the current device
+ * must be the one dedisp_set_dm_list ran on.
+ *   Limit: the bit planes of the call, nchans_pad * in_nbits * row_pitch * 4 bytes (row_pitch ~ (nsamps_out +
+ *   max_delay) / 32 + 200 words, nchans_pad = nchans rounded up to 32), must fit 32 MiB -- the HTRU gulp (1024 channels,
+ *   2 bits, 65 536 + 20 476 samples: 23.3 MB) does, the 8-bit wideband config (750 MB) does not: DEDISP_ERR_SCRATCH_LIMIT.
+ *   Plans the tiled kernel cannot serve return DEDISP_ERR_INVALID_ARG (there is no DIRECT fallback here).
+ *   Cost: every GPU that loads the library holds the 32 MiB until the process exits; no pair rows (they need 373 MB for
+ *   the gulp), so the gulp takes 1.20 ms instead of 1.04 ms.
+ *   Sharing: the array is ONE per process and device, shared by all plans, streams and threads, and keeps the last
+ *   call's contents (nothing needs clearing: the pre-pass rewrites every word a call reads).  Calls that overlap on the
+ *   GPU race on it and give wrong sums: serialise them (one stream, or events).  Calls of one plan on different
+ *   streams are ordered as for dedisp_execute. */
+#define DEDISP_STATIC_SCRATCH_BYTES (32u << 20)
+size_t dedisp_static_scratch_bytes(void);
+dedisp_status dedisp_execute_static(dedisp_plan plan, long long nsamps_out, const void *in_dev, int in_nbits,
+                                    void *out_dev, dedisp_out_dtype out_dtype, void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers (tight beam strides): copies the
  * packed input host->device, runs dedisp_execute_batch, copies the result back

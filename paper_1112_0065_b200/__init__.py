@@ -24,6 +24,7 @@ DEDISP_ERR_UNSUPPORTED_DTYPE = 4
 DEDISP_ERR_OVERFLOW = 5
 DEDISP_ERR_ALLOC = 6
 DEDISP_ERR_CUDA = 7
+DEDISP_ERR_SCRATCH_LIMIT = 8
 DEDISP_OUT_U32 = 0
 DEDISP_OUT_F32 = 1
 DEDISP_KERNEL_AUTO = 0
@@ -42,6 +43,8 @@ ABI = {
     "dedisp_get_in_row_stride_bytes_tscrunch": (_sz, [_vp, _i, _ll, _i]),
     "dedisp_execute_host": (_i, [_vp, _i, _ll, _vp, _i, _vp, _i]),
     "dedisp_reserve": (_i, [_vp, _i, _ll, _i]),
+    "dedisp_static_scratch_bytes": (_sz, []),
+    "dedisp_execute_static": (_i, [_vp, _ll, _vp, _i, _vp, _i, _vp]),
     "dedisp_destroy": (_i, [_vp]),
     "dedisp_get_max_delay": (_i, [_vp]),
     "dedisp_get_nchans": (_i, [_vp]),
@@ -169,6 +172,17 @@ def dedisp_execute_host(plan: int, nbeams: int, nsamps_out: int, in_host, in_nbi
 
 def dedisp_reserve(plan: int, nbeams: int, nsamps_out: int, in_nbits: int) -> None:
     _check(plan, lib().dedisp_reserve(plan, nbeams, nsamps_out, in_nbits), "dedisp_reserve")
+
+
+def dedisp_static_scratch_bytes() -> int:
+    return int(lib().dedisp_static_scratch_bytes())
+
+
+def dedisp_execute_static(plan: int, nsamps_out: int, in_ptr, in_nbits: int, out_ptr, out_dtype: int,
+                          stream: int = 0) -> None:
+    """dedisp_execute with the bit planes in a fixed 32 MiB device array: allocates nothing (include/dedisp.h)."""
+    st = lib().dedisp_execute_static(plan, nsamps_out, _ptr(in_ptr), in_nbits, _ptr(out_ptr), out_dtype, stream or None)
+    _check(plan, st, "dedisp_execute_static")
 
 
 def dedisp_destroy(plan: int) -> None:

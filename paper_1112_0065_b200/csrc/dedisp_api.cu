@@ -473,6 +473,7 @@ const char *dedisp_get_error_string(dedisp_status s)
         case DEDISP_ERR_OVERFLOW: return "sum or delay out of range";
         case DEDISP_ERR_ALLOC: return "allocation failed";
         case DEDISP_ERR_CUDA: return "CUDA error";
+        case DEDISP_ERR_SCRATCH_LIMIT: return "problem exceeds the 32 MiB static scratch of dedisp_execute_static";
     }
     return "unknown status";
 }
