@@ -321,7 +321,7 @@ def roofline_of(w, k, m, ms_per_step, props, peaks, config_name):
             "step_roofline_frac": max(t_alu, t_hbm) / (ms_per_step * 1e-3),
             "frac_note": "north_star's fraction counts one add per lane-op; a bit-sliced LOP3 pair adds 32 samples and "
                          "pair rows share two-channel sums, so it can exceed 1 -- instr_bound is the physical limiter",
-            "instr_bound": instr_bound(w, m, achieved, props, sm_max_mhz)}
+            "instr_bound": instr_bound(w, m, achieved, props, sm_max_mhz) if k == 1 else None}
 
 
 def run_ours(args) -> None:
