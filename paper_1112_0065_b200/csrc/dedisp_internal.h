@@ -213,3 +213,4 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
                           int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                           const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks);
 long long mf_warp_segment(long long nrows, long long nsamps);
+size_t mf_warp_workspace_bytes(long long nrows, long long nsamps, int nwidths);   // partial sums + per-row prefix sums

@@ -20,6 +20,7 @@
 // x[t-R-1]; the two trailing streams hit L2), two block scans, then the outputs of
 // the step that lags wmax samples behind, written with coalesced 4-byte stores.
 #include <cmath>
+#include <cstdlib>
 #include <type_traits>
 
 #include "dedisp_internal.h"
@@ -418,7 +419,10 @@ dedisp_status mf_run(const void *x_dev, dedisp_out_dtype x_dtype, long long nrow
                      int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                      const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks)
 {
-    if (sparse_list || !z_dev)
+    // (A/B hook: DEDISP_MF_WARP_DENSE=1 sends the dense pass of dedisp_matched_filter_rms -- which has a workspace for
+    // the prefix sums -- through the warp kernel too; profiles/r2_matched_filter.md)
+    static const bool warp_dense = getenv("DEDISP_MF_WARP_DENSE") != nullptr;
+    if (sparse_list || !z_dev || (warp_dense && rms_dev && workspace_dev))
         return mf_warp_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, z_dev, rms_dev, blockmax_dev,
                            workspace_dev, workspace_bytes, cuda_stream, sparse_list, sparse_count, zc, max_blocks);
     if (!x_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0)
@@ -531,9 +535,10 @@ extern "C" dedisp_status dedisp_matched_filter(const void *x_dev, dedisp_out_dty
 extern "C" size_t dedisp_matched_filter_rms_workspace_bytes(long long nrows, long long nsamps, int nwidths)
 {
     if (nrows < 1 || nsamps < 1 || nwidths < 1 || nwidths > MAXW) return 0;
-    const long long seg = mf_segment(nsamps), wseg = mf_warp_segment(nrows, nsamps);     // either kernel may serve the call
-    const long long a = (nsamps + seg - 1) / seg, b = (nsamps + wseg - 1) / wseg;
-    return (size_t)nwidths * (size_t)nrows * (size_t)(a > b ? a : b) * sizeof(double);
+    const long long seg = mf_segment(nsamps);     // either kernel may serve the call
+    const size_t a = (size_t)nwidths * (size_t)nrows * (size_t)((nsamps + seg - 1) / seg) * sizeof(double);
+    const size_t b = mf_warp_workspace_bytes(nrows, nsamps, nwidths);
+    return a > b ? a : b;
 }
 
 extern "C" dedisp_status dedisp_matched_filter_rms(const void *x_dev, dedisp_out_dtype x_dtype, long long nrows,

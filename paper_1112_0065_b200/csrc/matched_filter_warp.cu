@@ -48,13 +48,15 @@ constexpr int WPB = 2;           // (independent) warps per CTA
 constexpr int NT = 32 * WPB;
 constexpr int E = 2048;          // outputs per block of the block-maximum hint (dedisp_find_events_hinted)
 constexpr int MAXW = 16;         // boxcar widths per call
+constexpr int PB = 256;          // samples per block of the per-row prefix sums
 static_assert(E % WS == 0, "a hint block is a whole number of warp steps");
 
 struct MFParams {
     const void *x;               // [nrows][n] uint32 or float32 (exact integers)
     float *z;                    // [nw][nrows][n], or null (RMS / block maxima only)
     long long nrows, n;
-    long long nitems;            // dense: nrows * nseg work items
+    long long nitems;            // dense: work items of this launch = rows of the launch * nseg
+    long long row0;              // dense: first row of this launch (rows are processed in L2-sized blocks)
     long long plane;             // elements between the outputs of consecutive widths (nrows * n; 0 in sparse mode)
     int radius;
     int nw;
@@ -68,12 +70,19 @@ struct MFParams {
     int guard_lim;               // guarded 32-bit mode: |NY| <= guard_lim => every boxcar fits int32
     unsigned long long guard_hist;   // mask of the step flags the outputs of one step depend on
     int w[MAXW];
+    int wl[MAXW];                // width indices: those with w % 4 == 0 first (n4 of them), then the others
+    int n4;
     float scale[MAXW];           // fl32(1 / (N sqrt(w)))
     double *partial;             // RMS variant: [nw][nrows][nseg] sums of z^2 over a segment
     int *blockmax;               // RMS variant, optional: [nw][nrows][nblk] upper bounds of z per block of E outputs
     int nblk;
     // sparse re-computation (dedisp_search_events): warp i re-runs the steps that produce block sparse_list[i].y of
     // series sparse_list[i].x (= width index * nrows + row) and stores that block's E outputs at zc + i*E
+    // per-row prefix sums of x at multiples of PB samples (mf_prefix_kernel): prefix[row * (pnb + 1) + k] =
+    // sum of x[row][0 .. min(k * PB, n)); the window sum at the start of a work item is then two look-ups and two
+    // edges of < PB samples instead of a sum over N = 2R + 1 samples -- which makes short segments affordable
+    const unsigned long long *prefix;
+    int pnb;
     const int2 *sparse_list;     // nullptr: the dense pass
     const int *sparse_count;     // number of valid entries (device)
     float *zc;
@@ -209,7 +218,7 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
         seglen = (int)(want < nrem ? want : nrem);
     } else {
         if (item >= P.nitems) return;
-        row = item / P.nseg;
+        row = P.row0 + item / P.nseg;
         seg = (int)(item % P.nseg);
         lo = (long long)seg * P.seg;
         seglen = (int)((lo + P.seg < n) ? P.seg : n - lo);
@@ -229,20 +238,31 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
     if (a0 > n - N) a0 = n - N;
     ACC carryW = 0;
     {
-        const uint32_t *wb = xr + (a0 - lo);
-        int head = (int)((4 - (((uintptr_t)wb >> 2) & 3)) & 3);      // scalars up to 16-byte alignment
-        if (head > N) head = (int)N;
+        const uint32_t *wb = xr + (a0 - lo);      // first sample of the window; the window is [a0, a0 + N) of the row
         ACC part = 0;
-        if (lane < head) part += (ACC)cvt_x<XF32>(__ldg(wb + lane));
-        const int nvec = (int)((N - head) >> 2);
-        const uint4 *vb = reinterpret_cast<const uint4 *>(wb + head);
-        for (int v = lane; v < nvec; v += 32) {
-            const uint4 q = __ldg(vb + v);
-            part += (ACC)cvt_x<XF32>(q.x) + (ACC)cvt_x<XF32>(q.y) + (ACC)cvt_x<XF32>(q.z) +
-                    (ACC)cvt_x<XF32>(q.w);
+        const long long ka = (a0 + PB - 1) / PB, kb = (a0 + N) / PB;
+        if (P.prefix && ka <= kb) {
+            // whole blocks from the prefix sums, the two edges (< PB samples each) sample by sample
+            const unsigned long long *pr = P.prefix + (size_t)row * (size_t)(P.pnb + 1);
+            const int e0 = (int)(ka * PB - a0), e1 = (int)(a0 + N - kb * PB);
+            for (int i = lane; i < e0; i += 32) part += (ACC)cvt_x<XF32>(__ldg(wb + i));
+            const uint32_t *wt = wb + (N - e1);
+            for (int i = lane; i < e1; i += 32) part += (ACC)cvt_x<XF32>(__ldg(wt + i));
+            if (lane == 0) part += (ACC)(__ldg(pr + kb) - __ldg(pr + ka));
+        } else {
+            int head = (int)((4 - (((uintptr_t)wb >> 2) & 3)) & 3);      // scalars up to 16-byte alignment
+            if (head > N) head = (int)N;
+            if (lane < head) part += (ACC)cvt_x<XF32>(__ldg(wb + lane));
+            const int nvec = (int)((N - head) >> 2);
+            const uint4 *vb = reinterpret_cast<const uint4 *>(wb + head);
+            for (int v = lane; v < nvec; v += 32) {
+                const uint4 q = __ldg(vb + v);
+                part += (ACC)cvt_x<XF32>(q.x) + (ACC)cvt_x<XF32>(q.y) + (ACC)cvt_x<XF32>(q.z) +
+                        (ACC)cvt_x<XF32>(q.w);
+            }
+            const int tail = head + 4 * nvec + lane;
+            if (tail < N) part += (ACC)cvt_x<XF32>(__ldg(wb + tail));
         }
-        const int tail = head + 4 * nvec + lane;
-        if (tail < N) part += (ACC)cvt_x<XF32>(__ldg(wb + tail));
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
         carryW = part;
@@ -350,11 +370,14 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
         __syncwarp();
         // ---- outputs of the step that lags L behind (a sparse re-computation wants the block's own steps only) ----
         if (!sparse || tb >= tb_out) {
-            const bool interior = (tb - L >= 0) && (tb - L + WS <= seglen) &&
-                                  (tb + WS - 1 <= nrem);      // every output valid, every boxcar complete
+            // every boxcar of this step's outputs is complete (only steps at the end of a ROW are not); outputs before
+            // the segment (first step: the lag) or past it (last step) are masked per group of four
+            const bool complete = tb + WS - 1 <= nrem;
             constexpr bool store = STORE;
             const bool slow = GUARD && (slowbits & P.guard_hist);
-            if (MIRROR && interior && !slow && P.vec_out) {
+            if (MIRROR && complete && !slow && P.vec_out) {
+                const int oa = tb - L + 4 * lane, ob4 = oa + 4 * 32;
+                const bool va = oa >= 0 && oa + 4 <= seglen, vb = ob4 >= 0 && ob4 + 4 <= seglen;
                 // ---- vector path: lane = 2 x 4 consecutive outputs; ring read and z written 128 bits at a time ----
                 int s0 = rslot + 4 * lane, s1 = s0 + 4 * 32;
                 if (s0 >= RING) s0 -= RING;
@@ -367,9 +390,11 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
 #pragma unroll 1
                 for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll 1
-                    for (int iw = iw0; iw < iw1; ++iw) {
+                    // (the host lists the widths that are multiples of 4 first: wl[0 .. n4), then the others)
+                    for (int q = pass ? P.n4 : 0; q < (pass ? P.nw : P.n4); ++q) {
+                        const int iw = P.wl[q];
+                        if (sparse && iw != iw0) continue;
                         const int w = P.w[iw], wa = w & 3, wo = w - wa;
-                        if ((wa != 0) != (pass != 0)) continue;
                         float fa[4], fb[4];     // float32 of the exact integer numerators
                         const uint4 a0v = *reinterpret_cast<const uint4 *>(ring + s0 + wo);
                         const uint4 b0v = *reinterpret_cast<const uint4 *>(ring + s1 + wo);
@@ -391,18 +416,24 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
                         }
                         if (RMS) {
                             float2 st = racc[iw * 32 + lane];
+                            if (va) {
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) { st.x = __fmaf_rn(fa[i], fa[i], st.x); st.y = fmaxf(st.y, fa[i]); }
+                                for (int i = 0; i < 4; ++i) { st.x = __fmaf_rn(fa[i], fa[i], st.x); st.y = fmaxf(st.y, fa[i]); }
+                            }
+                            if (vb) {
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) { st.x = __fmaf_rn(fb[i], fb[i], st.x); st.y = fmaxf(st.y, fb[i]); }
+                                for (int i = 0; i < 4; ++i) { st.x = __fmaf_rn(fb[i], fb[i], st.x); st.y = fmaxf(st.y, fb[i]); }
+                            }
                             racc[iw * 32 + lane] = st;
                         }
                         if (store) {
                             const float scl = P.scale[iw];
                             float *zp = zp0 + (long long)iw * P.plane;
-                            __stcs(reinterpret_cast<float4 *>(zp), make_float4(fa[0] * scl, fa[1] * scl, fa[2] * scl, fa[3] * scl));
-                            __stcs(reinterpret_cast<float4 *>(zp + 4 * 32),
-                                   make_float4(fb[0] * scl, fb[1] * scl, fb[2] * scl, fb[3] * scl));
+                            if (va)
+                                __stcs(reinterpret_cast<float4 *>(zp), make_float4(fa[0] * scl, fa[1] * scl, fa[2] * scl, fa[3] * scl));
+                            if (vb)
+                                __stcs(reinterpret_cast<float4 *>(zp + 4 * 32),
+                                       make_float4(fb[0] * scl, fb[1] * scl, fb[2] * scl, fb[3] * scl));
                         }
                     }
                 }
@@ -486,6 +517,72 @@ __global__ void __launch_bounds__(NT, MF_MINB) mf_warp_kernel(const MFParams P)
     }
 }
 
+// prefix[row][k] = sum of x[row][0 .. min(k * PB, n)), k = 0 .. pnb (64-bit: exact; 32-bit users take it mod 2^32).
+// One CTA of 8 warps per row; a warp sums one block of PB = 256 samples at a time (8 consecutive samples per lane,
+// 128-bit loads where the row allows), the block sums of up to 2048 blocks are gathered in shared memory and
+// scanned by the CTA, with a carry across such chunks for very long rows.  Reads x once: HBM-bound.
+template <bool XF32>
+__global__ void __launch_bounds__(256) mf_prefix_kernel(const uint32_t *__restrict__ x, long long n, int pnb,
+                                                        unsigned long long *__restrict__ prefix, int vec, long long row0)
+{
+    constexpr int CHUNK = 2048;
+    __shared__ unsigned long long sb[CHUNK];
+    __shared__ unsigned long long swarp[8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t *xr = x + (size_t)(row0 + blockIdx.x) * (size_t)n;
+    unsigned long long *pr = prefix + (size_t)(row0 + blockIdx.x) * (size_t)(pnb + 1);
+    unsigned long long carry = 0;
+    for (int k0 = 0; k0 < pnb; k0 += CHUNK) {
+        const int nk = pnb - k0 < CHUNK ? pnb - k0 : CHUNK;
+        for (int k = warp; k < nk; k += 8) {
+            const long long t = (long long)(k0 + k) * PB + lane * 8;
+            unsigned long long v = 0;
+            if (vec && t + 8 <= n) {
+                const uint4 a = __ldg(reinterpret_cast<const uint4 *>(xr + t)), b = __ldg(reinterpret_cast<const uint4 *>(xr + t) + 1);
+                v = (unsigned long long)cvt_x<XF32>(a.x) + cvt_x<XF32>(a.y) + cvt_x<XF32>(a.z) + cvt_x<XF32>(a.w) +
+                    cvt_x<XF32>(b.x) + cvt_x<XF32>(b.y) + cvt_x<XF32>(b.z) + cvt_x<XF32>(b.w);
+            } else {
+                for (int i = 0; i < 8; ++i)
+                    if (t + i < n) v += cvt_x<XF32>(__ldg(xr + t + i));
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) sb[k] = v;
+        }
+        __syncthreads();
+        // exclusive scan of sb[0 .. nk): 8 consecutive entries per thread
+        unsigned long long loc[8], run = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int k = threadIdx.x * 8 + i;
+            loc[i] = run;
+            run += k < nk ? sb[k] : 0ull;
+        }
+        unsigned long long inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) swarp[warp] = inc;
+        __syncthreads();
+        unsigned long long base = carry, tot = 0;
+        for (int q = 0; q < 8; ++q) {
+            if (q < warp) base += swarp[q];
+            tot += swarp[q];
+        }
+        base += inc - run;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int k = threadIdx.x * 8 + i;
+            if (k < nk) pr[k0 + k] = base + loc[i];
+        }
+        carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) pr[pnb] = carry;
+}
+
 // rms[s] = fl32( sqrt( (sum of the nseg partials of series s, in order) / n ) )
 __global__ void mf_rms_finish_kernel(const double *__restrict__ partial, long long nseries, int nseg, long long n,
                                      float *__restrict__ rms)
@@ -497,33 +594,29 @@ __global__ void mf_rms_finish_kernel(const double *__restrict__ partial, long lo
     rms[s] = (float)sqrt(t / (double)n);
 }
 
-// Samples per work item (one warp): a multiple of E.  A longer segment amortises the item's start-up (the window
-// sum of N samples, ~ a quarter of a segment's own loads at N = 31 251) but leaves fewer items than resident warps,
-// or an unlucky tail of a second wave; pick the candidate with the least (waves x cost per item).  Depends only on
-// (nrows, nsamps, SMs of the current device) so that the workspace size can be computed ahead of the call.
 }  // namespace
 
+// Samples per work item (one warp): a multiple of E.  With the per-row prefix sums the start of an item is cheap, so
+// segments are short: the items of a row then run at the same time (consecutive items = consecutive segments of a
+// row), the rows in flight -- resident warps / segments per row -- fit L2, and the x[t - R - 1] and x[t] streams are
+// served from the lines the x[t + R] stream brought in (profiles/r2_matched_filter.md).  Depends only on nsamps, so
+// that the workspace size can be computed ahead of the call.
+#ifndef MF_WSEG
+#define MF_WSEG (2 * E)
+#endif
 long long mf_warp_segment(long long nrows, long long nsamps)
 {
-    int sms = 148, dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    else cudaGetLastError();
-    const long long capacity = (long long)sms * MF_MINB * WPB;     // resident warps
-    long long best_seg = E;
-    double best = 1e300;
-    for (long long seg = E; seg <= 16ll * E; seg += E) {
-        const long long nseg = (nsamps + seg - 1) / seg;
-        const long long items = nrows * nseg;
-        const long long waves = (items + capacity - 1) / capacity;
-        const long long s = seg < nsamps ? seg : nsamps;
-        const double cost = (double)waves * ((double)s + 4096.0);
-        if (cost < best * 0.999) {
-            best = cost;
-            best_seg = seg;
-        }
-        if (seg >= nsamps) break;
-    }
-    return best_seg;
+    (void)nrows;
+    long long seg = MF_WSEG;
+    if (seg > nsamps) seg = (nsamps + E - 1) / E * E;
+    return seg;
+}
+
+size_t mf_warp_workspace_bytes(long long nrows, long long nsamps, int nwidths)
+{
+    const long long seg = mf_warp_segment(nrows, nsamps), nseg = (nsamps + seg - 1) / seg;
+    const long long pnb = (nsamps + PB - 1) / PB;
+    return (size_t)nwidths * (size_t)nrows * (size_t)nseg * sizeof(double) + (size_t)nrows * (size_t)(pnb + 1) * 8;
 }
 
 // sparse_list / sparse_count / zc / max_blocks: the sparse re-computation of dedisp_search_events (one CTA per listed
@@ -534,6 +627,10 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
                      int *blockmax_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                      const int2 *sparse_list, const int *sparse_count, float *zc, long long max_blocks)
 {
+    // workspace (dense with rms_dev, and sparse): [nwidths * nrows * nseg doubles: partial sums of z^2][nrows * (pnb + 1)
+    // uint64: per-row prefix sums of x]; mf_warp_workspace_bytes().  The sparse pass re-uses the prefix sums the RMS
+    // pass of the same dedisp_search_events call left there.  Without a workspace (workspace_dev null) every work item
+    // sums its first window sample by sample.
     const bool sparse = sparse_list != nullptr;
     if (!x_dev || !widths_host || nrows < 1 || nsamps < 1 || radius < 0) return DEDISP_ERR_INVALID_ARG;
     if (sparse ? (!sparse_count || !zc || max_blocks < 1 || max_blocks > 0x7fffffffll || z_dev || rms_dev)
@@ -562,6 +659,12 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
         if (w > P.wmax) P.wmax = w;
     }
     for (int i = nwidths; i < MAXW; ++i) { P.w[i] = 1; P.scale[i] = 0.f; }
+    P.n4 = 0;
+    for (int i = 0; i < nwidths; ++i)
+        if (P.w[i] % 4 == 0) P.wl[P.n4++] = i;
+    for (int i = 0, q = P.n4; i < nwidths; ++i)
+        if (P.w[i] % 4 != 0) P.wl[q++] = i;
+    for (int i = nwidths; i < MAXW; ++i) P.wl[i] = 0;
     P.lag = P.wmax;       // (the hint geometry of dedisp_matched_filter_hint_blocks: outputs trail by the largest width)
     const int ring = (WS + P.lag + 8 + 7) & ~7;
     P.ring = ring;
@@ -574,6 +677,7 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
     const long long nseg = (nsamps + seg - 1) / seg;
     P.nseg = (int)nseg;
     P.nitems = nrows * nseg;
+    P.row0 = 0;
     P.plane = sparse ? 0 : nrows * nsamps;
     if (nrows * nseg > 0x7fffffffll) return DEDISP_ERR_INVALID_ARG;
     // |boxcar numerator| <= wmax * N * x_max must fit the signed accumulator
@@ -592,6 +696,12 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
     const size_t accb = wide ? 8 : 4;
     const bool rms = rms_dev != nullptr;
     P.partial = (double *)workspace_dev;
+    const long long pnb = (nsamps + PB - 1) / PB;
+    const size_t partial_bytes = (size_t)nwidths * (size_t)nrows * (size_t)nseg * sizeof(double);
+    const bool have_ws = workspace_dev && ((uintptr_t)workspace_dev & 7u) == 0 &&
+                         workspace_bytes >= partial_bytes + (size_t)nrows * (size_t)(pnb + 1) * 8;
+    P.prefix = have_ws ? (const unsigned long long *)((const uint8_t *)workspace_dev + partial_bytes) : nullptr;
+    P.pnb = (int)pnb;
     P.blockmax = blockmax_dev;
     P.nblk = (int)((nsamps + P.lag + E - 1) / E);
     P.sparse_list = sparse_list;
@@ -600,7 +710,7 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
     if (blockmax_dev && (!rms || ((uintptr_t)blockmax_dev & 3u))) return DEDISP_ERR_INVALID_ARG;
     if (rms) {
         if (!workspace_dev || ((uintptr_t)workspace_dev & 7u) || ((uintptr_t)rms_dev & 3u) ||
-            workspace_bytes < (size_t)nwidths * (size_t)nrows * (size_t)nseg * sizeof(double))
+            workspace_bytes < partial_bytes)
             return DEDISP_ERR_INVALID_ARG;
     }
     const size_t warp_smem = ((wide ? 1 : 2) * (size_t)ring * accb + (rms ? (size_t)nwidths * 32 * 16 : 0) + 15) &
@@ -609,11 +719,26 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
     const size_t smem = WPB * warp_smem;
     if (smem > 227 * 1024) return DEDISP_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const dim3 grid((unsigned)(((sparse ? max_blocks : nrows * nseg) + WPB - 1) / WPB)), block(NT);
+    if (nrows > 0x7fffffffll) return DEDISP_ERR_INVALID_ARG;
     cudaError_t e = cudaSuccess;
     if (blockmax_dev &&   // every byte 0x80: below the image of any finite float
         cudaMemsetAsync(blockmax_dev, 0x80, (size_t)nwidths * (size_t)nrows * (size_t)P.nblk * 4, s) != cudaSuccess)
         return DEDISP_ERR_CUDA;
+    // Dense passes with prefix sums can run in blocks of rows whose x fits L2 (MF_L2_ROW_BYTES: the prefix kernel of a
+    // block brings its rows in, the filter kernel of the block then reads them from L2).  Measured on the gulp it
+    // LOSES (search step 0.495 ms in one launch, 0.616 / 0.666 / 0.838 ms with 110 / 80 / 40 MB blocks): the filter
+    // kernel is bound by instruction issue and latency per work item, not by DRAM, and every launch pays its own
+    // ramp and tail.  The default is therefore one launch; the knob stays for other shapes.
+#ifndef MF_L2_ROW_BYTES
+#define MF_L2_ROW_BYTES (1ll << 50)
+#endif
+    long long rows_per_launch = nrows;
+    if (P.prefix && !sparse) {
+        rows_per_launch = MF_L2_ROW_BYTES / (nsamps * 4);
+        if (rows_per_launch < 64) rows_per_launch = 64;
+        if (rows_per_launch > nrows) rows_per_launch = nrows;
+    }
+    const bool f32 = (x_dtype == DEDISP_OUT_F32);
 #define MF_LAUNCH1(ACC, F, G, R, ST)                                                                  \
     do {                                                                                             \
         e = cudaFuncSetAttribute(mf_warp_kernel<ACC, F, G, R, ST>,                            \
@@ -626,22 +751,38 @@ dedisp_status mf_warp_run(const void *x_dev, dedisp_out_dtype x_dtype, long long
         else if (rms) MF_LAUNCH1(ACC, F, G, true, false);  \
         else MF_LAUNCH1(ACC, F, G, false, true);           \
     } while (0)
-    const bool f32 = (x_dtype == DEDISP_OUT_F32);
-    if (wide) {
-        if (f32) MF_LAUNCH(unsigned long long, true, false);
-        else MF_LAUNCH(unsigned long long, false, false);
-    } else if (guard) {
-        if (f32) MF_LAUNCH(uint32_t, true, true);
-        else MF_LAUNCH(uint32_t, false, true);
-    } else {
-        if (f32) MF_LAUNCH(uint32_t, true, false);
-        else MF_LAUNCH(uint32_t, false, false);
+    for (long long r0 = 0; r0 < nrows && e == cudaSuccess; r0 += rows_per_launch) {
+        const long long nr = nrows - r0 < rows_per_launch ? nrows - r0 : rows_per_launch;
+        if (P.prefix && !sparse) {
+            // per-row prefix sums of x for the cheap start of every work item (the sparse pass re-uses them)
+            unsigned long long *pw = const_cast<unsigned long long *>(P.prefix);
+            const int pvec = rows16 && ((uintptr_t)x_dev & 15u) == 0;
+            if (f32)
+                mf_prefix_kernel<true><<<(unsigned)nr, 256, 0, s>>>((const uint32_t *)x_dev, nsamps, P.pnb, pw, pvec, r0);
+            else
+                mf_prefix_kernel<false><<<(unsigned)nr, 256, 0, s>>>((const uint32_t *)x_dev, nsamps, P.pnb, pw, pvec, r0);
+            if (cudaGetLastError() != cudaSuccess) return DEDISP_ERR_CUDA;
+            ++g_launch_count;
+        }
+        P.row0 = r0;
+        P.nitems = nr * nseg;
+        const dim3 grid((unsigned)(((sparse ? max_blocks : nr * nseg) + WPB - 1) / WPB)), block(NT);
+        if (wide) {
+            if (f32) MF_LAUNCH(unsigned long long, true, false);
+            else MF_LAUNCH(unsigned long long, false, false);
+        } else if (guard) {
+            if (f32) MF_LAUNCH(uint32_t, true, true);
+            else MF_LAUNCH(uint32_t, false, true);
+        } else {
+            if (f32) MF_LAUNCH(uint32_t, true, false);
+            else MF_LAUNCH(uint32_t, false, false);
+        }
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) ++g_launch_count;
     }
 #undef MF_LAUNCH
 #undef MF_LAUNCH1
-    if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return DEDISP_ERR_CUDA;
-    ++g_launch_count;
     if (rms) {
         const long long nseries = (long long)nwidths * nrows;
         mf_rms_finish_kernel<<<(unsigned)((nseries + 255) / 256), 256, 0, s>>>(P.partial, nseries, P.nseg, nsamps, rms_dev);

@@ -547,7 +547,8 @@ dedisp_status dedisp_search_events(const void *x_dev, dedisp_out_dtype x_dtype, 
     clamp_block_count_kernel<<<1, 1, 0, s>>>(count, (int)max_blocks, count_dev);
     g_launch_count += 2;
     if (cudaGetLastError() != cudaSuccess) return DEDISP_ERR_CUDA;
-    st = mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, nullptr, nullptr, nullptr, nullptr, 0,
+    st = mf_run(x_dev, x_dtype, nrows, nsamps, radius, widths_host, nwidths, x_max, nullptr, nullptr, nullptr,
+                ws + L.off_partial, L.off_blockmax - L.off_partial,      // (the prefix sums of x pass 1 left there)
                 cuda_stream, list, count, zc, max_blocks);
     if (st != DEDISP_OK) return st;
     // pass 3: sigma-cut and grouping over the compact z (chunks the block maxima rule out are skipped as before)
