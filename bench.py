@@ -866,8 +866,13 @@ def run_reference(args) -> None:
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
            "data": "synthetic",
+           # the same config block as the CUDA arm prints (the bounded sample is described under cpu_baseline)
            "config": {"workload": w.name, "nchans": w.nchans, "ndm": w.ndm, "nsamps_out": w.nsamps_out,
-                      "nbits": w.nbits, "sample": sample},
+                      "nbits": w.nbits, "tscrunch": 1, "nbeams_per_gpu": w.nbeams, "out_dtype": w.out_dtype,
+                      "max_delay": md, "l2": "256 MiB flush buffer zeroed between timed iterations",
+                      "parallelism": f"replicas x{int(os.environ.get('WORLD_SIZE', '1'))} (one seeded beam set per GPU, "
+                                     "no collective)"},
+           "sample": sample,
            "cpu_baseline": {"value": value, "unit": "DM-trial-samples/s", "cores": used,
                             "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": "DM-trial-samples/s", "h2d_bytes_per_step": 0,
