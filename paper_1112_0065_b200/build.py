@@ -2,10 +2,12 @@
 
     python -m paper_1112_0065_b200.build [--force] [--verbose]
 
-Every translation unit is compiled to an object file (in parallel, re-compiled only when it or a
-header changed) and the objects are linked into the shared library.  The object cache lives in the
-system temp directory (DEDISP_B200_OBJDIR overrides it): it is a few hundred MB and must not travel
-with the source tree.
+Every translation unit is compiled to an object file (in parallel) and the objects are linked into
+the shared library.  Objects are cached by CONTENT -- the file name carries a hash of the source, of
+every header and of the flags -- so a cache left behind by another checkout or an older snapshot
+can never be linked by mistake, whatever the file times say.  The cache lives in the system temp
+directory (DEDISP_B200_OBJDIR overrides it): it is a few hundred MB and must not travel with the
+source tree.
 """
 from __future__ import annotations
 
@@ -51,8 +53,13 @@ def stale(lib: Path | None = None) -> bool:
 
 
 def _compile(src: Path, obj: Path, defs: list[str]) -> tuple[int, str]:
-    cmd = [_nvcc(), *NVCC_FLAGS, *[f"-D{d}" for d in defs], f"-I{INCLUDE}", f"-I{CSRC}", "-c", "-o", str(obj), str(src)]
+    tmp = obj.with_suffix(f".tmp{os.getpid()}.o")
+    cmd = [_nvcc(), *NVCC_FLAGS, *[f"-D{d}" for d in defs], f"-I{INCLUDE}", f"-I{CSRC}", "-c", "-o", str(tmp), str(src)]
     r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode == 0:
+        os.replace(tmp, obj)
+    else:
+        tmp.unlink(missing_ok=True)
     return r.returncode, r.stdout + r.stderr
 
 
@@ -64,14 +71,20 @@ def build(force: bool = False, verbose: bool = False, defs: list[str] | None = N
     sources = list(sources or SOURCES)
     if not force and not defs and not out and sources == SOURCES and not stale():
         return LIB
-    tag = hashlib.sha1(" ".join(defs).encode()).hexdigest()[:8] if defs else "default"
-    objdir = OBJDIR / tag
+    objdir = OBJDIR
     objdir.mkdir(parents=True, exist_ok=True)
-    hdr_t = max(h.stat().st_mtime for h in _headers())
-    jobs = []
+    hh = hashlib.sha1()
+    for h in _headers():
+        hh.update(h.name.encode() + b"\0" + h.read_bytes())
+    hh.update(" ".join(NVCC_FLAGS + sorted(defs)).encode())
+    common = hh.digest()
+    objs, jobs = {}, []
     for s in sources:
-        src, obj = CSRC / s, objdir / (Path(s).stem + ".o")
-        if force or not obj.exists() or obj.stat().st_mtime < max(src.stat().st_mtime, hdr_t):
+        src = CSRC / s
+        key = hashlib.sha1(common + src.read_bytes()).hexdigest()[:16]
+        obj = objdir / f"{Path(s).stem}.{key}.o"
+        objs[s] = obj
+        if force or not obj.exists():
             jobs.append((src, obj))
     logs = []
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
@@ -82,9 +95,13 @@ def build(force: bool = False, verbose: bool = False, defs: list[str] | None = N
             if rc != 0:
                 obj.unlink(missing_ok=True)
                 raise RuntimeError(f"nvcc failed compiling {src.name}")
+    for src, obj in jobs:      # older objects of the same translation unit are of no use any more
+        for old in objdir.glob(f"{src.stem}.*.o"):
+            if old != obj and not force and old.stat().st_mtime < obj.stat().st_mtime - 6 * 3600:
+                old.unlink(missing_ok=True)
     tmp = target.with_suffix(f".tmp{os.getpid()}.so")
     cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC", "-o", str(tmp)] + \
-          [str(objdir / (Path(s).stem + ".o")) for s in sources]
+          [str(objs[s]) for s in sources]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
