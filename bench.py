@@ -176,7 +176,8 @@ def ncu_traffic_bytes(config: str):
     return ncu_traffic(config)[0]
 
 
-KERNEL_NAMES = {1: "direct_kernel", 2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows"}
+KERNEL_NAMES = {1: "direct_kernel", 2: "bitslice_dedisperse", 3: "bitslice_dedisperse on pair rows",
+                4: "bitslice_dedisperse on quad rows"}
 # ALU-pipe (LOP3 / SHF / LEA: 64 lanes per clock and SM) instructions per addition of the dominant kernel's hot loop,
 # counted on the SASS / the ncu source page: (kernel, nbits) -> (lane-instructions per add, where it was counted)
 ALU_PIPE_INSTR_PER_ADD = {
@@ -196,7 +197,7 @@ def measure_dedisperse(torch, dd, w, k, kernel, steps, warmup, rank, world, dev,
     dd.dedisp_set_dm_list(plan, list(w.dms()))
     set_dm_ms = (time.perf_counter() - t0) * 1e3
     dd.dedisp_set_kernel(plan, {"auto": dd.DEDISP_KERNEL_AUTO, "bitslice": dd.DEDISP_KERNEL_BITSLICE,
-                                "pairs": dd.DEDISP_KERNEL_PAIRS}[kernel])
+                                "pairs": dd.DEDISP_KERNEL_PAIRS, "quads": dd.DEDISP_KERNEL_QUADS}[kernel])
     md = dd.dedisp_get_max_delay(plan)
     kw = {}
     if w.kind == "gauss2_pulses":   # pulse sweeps from the product's own delay builder
@@ -891,7 +892,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false",
                     help="skip the per_config block (the other four BASELINE configs, timed in the default run)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "bitslice", "pairs"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "bitslice", "pairs", "quads"],
                     help="A/B: force the plain tiled kernel or its pair-row variant (dedisp_set_kernel)")
     ap.add_argument("--search-mode", default="fused", choices=["fused", "dense"],
                     help="--op search: dedisp_search_events (no z written; default) or the dense two-call chain")

@@ -92,13 +92,17 @@ typedef enum {
     DEDISP_KERNEL_AUTO = 0,     /* bit-sliced tiled kernel when the plan fits it, else DIRECT */
     DEDISP_KERNEL_DIRECT = 1,   /* one thread per output group, reads packed input from global */
     DEDISP_KERNEL_BITSLICE = 2, /* TMA-staged (DM x time) tiles, bit-plane carry-save adders */
-    DEDISP_KERNEL_PAIRS = 3     /* the same tiled kernel on pair rows: in[2p][t] + in[2p+1][t + delta] is formed
+    DEDISP_KERNEL_PAIRS = 3,    /* the same tiled kernel on pair rows: in[2p][t] + in[2p+1][t + delta] is formed
                                    once per delay difference delta of the DM list (nbits + 1 bit planes) and the tiles
                                    add nchans/2 such rows -- the identical integer sum, re-associated.  2-, 4-
                                    and 8-bit samples; AUTO picks it when the plan fits (see dedisp_get_last_kernel)
                                    and falls back to the plain tiled kernel when the scratch for the rows
                                    cannot be allocated (forced PAIRS then returns DEDISP_ERR_ALLOC);
                                    BITSLICE forces the plain tiled kernel */
+    DEDISP_KERNEL_QUADS = 4     /* ... and on quad rows: the sum of FOUR adjacent channels formed once per triple of delay
+                                   differences of the DM list (nbits + 2 planes), nchans/4 rows per output.  8-bit samples
+                                   only; needs up to tens of GB of scratch for long DM lists (8-bit wideband config:
+                                   17.7 GB); AUTO takes it when it pays and fits, else pair rows, else planes */
 } dedisp_kernel;
 
 /* Create a plan for nchans channels, sample time dt_s (s), channel 0 at f_top_mhz,
@@ -215,9 +219,9 @@ size_t dedisp_get_in_row_stride_bytes(dedisp_plan plan, long long nsamps_out, in
 dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out);
 
 /* Force a kernel variant for subsequent executes (default DEDISP_KERNEL_AUTO).
- * Forcing BITSLICE or PAIRS on a plan it cannot serve makes execute return INVALID_ARG. */
+ * Forcing BITSLICE, PAIRS or QUADS on a plan it cannot serve makes execute return INVALID_ARG. */
 dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which);
-/* Variant the last execute on this plan used (DEDISP_KERNEL_DIRECT/BITSLICE/PAIRS), 0 if none. */
+/* Variant the last execute on this plan used (DEDISP_KERNEL_DIRECT/BITSLICE/PAIRS/QUADS), 0 if none. */
 int dedisp_get_last_kernel(dedisp_plan plan);
 
 /* Per-kernel device timing (for the bench's roofline line).  When enabled, execute

@@ -31,6 +31,7 @@ DEDISP_KERNEL_AUTO = 0
 DEDISP_KERNEL_DIRECT = 1
 DEDISP_KERNEL_BITSLICE = 2
 DEDISP_KERNEL_PAIRS = 3
+DEDISP_KERNEL_QUADS = 4
 
 # every symbol include/dedisp.h declares: (restype, argtypes)
 _vp, _i, _ll, _sz, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_size_t, ctypes.c_double

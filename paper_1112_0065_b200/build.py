@@ -28,7 +28,7 @@ OBJDIR = Path(os.environ.get("DEDISP_B200_OBJDIR") or
 SOURCES = ["dedisp_api.cu", "delay_table.cu", "direct_kernel.cu", "bitslice_prepare.cu", "bitslice_kernel.cu",
            "bitslice_inst_cfg1.cu", "bitslice_inst_cfg2.cu", "bitslice_inst_cfg3.cu", "bitslice_inst_cfg4.cu",
            "bitslice_inst_cfg5.cu", "bitslice_inst_cfg6.cu", "bitslice_inst_cfg8.cu", "bitslice_inst_pairs2.cu",
-           "bitslice_inst_pairs4.cu", "bitslice_inst_pairs8.cu", "pair_rows.cu", "static_scratch.cu", "matched_filter.cu", "matched_filter_warp.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
+           "bitslice_inst_pairs4.cu", "bitslice_inst_pairs8.cu", "bitslice_inst_quads8.cu", "pair_rows.cu", "quad_rows.cu", "static_scratch.cu", "matched_filter.cu", "matched_filter_warp.cu", "peak_finding.cu", "rfi_mask.cu", "time_major.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=false", "-Xptxas", "-v"]
 

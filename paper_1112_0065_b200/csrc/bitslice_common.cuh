@@ -98,8 +98,14 @@ struct Cfg {
     static constexpr int VSKEW = BS_VSKEW_UNIT * (NV_ - 1);
     static __host__ __device__ constexpr int vskew(int v) { return BS_VSKEW_UNIT * v; }
 #else
-    static constexpr int VSKEW = NV_ > 1 ? 16 : 0;
-    static __host__ __device__ constexpr int vskew(int v) { return (v & 1) * VSKEW; }
+    // up to 3 variants (pair rows): odd variants 16 banks away.  More (quad rows, NV = 7): 0, 16, 8, 24, 4, 20, 12
+    // banks -- any two variants at least 4 banks apart, so lanes at the same or a neighbouring window offset in
+    // different variants never share a bank (profiles/r2_wide8.md)
+    static constexpr int VSKEW = NV_ > 3 ? 28 : NV_ > 1 ? 16 : 0;
+    static __host__ __device__ constexpr int vskew(int v)
+    {
+        return NV_ > 3 ? ((v & 1) * 16 + ((v >> 1) & 1) * 8 + ((v >> 2) & 1) * 4) : (v & 1) * VSKEW;
+    }
 #endif
     template <int WIN> static constexpr int plane_words() { return WIN + VSKEW; }
     template <int WIN> static constexpr int vslot_words()
@@ -218,6 +224,15 @@ using Cfg5P = Cfg<5, BS5P_NW, 4, BS5P_TREE_K, BS5P_NSTAGE, 16, 96, 96, BS5P_NSPL
 #endif
 using Cfg9P = Cfg<9, BS9P_NW, BS9P_W, BS9P_TREE_K, BS9P_NSTAGE, 20, BS9P_WIN, BS9P_WIN, BS9P_NSPLIT, 3>;
 
+// Quad rows (quad_rows.cu): a virtual channel is the exact sum of FOUR adjacent 8-bit channels at fixed delay
+// differences (d1, d2, d3) to the first of them, one 10-plane row per difference triple that occurs in the DM list;
+// the trials of a group use at most NV = 7 distinct triples of a quad (else the plan stays on the pair rows).  Four
+// quads (16 channels) per stage, one plane per adder tree; window 72 + 28 words of skew per plane line.
+#ifndef BS10Q_NW
+#define BS10Q_NW 11
+#endif
+using Cfg10Q = Cfg<10, BS10Q_NW, 4, 1, 2, 20, 72, 72, 10, 7>;
+
 constexpr int NGEOM = 9;                                   // geometries are indexed by plane count 1..8
 constexpr int geom_index(int nplanes) { return nplanes; }
 // planes needed for the block sums of k samples of nbits bits, rounded up to a built geometry (0: none)
@@ -253,6 +268,10 @@ struct BitsliceParams {
     // (vinfo & 0x0fffffff) .. + (vinfo >> 28) of it; rel carries the lane's variant in its byte offset
     const uint32_t *vinfo;     // [ngroups][nchans_pad]
     int vrows;                 // rows per beam
+    // quad rows (Cfg::NV > 3): the rows a slot stages are listed explicitly, vlist[(group * nchans_pad + slot) * NV + v]
+    // = (row of variant v or -1, first word of its box for tile 0): every variant has a window start of its own, placed
+    // so that the lanes of the group fall into different shared-memory banks (quad_rows.cu)
+    const int2 *vlist;
     // self-checks (library built with -DDEDISP_CHECKS; see dedisp_debug_check_errors): failure counters in device
     // memory and the extent of the scratch the producer may read
     unsigned long long *check_errors;   // [DEDISP_NCHECK] or nullptr

@@ -21,6 +21,9 @@ using namespace bs;
 #ifndef PAIRS8_AUTO
 #define PAIRS8_AUTO 1          // 8-bit pair rows (wide8: 59.9 -> 41.2 ms per step; the same break-even holds)
 #endif
+#ifndef QUADS8_AUTO
+#define QUADS8_AUTO 1
+#endif
 #ifndef PAIRS_MAX_BYTES
 #define PAIRS_MAX_BYTES (24ull << 30)
 #endif
@@ -50,6 +53,25 @@ dedisp_status bitslice_execute(dedisp_plan plan, int nbeams, long long nsamps_ou
                                out_beam_stride, out_f32, s, rg, reserve_only};
     const bool pairs_fit = (nbits == 2 || nbits == 4 || nbits == 8) && tscrunch == 1 && PT.usable;
     if (plan->want == DEDISP_KERNEL_PAIRS && !pairs_fit) return DEDISP_ERR_INVALID_ARG;
+    // quad rows (8-bit samples at full time resolution): the step after the pair rows.  AUTO takes them when a (DM
+    // group, quad) amortises its share of the rows -- measured on B200 (profiles/r2_wide8.md) a quad slot of a DM group
+    // is ~240 ns x SMs cheaper than its two pair slots and a row costs ~60 ns to build, break-even near 4 rows per
+    // (group, quad): taken at <= 3 -- and the rows of all beams stay below PAIRS_MAX_BYTES of scratch.
+    const QuadTables &QT = plan->quads8;
+    const bool quads_fit = nbits == 8 && tscrunch == 1 && QT.usable;
+    if (plan->want == DEDISP_KERNEL_QUADS && !quads_fit) return DEDISP_ERR_INVALID_ARG;
+    bool quads_pay = false;
+    if (quads_fit && plan->want == DEDISP_KERNEL_AUTO && (rg.prepass || plan->bitslice_kind == DEDISP_KERNEL_QUADS)) {
+        const long long ntiles = (nsamps_out + Cfg10Q::TILE_SAMPS - 1) / Cfg10Q::TILE_SAMPS;
+        const unsigned long long bytes = (unsigned long long)QT.nrows * Cfg10Q::NB * 4ull * (unsigned long long)nbeams *
+                                         (unsigned long long)((plan->max_delay >> 5) + ntiles * Cfg10Q::TILE_WORDS + 128);
+        quads_pay = (long long)QT.nrows <= 3ll * G.ngroups * QT.nquads_pad && bytes <= PAIRS_MAX_BYTES && QUADS8_AUTO;
+    }
+    if (quads_fit && (plan->want == DEDISP_KERNEL_QUADS || quads_pay)) {
+        plan->bitslice_kind = DEDISP_KERNEL_QUADS;
+        const dedisp_status st = bitslice_run_quads8(call);
+        if (st != DEDISP_ERR_ALLOC || plan->want != DEDISP_KERNEL_AUTO) return st;      // (else: pair rows, then planes)
+    }
     bool pairs_pay = false;
     // (a DM-group range that continues an execute -- no pre-pass of its own -- stays on what the first range ran)
     if (pairs_fit && plan->want == DEDISP_KERNEL_AUTO && (rg.prepass || plan->bitslice_kind == DEDISP_KERNEL_PAIRS)) {

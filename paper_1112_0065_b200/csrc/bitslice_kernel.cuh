@@ -377,6 +377,25 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                     // pair rows: one box (NB plane lines x PLW words) per (channel slot, variant the group uses)
                     static_assert(C::NV == 1 || CH <= 32, "one lane per channel slot counts the variants");
                     const size_t c0 = grow + (size_t)(P.chunk0 + chunk) * CH;
+                    if constexpr (C::NV > 3) {
+                        // quad rows: lane = (slot, variant); the row of each variant is listed explicitly
+                        static_assert(C::NV <= 3 || CH * C::NV <= 32, "one lane per (slot, variant)");
+                        const int cl = lane / C::NV, v = lane % C::NV;
+                        const int2 vr = lane < CH * C::NV ? P.vlist[(c0 + cl) * C::NV + v] : make_int2(-1, 0);
+                        const int row = vr.x;
+                        const int nbox = __reduce_add_sync(0xffffffffu, row >= 0 ? 1 : 0);
+                        if (lane == 0) mbar_expect_tx(fb, S::REL_BYTES + nbox * S::BOX_BYTES);
+                        __syncwarp();
+                        if (row >= 0) {
+                            // (the box may start before the row or run past its end: those words are zero-filled and
+                            // never read -- the lanes' own words lie inside, quad_rows.cu::prepare_tables)
+                            const int x = vr.y + tile * C::TILE_WORDS;
+                            const int y = (beam * P.vrows + row) * NB;
+                            BS_CHECK(x > -S::PLW && x < P.row_pitch && y >= 0 &&
+                                         (unsigned long long)(y + NB) * P.row_pitch <= P.scratch_words, CHK_TMA_SRC);
+                            tma_box_g2s(sb + cl * S::CPITCH + v * S::VSLOT, &tmap, x, y, fb);
+                        }
+                    } else {
                     const int mine = lane < CH ? (int)(P.vinfo[c0 + lane] >> 28) + 1 : 0;
                     const int nbox = __reduce_add_sync(0xffffffffu, mine);
                     if (lane == 0) mbar_expect_tx(fb, S::REL_BYTES + nbox * S::BOX_BYTES);
@@ -393,6 +412,7 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                                          (unsigned long long)(y + NB) * P.row_pitch <= P.scratch_words && (x & 3) == 0, CHK_TMA_SRC);
                             tma_box_g2s(sb + cl * S::CPITCH + v * S::VSLOT, &tmap, x, y, fb);
                         }
+                    }
                     }
                 }
                 if (lane == 0)
@@ -520,6 +540,7 @@ dedisp_status execute_cfg(dedisp_plan plan, const BitsliceGeom &G, int nbeams, l
     P.scratch_words = plan->planes_bytes / 4;
     P.ndm = plan->ndm;
     P.vinfo = nullptr;
+    P.vlist = nullptr;
     P.vrows = 0;
     const BitsliceTables &T = plan->tab[G.tab];
     P.ws = T.d_ws;
@@ -667,6 +688,7 @@ dedisp_status execute_pairs(dedisp_plan plan, const PairTables &T, int nbeams, l
     P.ws = T.d_ws;
     P.rel = T.d_rel;
     P.vinfo = T.d_vinfo;
+    P.vlist = nullptr;
     P.order = plan->tab[G.tab].d_order;
     P.out = (uint8_t *)out;
     P.out_beam_stride = out_beam_stride;
@@ -699,6 +721,125 @@ dedisp_status execute_pairs(dedisp_plan plan, const PairTables &T, int nbeams, l
         P.nchunks = (int)((c1 - c0) / C::CH);
         P.accumulate = c0 > 0;
         const bool f32 = out_f32 && c1 == T.npairs_pad;
+        const cudaError_t e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s, plan->device, &tm)
+                                  : launch_one<C, C::WIN_S, false>(P, grid, s, plan->device, &tm);
+        DEDISP_CUDA_TRY(plan, e);
+    }
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[3], s);
+        plan->timing_valid = true;
+        plan->timing_has_prepass = true;
+    }
+    return scratch_release(plan, s);
+}
+
+// Quad rows (quad_rows.cu): RAWNB-bit planes -> one (RAWNB+2)-plane row per (channel quad, triple of delay
+// differences) -> the tiled kernel over nchans/4 virtual channels (geometry C).  Same DM groups and tiles as the plain
+// geometry of the sample width.
+template <class C, int RAWNB>
+dedisp_status execute_quads(dedisp_plan plan, const QuadTables &T, int nbeams, long long nsamps_out,
+                            const uint8_t *in, size_t row_stride, size_t in_beam_stride, void *out,
+                            size_t out_beam_stride, int out_f32, cudaStream_t s, const BitsliceRange &range,
+                            bool reserve_only)
+{
+    static_assert(C::NB == RAWNB + 2, "a sum of four samples has two more planes than a sample");
+    const BitsliceGeom &G = plan->geom[geom_index(RAWNB)];
+    const long long ntiles = (nsamps_out + C::TILE_SAMPS - 1) / C::TILE_SAMPS;
+    const long long pitch =
+        (((long long)(plan->max_delay >> 5) + ntiles * C::TILE_WORDS + C::WIN_S + 4) + 3) & ~3ll;
+    if (ntiles > 0x7fffffff / C::TILE_WORDS || pitch > 0x7fffffff || nbeams > 65535) return DEDISP_ERR_INVALID_ARG;
+    const size_t raw_beam = (size_t)G.nchans_pad * RAWNB * (size_t)pitch;
+    const size_t rows_beam = (size_t)T.nrows * C::NB * (size_t)pitch;
+    if ((unsigned long long)nbeams * T.nrows * C::NB > 0x7fffffffull) return DEDISP_ERR_INVALID_ARG;
+    const size_t need_raw = raw_beam * (size_t)nbeams * 4, need_rows = rows_beam * (size_t)nbeams * 4;
+    if (G.nchans_pad > 65535) return DEDISP_ERR_INVALID_ARG;   // grid.y of the unpack pre-pass
+    dedisp_status sst = scratch_reserve(plan, &plan->d_planes, &plan->planes_bytes, need_raw, s);
+    if (sst == DEDISP_OK) sst = scratch_reserve(plan, &plan->d_pair_rows, &plan->pair_rows_bytes, need_rows, s);
+    if (sst != DEDISP_OK || reserve_only) return sst;
+    const int sms = plan->sm_count;
+    sst = scratch_acquire(plan, s);
+    if (sst != DEDISP_OK) return sst;
+    if (plan->poison >= 0 && range.prepass) {
+        DEDISP_CUDA_TRY(plan, cudaMemsetAsync(plan->d_planes, plan->poison, plan->planes_bytes, s));
+        DEDISP_CUDA_TRY(plan, cudaMemsetAsync(plan->d_pair_rows, plan->poison, plan->pair_rows_bytes, s));
+    }
+    if (plan->timing) cudaEventRecord(plan->ev[0], s);
+    if (range.prepass) {
+        DEDISP_CUDA_TRY(plan, launch_planes(RAWNB, in, in_beam_stride, row_stride, plan->nchans, nbeams,
+                                            plan->d_planes, (int)pitch, G.nchans_pad, s));
+        DEDISP_CUDA_TRY(plan, launch_quad_rows(T, RAWNB, plan->d_planes, raw_beam, G.nchans_pad, plan->d_pair_rows,
+                                               rows_beam, (int)pitch, nbeams, s));
+    }
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[1], s);
+        cudaEventRecord(plan->ev[2], s);
+    }
+    // the rows as a 2-D tensor [nbeams * nrows * NB lines][pitch words]; a box = the NB plane lines of one row x
+    // one window (words outside the tensor read as zero: variant v starts vskew(v) words early)
+    // (encoded once and kept in the plan: re-encoded only when the scratch pointer, the pitch or the line count change)
+    TensorMapCache &tc = plan->tmap[3];
+    const unsigned long long lines = (unsigned long long)nbeams * T.nrows * C::NB;
+    if (!tc.valid || tc.base != (void *)plan->d_pair_rows || tc.pitch != pitch || tc.lines != lines) {
+        EncodeTiledFn enc = encode_tiled_fn();
+        if (!enc) return DEDISP_ERR_CUDA;
+        const cuuint64_t dims[2] = {(cuuint64_t)pitch, (cuuint64_t)lines};
+        const cuuint64_t strides[1] = {(cuuint64_t)pitch * 4};
+        const cuuint32_t box[2] = {(cuuint32_t)C::template plane_words<C::WIN_S>(), (cuuint32_t)C::NB};
+        const cuuint32_t estr[2] = {1, 1};
+        static_assert(sizeof(CUtensorMap) == sizeof(tc.map), "tensor map storage");
+        if (enc(reinterpret_cast<CUtensorMap *>(tc.map), CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, plan->d_pair_rows, dims,
+                strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return DEDISP_ERR_CUDA;
+        tc.valid = true;
+        tc.base = plan->d_pair_rows;
+        tc.pitch = pitch;
+        tc.lines = lines;
+    }
+    const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tc.map);
+    BitsliceParams P;
+    P.planes = plan->d_pair_rows;
+    P.check_errors = plan->d_check_errors;
+    P.inject_fault = plan->inject_fault;
+    P.scratch_words = plan->pair_rows_bytes / 4;
+    P.ndm = plan->ndm;
+    P.vrows = T.nrows;
+    P.ws = T.d_ws;
+    P.rel = T.d_rel;
+    P.vinfo = nullptr;
+    P.vlist = T.d_vlist;
+    P.order = plan->tab[G.tab].d_order;
+    P.out = (uint8_t *)out;
+    P.out_beam_stride = out_beam_stride;
+    P.beam_pitch_words = rows_beam;
+    P.nsamps_out = nsamps_out;
+    P.row_pitch = (int)pitch;
+    P.nchans_pad = T.nquads_pad;
+    P.ngroups = range.g_count > 0 ? range.g_count : G.ngroups;
+    P.g_begin = range.g_begin;
+    P.ntiles = (int)ntiles;
+    P.nbeams = nbeams;
+    // rows beyond L2: tile-major inside blocks of gblock groups, as in execute_cfg
+    P.gblock = 1;
+    if (rows_beam * 4 > (size_t)64 << 20) {
+        const double spread = (double)(plan->max_delay >> 5) + 1.0;
+        int gb = (int)std::sqrt((double)sms * C::TILE_WORDS * G.ngroups / spread);
+        P.gblock = gb < 1 ? 1 : gb > P.ngroups ? P.ngroups : gb;
+    }
+    P.vec_ok = ((uintptr_t)out % 16 == 0) && (nsamps_out % 4 == 0) &&
+               (nbeams == 1 || out_beam_stride % 16 == 0);
+    const long long nitems = (long long)nbeams * P.ngroups * ntiles;
+    const int grid = (int)(nitems < sms ? nitems : sms);
+    // channel blocks as in execute_cfg: a quad sum is at most 4 (2^RAWNB - 1)
+    long long cblk = (((1ll << C::NP) - 1) / (4 * ((1ll << RAWNB) - 1))) / CH_PAD * CH_PAD;
+    if (cblk < CH_PAD) return DEDISP_ERR_INVALID_ARG;
+    if (cblk > T.nquads_pad) cblk = T.nquads_pad;
+    for (long long c0 = 0; c0 < T.nquads_pad; c0 += cblk) {
+        const long long c1 = c0 + cblk < T.nquads_pad ? c0 + cblk : T.nquads_pad;
+        P.chunk0 = (int)(c0 / C::CH);
+        P.nchunks = (int)((c1 - c0) / C::CH);
+        P.accumulate = c0 > 0;
+        const bool f32 = out_f32 && c1 == T.nquads_pad;
         const cudaError_t e = f32 ? launch_one<C, C::WIN_S, true>(P, grid, s, plan->device, &tm)
                                   : launch_one<C, C::WIN_S, false>(P, grid, s, plan->device, &tm);
         DEDISP_CUDA_TRY(plan, e);

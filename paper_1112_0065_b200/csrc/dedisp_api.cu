@@ -36,6 +36,7 @@ void free_dm_state(dedisp_plan p)
     p->ndm = 0;
     p->max_delay = -1;
     p->dms.clear();
+    quad_release(p);
     pair_release(p);
     bitslice_release(p);
 }
@@ -167,6 +168,7 @@ dedisp_status dedisp_set_dm_list(dedisp_plan plan, const double *dms_host, int n
 #endif
     dedisp_status st = bitslice_prepare(plan);
     if (st == DEDISP_OK) st = pair_prepare(plan);
+    if (st == DEDISP_OK) st = quad_prepare(plan);
     if (st != DEDISP_OK) free_dm_state(plan);
     return st;
 }
@@ -195,7 +197,8 @@ dedisp_status dedisp_execute_tscrunch(dedisp_plan plan, int tscrunch, int nbeams
             return DEDISP_OK;
         }
         // INVALID_ARG from bitslice_execute means "plan does not fit this kernel"
-        if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE || plan->want == DEDISP_KERNEL_PAIRS)
+        if (st != DEDISP_ERR_INVALID_ARG || plan->want == DEDISP_KERNEL_BITSLICE || plan->want == DEDISP_KERNEL_PAIRS ||
+            plan->want == DEDISP_KERNEL_QUADS)
             return st;
     }
     int direct_nbits = in_nbits;
@@ -397,7 +400,7 @@ dedisp_status dedisp_get_delay_table(dedisp_plan plan, int *host_out)
 
 dedisp_status dedisp_set_kernel(dedisp_plan plan, dedisp_kernel which)
 {
-    if (!plan || (int)which < 0 || (int)which > 3) return DEDISP_ERR_INVALID_ARG;
+    if (!plan || (int)which < 0 || (int)which > 4) return DEDISP_ERR_INVALID_ARG;
     plan->want = which;
     return DEDISP_OK;
 }

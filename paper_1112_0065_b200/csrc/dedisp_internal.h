@@ -47,6 +47,19 @@ struct PairTables {
     bool usable = false;
 };
 
+// Tables of the quad-row path (quad_rows.cu): virtual channel q = channels 4q .. 4q+3 summed at fixed delay differences
+// (d1, d2, d3) to channel 4q; one (nbits + 2)-plane row per (quad, triple) that occurs in the DM list.
+struct QuadTables {
+    uint32_t *d_rel = nullptr;      // [ngroups][nquads_pad][32] ((variant slot + word in the variant's box) bytes << 16) | shift
+    int32_t *d_ws = nullptr;        // [ngroups][nquads_pad] window start word (of channel 4q; kept for the checks)
+    int2 *d_vlist = nullptr;        // [ngroups][nquads_pad][NV] (row of each variant the group uses or -1, box start word)
+    int32_t *d_row0 = nullptr;      // [nquads_pad + 1] first row of each quad (rows of a quad: triples in ascending order)
+    int32_t *d_trip = nullptr;      // [nrows][4] (d1, d2, d3, 0) of each row
+    int nrows = 0;
+    int nquads_pad = 0;
+    bool usable = false;
+};
+
 // The encoded 2-D tensor map of the pair rows (cuTensorMapEncodeTiled), kept until the scratch moves or the shape changes.
 struct TensorMapCache {
     alignas(64) unsigned char map[128] = {};
@@ -78,7 +91,8 @@ struct dedisp_plan_s {
     PairTables pairs8;            // pair-row path, 8-bit samples (Cfg9P, DM groups of tab[1])
     uint32_t *d_pair_rows = nullptr;
     size_t pair_rows_bytes = 0;
-    TensorMapCache tmap[3];       // pair rows of 2-, 4- and 8-bit samples
+    QuadTables quads8;            // quad-row path, 8-bit samples (Cfg10Q, DM groups of tab[1])
+    TensorMapCache tmap[4];       // pair rows of 2-, 4- and 8-bit samples; quad rows of 8-bit samples
     // diagnostics (dedisp_debug_set_poison / dedisp_debug_check_errors)
     int poison = -1;                               // >= 0: every execute first fills the scratch with this byte
     int inject_fault = 0;                          // -DDEDISP_CHECKS builds: a deliberate fault the checks must count
@@ -180,6 +194,7 @@ dedisp_status bitslice_run_cfg8(const BitsliceCall &c);
 dedisp_status bitslice_run_pairs2(const BitsliceCall &c);
 dedisp_status bitslice_run_pairs4(const BitsliceCall &c);
 dedisp_status bitslice_run_pairs8(const BitsliceCall &c);
+dedisp_status bitslice_run_quads8(const BitsliceCall &c);
 
 // Plan-owned scratch (dedisp_api.cu).  reserve: grow *ptr to `need` bytes (cudaFree + cudaMalloc: synchronises the
 // device, so nothing in flight still reads the old buffer; refused with DEDISP_ERR_CUDA while `s` is being captured
@@ -197,6 +212,11 @@ dedisp_status scratch_release(dedisp_plan plan, cudaStream_t s);
 dedisp_status pair_prepare(dedisp_plan plan);       // after bitslice_prepare; leaves pairs.usable
 void pair_release(dedisp_plan plan);
 cudaError_t launch_pair_rows(const PairTables &T, int raw_nbits, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
+                             uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s);
+// quad_rows.cu
+dedisp_status quad_prepare(dedisp_plan plan);       // after pair_prepare; leaves quads8.usable
+void quad_release(dedisp_plan plan);
+cudaError_t launch_quad_rows(const QuadTables &T, int raw_nbits, const uint32_t *raw, size_t raw_beam_pitch, int nchans_pad,
                              uint32_t *rows, size_t rows_beam_pitch, int row_pitch, int nbeams, cudaStream_t s);
 // DM groups of the plan's bit-sliced geometry for this sample width, or 0 if the kernel cannot serve it
 int bitslice_ngroups(dedisp_plan plan, int nbits);

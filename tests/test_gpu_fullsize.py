@@ -43,8 +43,11 @@ def test_full_size_config(name, golden_dir):
     got = gpu_dedisperse(p, x, w.nbits, w.nsamps_out, w.out_dtype)
     used = dd.dedisp_get_last_kernel(p)
     dd.dedisp_destroy(p)
-    assert used in (dd.DEDISP_KERNEL_DIRECT, dd.DEDISP_KERNEL_BITSLICE, dd.DEDISP_KERNEL_PAIRS)
-    if name != "tiny":
+    assert used in (dd.DEDISP_KERNEL_DIRECT, dd.DEDISP_KERNEL_BITSLICE, dd.DEDISP_KERNEL_PAIRS,
+                    dd.DEDISP_KERNEL_QUADS)
+    if name == "wide8":
+        assert used == dd.DEDISP_KERNEL_QUADS      # 8-bit samples, 64 DM groups: the quad rows pay
+    elif name != "tiny":
         assert used == dd.DEDISP_KERNEL_PAIRS      # the HTRU and wideband DM lists pay for the pair rows
     # (2) sampled whole rows, element by element against the oracle
     rows = sorted({0, 1, w.ndm // 3, w.ndm // 2, w.ndm - 2, w.ndm - 1} & set(range(w.ndm)))

@@ -13,7 +13,7 @@ import workloads as W  # noqa: E402
 from gpu_helpers import gpu_dedisperse, make_plan, oracle_inputs  # noqa: E402
 
 KERNELS = [dd.DEDISP_KERNEL_AUTO, dd.DEDISP_KERNEL_DIRECT]
-TILED = (dd.DEDISP_KERNEL_BITSLICE, dd.DEDISP_KERNEL_PAIRS)   # the tiled kernel, on planes or on pair rows
+TILED = (dd.DEDISP_KERNEL_BITSLICE, dd.DEDISP_KERNEL_PAIRS, dd.DEDISP_KERNEL_QUADS)   # the tiled kernel: planes, pair or quad rows
 
 
 @pytest.fixture(scope="module", autouse=True)
