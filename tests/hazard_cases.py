@@ -19,6 +19,7 @@ tests/test_gpu_selfcheck.py runs both builds over all cases.  Cases:
   tiny_auto / tiny_direct   BASELINE configs[0] through the tiled kernel (plain planes, 1-D TMA) / the DIRECT kernel
   pairs3     cut-down HTRU shape at the top of the DM range: pair rows, 3 variants per slot, negative-x TMA boxes
   pairs8     8-bit wideband channelisation on 9-plane pair rows (Cfg9P)
+  quads8     ... on 10-plane quad rows (Cfg10Q): per-variant box starts, boxes that begin before / end after a row
   blocks     4100 channels of 2-bit samples: channel blocks, the epilogue reads `out` back (accumulate)
   unaligned  input base pointer at odd byte offsets: the guarded 128-bit straddling loads of the unpack pre-pass
   multi      several persistent work items per CTA (the ring wraps many times) and a ragged last tile
@@ -95,6 +96,13 @@ def pairs3():
 def pairs8():
     w = W.CONFIGS["wide8"].scaled(nchans=1001, ndm=70, dm_lo=900.0, dm_hi=900.0 + STEP8 * 69, nsamps_out=3000)
     _run(w, dd.DEDISP_KERNEL_PAIRS, 8, expect=dd.DEDISP_KERNEL_PAIRS)
+
+
+def quads8():
+    w = W.CONFIGS["wide8"].scaled(nchans=1001, ndm=262, dm_lo=1744.0, dm_hi=1744.0 + STEP8 * 261, nsamps_out=3000)
+    _run(w, dd.DEDISP_KERNEL_QUADS, 8, expect=dd.DEDISP_KERNEL_QUADS)
+    w = W.CONFIGS["wide8"].scaled(nchans=64, ndm=256, dm_hi=STEP8 * 255, nsamps_out=1409)
+    _run(w, dd.DEDISP_KERNEL_QUADS, 8, od="f32", expect=dd.DEDISP_KERNEL_QUADS)
 
 
 def blocks():
@@ -179,7 +187,7 @@ def fault_injection():
     return f"bit-exact vs oracle; injected wrong stage tags counted by the checks: {counted} (pair rows, planes)"
 
 
-CASES = {f.__name__: f for f in (tiny_auto, tiny_direct, pairs3, pairs8, blocks, unaligned, multi, search, fault_injection)}
+CASES = {f.__name__: f for f in (tiny_auto, tiny_direct, pairs3, pairs8, quads8, blocks, unaligned, multi, search, fault_injection)}
 
 
 def main(argv):
