@@ -156,15 +156,18 @@ def cpu_baseline(w: W.Workload, tscrunch: int = 1) -> dict:
     return res
 
 
-def ncu_traffic(config: str):
+def ncu_traffic(config: str, kernel: str | None = None):
     """(DRAM bytes per launch of the dominant kernel, source file, commit of the capture) from the committed ncu
-    captures (profiles/traffic.csv: config,bytes_per_launch,source,commit), or (None, None, None)."""
+    captures (profiles/traffic.csv: config,bytes_per_launch,source,commit[,kernel]), or (None, None, None).  A row that
+    names a kernel only serves a run of that kernel (--kernel can force another one than the capture saw)."""
     p = ROOT / "profiles" / "traffic.csv"
     if not p.exists():
         return None, None, None
     for line in p.read_text().splitlines():
         f = [v.strip() for v in line.split(",")]
         if len(f) >= 2 and f[0] == config:
+            if kernel is not None and len(f) > 4 and f[4] and f[4] != kernel:
+                continue
             try:
                 return float(f[1]), (f[2] if len(f) > 2 else None), (f[3] if len(f) > 3 else None)
             except ValueError:
@@ -309,7 +312,7 @@ def roofline_of(w, k, m, ms_per_step, props, peaks, config_name):
     t_alu, t_hbm = adds / alu_peak, (m["in_bytes"] + m["out_bytes"]) / hbm_peak
     mm = statistics.mean(m["main_ms"]) * 1e-3
     achieved = adds / mm
-    traffic, tsrc, tcommit = ncu_traffic(config_name)
+    traffic, tsrc, tcommit = ncu_traffic(config_name, KERNEL_NAMES.get(m["kernel_used"], "direct_kernel"))
     return {"bound": "alu", "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
             "frac": achieved / alu_peak, "traffic": traffic, "traffic_source": tsrc, "traffic_capture_commit": tcommit,
             "kernel": KERNEL_NAMES.get(m["kernel_used"], "direct_kernel"),

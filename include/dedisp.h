@@ -42,7 +42,7 @@
  * launch counter and the per-kernel attribute flags, is atomic).
  *
  * Streams and scratch: the execute calls only enqueue work on the caller's stream.  A plan
- * owns device scratch (bit planes, pair rows) that every execute of that plan re-uses:
+ * owns device scratch (bit planes, pair or quad rows) that every execute of that plan re-uses:
  * executes of ONE plan are therefore ordered -- a call on another stream than the plan's
  * previous call first waits (cudaStreamWaitEvent) for the event the previous call recorded
  * behind its kernels, so double-buffered callers stay correct but two executes of one plan
@@ -162,7 +162,7 @@ size_t dedisp_get_in_row_stride_bytes_tscrunch(dedisp_plan plan, int tscrunch, l
                                                int in_nbits);
 
 /* Grow the plan's scratch to what dedisp_execute_batch(plan, nbeams, nsamps_out, .., in_nbits, ..)
- * needs with the kernel selection in force (AUTO: pair rows where they pay, else bit planes), so that
+ * needs with the kernel selection in force (AUTO: quad or pair rows where they pay, else bit planes), so that
  * later executes of that size or smaller never allocate (see "Streams and scratch").  Synchronises
  * the device if it has to re-allocate.  Errors: INVALID_ARG, NO_DM_LIST, UNSUPPORTED_NBITS, ALLOC. */
 dedisp_status dedisp_reserve(dedisp_plan plan, int nbeams, long long nsamps_out, int in_nbits);
