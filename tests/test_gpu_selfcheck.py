@@ -12,6 +12,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 ROOT = Path(__file__).resolve().parent.parent
 CHECKS_LIB = ROOT / "paper_1112_0065_b200" / "libdedisp_b200_checks.so"
+NCASES = 10      # tests/hazard_cases.py::CASES
 
 
 def _run_cases(env_extra):
@@ -24,7 +25,7 @@ def _run_cases(env_extra):
 
 def test_hazard_cases_product_build():
     out = _run_cases({"DEDISP_B200_LIB": ""})
-    assert "9 cases ok" in out and "checks compiled: False" in out
+    assert f"{NCASES} cases ok" in out and "checks compiled: False" in out
 
 
 def test_hazard_cases_with_in_kernel_checks():
@@ -32,4 +33,4 @@ def test_hazard_cases_with_in_kernel_checks():
     if not CHECKS_LIB.exists() or build.stale(CHECKS_LIB):
         build.build(defs=["DEDISP_CHECKS"], out=CHECKS_LIB)
     out = _run_cases({"DEDISP_B200_LIB": str(CHECKS_LIB)})
-    assert "9 cases ok" in out and "checks compiled: True" in out
+    assert f"{NCASES} cases ok" in out and "checks compiled: True" in out
