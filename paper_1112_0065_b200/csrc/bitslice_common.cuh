@@ -98,9 +98,9 @@ struct Cfg {
     static constexpr int VSKEW = BS_VSKEW_UNIT * (NV_ - 1);
     static __host__ __device__ constexpr int vskew(int v) { return BS_VSKEW_UNIT * v; }
 #else
-    // up to 3 variants (pair rows): odd variants 16 banks away.  More (quad rows, NV = 7): 0, 16, 8, 24, 4, 20, 12
-    // banks -- any two variants at least 4 banks apart, so lanes at the same or a neighbouring window offset in
-    // different variants never share a bank (profiles/r2_wide8.md)
+    // up to 3 variants (pair rows): odd variants 16 banks away.  More (quad rows, NV = 7): no fixed skew -- every
+    // variant of a (DM group, quad) has a box start of its own, placed by quad_prepare so that the lanes' words fall
+    // into different banks (quad_rows.cu); VSKEW = 28 is the room the box leaves for that placement
     static constexpr int VSKEW = NV_ > 3 ? 28 : NV_ > 1 ? 16 : 0;
     static __host__ __device__ constexpr int vskew(int v)
     {

@@ -775,7 +775,7 @@ dedisp_status execute_quads(dedisp_plan plan, const QuadTables &T, int nbeams, l
         cudaEventRecord(plan->ev[2], s);
     }
     // the rows as a 2-D tensor [nbeams * nrows * NB lines][pitch words]; a box = the NB plane lines of one row x
-    // one window (words outside the tensor read as zero: variant v starts vskew(v) words early)
+    // one window (words outside the tensor read as zero: a variant's box may start before its row or end after it)
     // (encoded once and kept in the plan: re-encoded only when the scratch pointer, the pitch or the line count change)
     TensorMapCache &tc = plan->tmap[3];
     const unsigned long long lines = (unsigned long long)nbeams * T.nrows * C::NB;
