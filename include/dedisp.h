@@ -452,7 +452,28 @@ dedisp_status dedisp_transpose_time_major(const void *in_dev, int nchans, long l
  * in a normal build.  Synchronises the device.
  * dedisp_debug_inject_fault: kind 1 makes the producer warp of a -DDEDISP_CHECKS build stamp a wrong tag on the
  * first ring stage every CTA fills (the data is still right), so that the stage-tag check must count failures --
- * the test that the checks can fail at all; kind 0 switches it off; no effect in a normal build. */
+ * the test that the checks can fail at all; kind 0 switches it off; no effect in a normal build.
+ * dedisp_debug_quad_tables: HOST only, needs no GPU -- the tables dedisp_set_dm_list prepares for the quad-row path
+ * (DEDISP_KERNEL_QUADS), built by the same host code from a delay table and a lane order the CALLER passes in host
+ * memory, so that their addressing contract can be checked without a device (tests/test_quad_tables_cpu.py):
+ *   delay_host [nchans][ndm] int32, delays in samples, >= 0, non-decreasing along the channels of a quad;
+ *   lanes_host [ngroups][32] int32: the trial (column of delay_host) each lane of a DM group serves, -1 = padding lane
+ *              (it repeats the last trial before it; lane 0 of a group is never padding);
+ *   info       filled always: nv = variant slots per (group, quad), vslot_bytes = bytes of one variant slot of a stage,
+ *              plane_words = words of one plane line of a staged box, tile_words = words per tile, nquads_pad,
+ *              nrows = rows to build, usable = 0 when the list cannot take quad rows (more than nv distinct triples in
+ *              a group, differences outside 0 .. 2^20 - 1, windows wider than a box) -- then nothing else is written;
+ *   row0 [nquads_pad + 1], trip [nrows][4] = (d1, d2, d3, 0) of each row, vlist [ngroups][nquads_pad][nv][2] = (row or
+ *   -1, first word of the variant's box for tile 0), rel [ngroups][nquads_pad][32] = (byte offset of the lane's first
+ *   word in the slot << 16) | (delay & 31): each written when non-NULL (call once with NULL buffers to size them).
+ * Errors: INVALID_ARG (NULL delay / lanes / info, nchans < 4, ndm < 1, ngroups < 1, a lane index outside the table,
+ * tables beyond 2^28 entries). */
+typedef struct {
+    int nv, vslot_bytes, plane_words, tile_words, nquads_pad, nrows, usable;
+} dedisp_quad_table_info;
+dedisp_status dedisp_debug_quad_tables(int nchans, int ndm, const int *delay_host, int ngroups, const int *lanes_host,
+                                       dedisp_quad_table_info *info, int *row0, int *trip, int *vlist,
+                                       unsigned int *rel);
 int dedisp_debug_checks_compiled(void);
 dedisp_status dedisp_debug_inject_fault(dedisp_plan plan, int kind);
 dedisp_status dedisp_debug_set_poison(dedisp_plan plan, int byte_value);

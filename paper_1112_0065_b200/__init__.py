@@ -57,6 +57,7 @@ ABI = {
     "dedisp_set_timing": (_i, [_vp, _i]),
     "dedisp_get_last_kernel_ms": (_i, [_vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
     "dedisp_get_launch_count": (ctypes.c_ulonglong, []),
+    "dedisp_debug_quad_tables": (_i, [_i, _i, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
     "dedisp_debug_checks_compiled": (_i, []),
     "dedisp_debug_set_poison": (_i, [_vp, _i]),
     "dedisp_debug_inject_fault": (_i, [_vp, _i]),
@@ -220,6 +221,37 @@ def dedisp_set_kernel(plan: int, which: int) -> None:
 
 def dedisp_get_last_kernel(plan: int) -> int:
     return lib().dedisp_get_last_kernel(plan)
+
+
+class _QuadTableInfo(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int) for n in ("nv", "vslot_bytes", "plane_words", "tile_words", "nquads_pad", "nrows",
+                                            "usable")]
+
+
+def dedisp_debug_quad_tables(delay_host, lanes_host):
+    """Host only (no GPU): (info dict, row0, trip, vlist, rel) -- the quad-row tables for a delay table
+    int32 [nchans][ndm] and a lane order int32 [ngroups][32]; the arrays are None when info["usable"] is 0."""
+    import numpy as np
+    delay = np.ascontiguousarray(delay_host, dtype=np.int32)
+    lanes = np.ascontiguousarray(lanes_host, dtype=np.int32)
+    nchans, ndm = delay.shape
+    ngroups = lanes.shape[0]
+    info = _QuadTableInfo()
+    p = lambda a: a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+    st = lib().dedisp_debug_quad_tables(nchans, ndm, p(delay), ngroups, p(lanes), ctypes.byref(info), None, None, None,
+                                        None)
+    _check(None, st, "dedisp_debug_quad_tables")
+    d = {n: getattr(info, n) for n, _ in _QuadTableInfo._fields_}
+    if not d["usable"]:
+        return d, None, None, None, None
+    row0 = np.empty(d["nquads_pad"] + 1, dtype=np.int32)
+    trip = np.empty((d["nrows"], 4), dtype=np.int32)
+    vlist = np.empty((ngroups, d["nquads_pad"], d["nv"], 2), dtype=np.int32)
+    rel = np.empty((ngroups, d["nquads_pad"], 32), dtype=np.uint32)
+    st = lib().dedisp_debug_quad_tables(nchans, ndm, p(delay), ngroups, p(lanes), ctypes.byref(info), p(row0), p(trip),
+                                        p(vlist), p(rel))
+    _check(None, st, "dedisp_debug_quad_tables")
+    return d, row0, trip, vlist, rel
 
 
 def dedisp_debug_checks_compiled() -> bool:

@@ -166,34 +166,34 @@ void release_tables(QuadTables &T)
 
 void quad_release(dedisp_plan p) { release_tables(p->quads8); }
 
-// Called after pair_prepare.  Host bookkeeping on the delay table the device built (copied back once per set_dm_list):
-// differences, de-duplication and indices only -- no arithmetic of the method.  Leaves T.usable false (not an error)
-// when the plan cannot take quad rows.
+// The host half of quad_prepare, on HOST copies of the delay table [nchans][ndm] and of the lane order
+// [ngroups][32] (output row of each lane, -1 = padding): pure bookkeeping, no CUDA call -- also reachable without a GPU
+// through dedisp_debug_quad_tables (tests/test_quad_tables_cpu.py checks the addressing contract of the tables).
+struct QuadHost {
+    std::vector<int32_t> row0, ws, trip;
+    std::vector<int2> vlist;
+    std::vector<uint32_t> rel;
+    long long nrows = 0;
+    bool fits = false;
+};
+
 template <class C>
-static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G, const BitsliceTables &B, QuadTables &T)
+static void build_tables_host(const int32_t *delay, const int32_t *lanes, int nchans, int ndm, int ngroups,
+                              int nquads_pad, QuadHost &H)
 {
-    release_tables(T);
-    if (!G.usable || !B.d_order || p->nchans < 4 || B.dms_per_group < 1) return DEDISP_OK;
-    const int ndm = p->ndm, nchans = p->nchans, ngroups = B.ngroups;
-    const int nquads_pad = ((G.nchans_pad / 4) + CH_PAD - 1) / CH_PAD * CH_PAD;
-    const size_t tbl = (size_t)nchans * ndm;
-    if (tbl > ((size_t)1 << 28) || (size_t)ngroups * nquads_pad * 32 > ((size_t)1 << 28)) return DEDISP_OK;   // host budget
-    std::vector<int32_t> delay(tbl), lanes((size_t)ngroups * 32);
-    cudaError_t e = cudaMemcpy(delay.data(), p->d_delay, tbl * sizeof(int32_t), cudaMemcpyDeviceToHost);
-    if (e == cudaSuccess) e = cudaMemcpy(lanes.data(), B.d_order, lanes.size() * sizeof(int32_t), cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) {
-        p->last_cuda_error = (int)e;
-        return DEDISP_ERR_CUDA;
-    }
     constexpr int NV = C::NV;
     constexpr int VSLOT_BYTES = C::template vslot_words<C::WIN_S>() * 4;
     constexpr int PLW = C::template plane_words<C::WIN_S>();      // words of one plane line of a staged box
     constexpr int PMAX = PLW - C::TILE_WORDS - 1;                 // last box word a lane's window may start at
     static_assert(VSLOT_BYTES % 128 == 0, "the variant slots start at bank 0");
-    std::vector<int32_t> row0(nquads_pad + 1, 0), ws((size_t)ngroups * nquads_pad, 0);
-    std::vector<int2> vlist((size_t)ngroups * nquads_pad * NV, make_int2(-1, 0));
-    std::vector<uint32_t> rel((size_t)ngroups * nquads_pad * 32, 0u);
-    std::vector<int32_t> trip;
+    std::vector<int32_t> &row0 = H.row0, &ws = H.ws, &trip = H.trip;
+    std::vector<int2> &vlist = H.vlist;
+    std::vector<uint32_t> &rel = H.rel;
+    row0.assign(nquads_pad + 1, 0);
+    ws.assign((size_t)ngroups * nquads_pad, 0);
+    vlist.assign((size_t)ngroups * nquads_pad * NV, make_int2(-1, 0));
+    rel.assign((size_t)ngroups * nquads_pad * 32, 0u);
+    trip.clear();
     std::vector<uint64_t> keys(ndm), uniq;
     bool fits = true;
     long long nrows = 0;
@@ -285,6 +285,37 @@ static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G, const 
         if (nrows > 0x03ffffff) fits = false;
     }
     row0[nquads_pad] = (int32_t)nrows;
+    H.nrows = nrows;
+    H.fits = fits;
+}
+
+// Called after pair_prepare.  Host bookkeeping on the delay table the device built (copied back once per set_dm_list):
+// differences, de-duplication and indices only -- no arithmetic of the method.  Leaves T.usable false (not an error)
+// when the plan cannot take quad rows.
+template <class C>
+static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G, const BitsliceTables &B, QuadTables &T)
+{
+    release_tables(T);
+    if (!G.usable || !B.d_order || p->nchans < 4 || B.dms_per_group < 1) return DEDISP_OK;
+    const int ndm = p->ndm, nchans = p->nchans, ngroups = B.ngroups;
+    const int nquads_pad = ((G.nchans_pad / 4) + CH_PAD - 1) / CH_PAD * CH_PAD;
+    const size_t tbl = (size_t)nchans * ndm;
+    if (tbl > ((size_t)1 << 28) || (size_t)ngroups * nquads_pad * 32 > ((size_t)1 << 28)) return DEDISP_OK;   // host budget
+    std::vector<int32_t> delay(tbl), lanes((size_t)ngroups * 32);
+    cudaError_t e = cudaMemcpy(delay.data(), p->d_delay, tbl * sizeof(int32_t), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(lanes.data(), B.d_order, lanes.size() * sizeof(int32_t), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) {
+        p->last_cuda_error = (int)e;
+        return DEDISP_ERR_CUDA;
+    }
+    QuadHost H;
+    build_tables_host<C>(delay.data(), lanes.data(), nchans, ndm, ngroups, nquads_pad, H);
+    constexpr int NV = C::NV;
+    const bool fits = H.fits;
+    const long long nrows = H.nrows;
+    std::vector<int32_t> &row0 = H.row0, &ws = H.ws, &trip = H.trip;
+    std::vector<int2> &vlist = H.vlist;
+    std::vector<uint32_t> &rel = H.rel;
     if (!fits) return DEDISP_OK;
     const size_t ntab = (size_t)ngroups * nquads_pad;
     e = cudaMalloc(&T.d_rel, ntab * 32 * sizeof(uint32_t));
@@ -306,6 +337,43 @@ static dedisp_status prepare_tables(dedisp_plan p, const BitsliceGeom &G, const 
     T.nrows = (int)nrows;
     T.nquads_pad = nquads_pad;
     T.usable = true;
+    return DEDISP_OK;
+}
+
+// include/dedisp.h: the tables of the quad-row path from host arrays, no GPU involved
+extern "C" dedisp_status dedisp_debug_quad_tables(int nchans, int ndm, const int *delay_host, int ngroups,
+                                                  const int *lanes_host, dedisp_quad_table_info *info, int *row0,
+                                                  int *trip, int *vlist, unsigned int *rel)
+{
+    using C = Cfg10Q;
+    if (!delay_host || !lanes_host || !info || nchans < 4 || ndm < 1 || ngroups < 1) return DEDISP_ERR_INVALID_ARG;
+    const int nchans_pad = (nchans + CH_PAD - 1) / CH_PAD * CH_PAD;
+    const int nquads_pad = ((nchans_pad / 4) + CH_PAD - 1) / CH_PAD * CH_PAD;
+    if ((size_t)nchans * ndm > ((size_t)1 << 28) || (size_t)ngroups * nquads_pad * 32 > ((size_t)1 << 28))
+        return DEDISP_ERR_INVALID_ARG;
+    for (int g = 0; g < ngroups; ++g) {
+        if (lanes_host[(size_t)g * 32] < 0) return DEDISP_ERR_INVALID_ARG;
+        for (int l = 0; l < 32; ++l)
+            if (lanes_host[(size_t)g * 32 + l] >= ndm) return DEDISP_ERR_INVALID_ARG;
+    }
+    QuadHost H;
+    build_tables_host<C>(delay_host, lanes_host, nchans, ndm, ngroups, nquads_pad, H);
+    info->nv = C::NV;
+    info->vslot_bytes = C::template vslot_words<C::WIN_S>() * 4;
+    info->plane_words = C::template plane_words<C::WIN_S>();
+    info->tile_words = C::TILE_WORDS;
+    info->nquads_pad = nquads_pad;
+    info->nrows = H.fits ? (int)H.nrows : 0;
+    info->usable = H.fits ? 1 : 0;
+    if (!H.fits) return DEDISP_OK;
+    if (row0) std::copy(H.row0.begin(), H.row0.end(), row0);
+    if (trip) std::copy(H.trip.begin(), H.trip.end(), trip);
+    if (vlist)
+        for (size_t i = 0; i < H.vlist.size(); ++i) {
+            vlist[2 * i] = H.vlist[i].x;
+            vlist[2 * i + 1] = H.vlist[i].y;
+        }
+    if (rel) std::copy(H.rel.begin(), H.rel.end(), rel);
     return DEDISP_OK;
 }
 
