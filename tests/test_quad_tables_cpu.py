@@ -133,3 +133,38 @@ def test_lists_that_cannot_take_quad_rows_and_bad_arguments():
     delay2 = delay.copy()
     delay2[0] = 5
     assert dd.dedisp_debug_quad_tables(delay2, lanes)[0]["usable"] == 0
+
+
+def test_walking_the_tables_on_the_cpu_reproduces_the_oracle_sums():
+    """The data flow of the quad path replayed in numpy from the PRODUCT's tables (rows from trip/row0, every lane
+    gathering from the row, box start, word and shift its tables name) against oracle.dedisperse: the tables alone
+    decide which samples are summed, so this pins them end to end without a GPU."""
+    nchans, ndm, nso = 70, 256, 200                 # 70 channels: the last quad has two
+    w = WIDE8.scaled(nchans=nchans, ndm=ndm, df=-4.0, dm_lo=100.0, dm_hi=100.0 + 0.02 * (ndm - 1), nsamps_out=nso)
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    x = W.generate(w, md)                            # uint8 [nchans][nsamps_in]: 8-bit samples are the bytes
+    lanes = np.arange(ndm, dtype=np.int32).reshape(ndm // 32, 32)
+    info, row0, trip, vlist, rel = dd.dedisp_debug_quad_tables(delay, lanes)
+    assert info["usable"] == 1 and info["nrows"] > 5 * info["nquads_pad"]    # many triples per quad (232 rows, 18 quads)
+    vslot = info["vslot_bytes"]
+    nin = nso + md
+    xs8 = np.zeros((4 * info["nquads_pad"], nin + 64), dtype=np.int64)       # channels / samples beyond the input: zero
+    xs8[:nchans, :nin] = x[:, :nin]
+    t = np.arange(nso)
+    got = np.zeros((ndm, nso), dtype=np.int64)
+    for g in range(lanes.shape[0]):
+        for l in range(32):
+            d = lanes[g, l]
+            for q in range(info["nquads_pad"]):
+                r = int(rel[g, q, l])
+                off = r >> 16
+                v, pos = off // vslot, (off % vslot) // 4
+                row, box = vlist[g, q, v]
+                assert row0[q] <= row < row0[q + 1]
+                first = (box + pos) * 32 + (r & 0xFFFF)          # sample of the row the lane's output t = 0 reads
+                d1, d2, d3, _ = trip[row]
+                for k, dk in enumerate((0, d1, d2, d3)):         # the row: sum of the quad's channels at its triple
+                    got[d] += xs8[4 * q + k, first + dk + t]
+    want = oracle.dedisperse(delay, x, 8, nso)
+    assert np.array_equal(got, want.astype(np.int64))
