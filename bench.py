@@ -186,9 +186,7 @@ KERNEL_NAMES = {1: "direct_kernel", 2: "bitslice_dedisperse", 3: "bitslice_dedis
 ALU_PIPE_INSTR_PER_ADD = {
     (3, 2): (626.0 / 4096.0, "profiles/r2_sass_cfg3p.txt: 626 ALU-pipe of 918 instructions per 4096 adds"),
     (3, 8): (0.455, "profiles/r2_wide8.md: ncu source page, LOP3 + SHF share of 23.97 G instructions"),
-    (4, 8): (0.244, "profiles/r2_wide8.md: ncu source page of capture r2b, LOP3 + SHF + LEA = 61.8 % of the "
-                    "13.56 G warp instructions (smsp__inst_executed.sum) per 1.0995e12 adds"),
-    (2, 2): (0.21, "DESIGN.md Sec. 6 C: 62 full adders + ripple + 64 SHF per 32 channels and word"),
+    (4, 8): (531.0 / 2048.0, "profiles/r2_sass_cfg10q.txt: 531 ALU-pipe of 774 instructions per 2048 adds"),
 }
 ALU_PIPE_LANES_PER_CLK_PER_SM = 64
 
