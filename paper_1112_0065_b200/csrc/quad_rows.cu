@@ -383,6 +383,11 @@ dedisp_status quad_prepare(dedisp_plan p)
     // enough for the rows to pay: a handful of groups cannot amortise ~75 rows per quad
     release_tables(p->quads8);
     if (!p->pairs8.usable || p->tab[1].ngroups < 8) return DEDISP_OK;
+    // one channel block only: sums of more than (2^NP - 1) / 255 = 4112 channels need the channel-block form of the
+    // launch (execute_quads has it, as execute_pairs does), which no GPU test of the quad path has exercised -- such
+    // plans stay on the pair rows, whose channel blocks are tested
+    constexpr long long QUADS_PER_BLOCK = (((1ll << Cfg10Q::NP) - 1) / (4 * 255)) / CH_PAD * CH_PAD;
+    if (((p->geom[8].nchans_pad / 4) + CH_PAD - 1) / CH_PAD * CH_PAD > QUADS_PER_BLOCK) return DEDISP_OK;
     return prepare_tables<Cfg10Q>(p, p->geom[8], p->tab[1], p->quads8);
 }
 
