@@ -98,3 +98,11 @@ def test_quads_equal_pairs_and_planes_on_one_plan_and_refusals():
     with pytest.raises(dd.DedispError):
         gpu_dedisperse(p, W.generate(w3, md3)[None], 8, w3.nsamps_out)
     dd.dedisp_destroy(p)
+    # more than 4096 channels would need two channel blocks: such plans have no quad rows either
+    w4 = _workload(4100, 0.0, 256, 100)
+    _, md4 = oracle.delay_table(w4.nchans, w4.dt, w4.f_top, w4.df, w4.dms())
+    p = make_plan(w4.nchans, w4.dt, w4.f_top, w4.df, w4.dms(), dd.DEDISP_KERNEL_QUADS)
+    with pytest.raises(dd.DedispError) as e:
+        gpu_dedisperse(p, W.generate(w4, md4)[None], 8, w4.nsamps_out)
+    assert e.value.status == dd.DEDISP_ERR_INVALID_ARG
+    dd.dedisp_destroy(p)
