@@ -20,13 +20,17 @@ WIDE8 = W.CONFIGS["wide8"]
 STEP8 = 2000.0 / 2047
 
 
-def _tables(nchans, dm_lo, ndm, step=STEP8):
+def _tables(nchans, dm_lo, ndm, step=STEP8, shuffle=False):
     w = WIDE8.scaled(nchans=nchans, ndm=ndm, dm_lo=dm_lo, dm_hi=dm_lo + step * (ndm - 1))
-    delay, _ = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    dms = np.asarray(w.dms())
+    if shuffle:         # the caller's list in any order: the plan sorts the trials, a lane holds the caller's index
+        dms = np.random.default_rng(5).permutation(dms)
+    delay, _ = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, dms)
     delay = np.ascontiguousarray(delay, dtype=np.int32)
     ngroups = (ndm + 31) // 32
-    lanes = np.arange(ngroups * 32, dtype=np.int32).reshape(ngroups, 32)
-    lanes[lanes >= ndm] = -1
+    lanes = np.full(ngroups * 32, -1, dtype=np.int32)
+    lanes[:ndm] = np.argsort(dms, kind="stable")
+    lanes = lanes.reshape(ngroups, 32)
     return delay, lanes, dd.dedisp_debug_quad_tables(delay, lanes)
 
 
@@ -44,14 +48,15 @@ def _diffs(delay, nchans, q):
     return np.stack([delay[4 * q + k] - d0 if 4 * q + k < nchans else np.zeros_like(d0) for k in (1, 2, 3)], axis=1)
 
 
-@pytest.mark.parametrize("nchans,dm_lo,ndm", [
-    (4096, 0.0, 256),        # bottom of the DM range: few triples
-    (4096, 1744.0, 262),     # top of the range: up to 7 variants per (group, quad); ragged last group
-    (1001, 900.0, 288),      # last quad has one channel
-    (514, 1200.0, 257),      # last quad has two channels; one trial in the last group
+@pytest.mark.parametrize("nchans,dm_lo,ndm,shuffle", [
+    (4096, 0.0, 256, False),        # bottom of the DM range: few triples
+    (4096, 1744.0, 262, False),     # top of the range: up to 7 variants per (group, quad); ragged last group
+    (1001, 900.0, 288, False),      # last quad has one channel
+    (514, 1200.0, 257, False),      # last quad has two channels; one trial in the last group
+    (2048, 1500.0, 300, True),      # the caller's DM list in random order
 ])
-def test_addressing_contract(nchans, dm_lo, ndm):
-    delay, lanes, (info, row0, trip, vlist, rel) = _tables(nchans, dm_lo, ndm)
+def test_addressing_contract(nchans, dm_lo, ndm, shuffle):
+    delay, lanes, (info, row0, trip, vlist, rel) = _tables(nchans, dm_lo, ndm, shuffle=shuffle)
     assert info["usable"] == 1
     nv, vslot, plw, tw, nq = (info[k] for k in ("nv", "vslot_bytes", "plane_words", "tile_words", "nquads_pad"))
     assert nv == 7 and vslot % 128 == 0 and plw * 10 * 4 <= vslot and tw % 4 == 0
