@@ -173,3 +173,20 @@ def test_walking_the_tables_on_the_cpu_reproduces_the_oracle_sums():
                     got[d] += xs8[4 * q + k, first + dk + t]
     want = oracle.dedisperse(delay, x, 8, nso)
     assert np.array_equal(got, want.astype(np.int64))
+
+
+def test_the_wideband_config_takes_quad_rows_with_the_documented_table_sizes():
+    # BASELINE.json:configs[3] in full (4096 channels x 2048 trials): the numbers DESIGN.md Sec. 6 C and
+    # profiles/r2_wide8.md quote for the quad path come from these tables
+    w = WIDE8
+    delay, md = oracle.delay_table(w.nchans, w.dt, w.f_top, w.df, w.dms())
+    lanes = np.arange(w.ndm, dtype=np.int32).reshape(w.ndm // 32, 32)
+    info, row0, trip, vlist, rel = dd.dedisp_debug_quad_tables(np.ascontiguousarray(delay, dtype=np.int32), lanes)
+    assert info["usable"] == 1 and info["nquads_pad"] == 1024 and info["nrows"] == 88042
+    nvar = (vlist[:, :, :, 0] >= 0).sum(axis=2)              # variants per (DM group, quad)
+    assert nvar.min() >= 1 and nvar.max() == 7 and abs(nvar.mean() - 4.256) < 0.001
+    # AUTO's rule (bitslice_kernel.cu): at most 3 rows to build per (group, quad) slot served, rows within 24 GB
+    assert info["nrows"] <= 3 * lanes.shape[0] * info["nquads_pad"]
+    ntiles = -(-w.nsamps_out // (32 * info["tile_words"]))
+    pitch = ((md >> 5) + ntiles * info["tile_words"] + 72 + 4 + 3) & ~3
+    assert abs(info["nrows"] * 10 * pitch * 4 / 1e9 - 20.13) < 0.01 and info["nrows"] * 10 * pitch * 4 < 24 << 30
