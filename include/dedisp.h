@@ -102,7 +102,7 @@ typedef enum {
     DEDISP_KERNEL_QUADS = 4     /* ... and on quad rows: the sum of FOUR adjacent channels formed once per triple of delay
                                    differences of the DM list (nbits + 2 planes), nchans/4 rows per output.  8-bit samples
                                    only; needs up to tens of GB of scratch for long DM lists (8-bit wideband config:
-                                   20.1 GB); up to 4096 channels, >= 8 DM groups, <= 7 distinct triples per group and
+                                   20.3 GB); up to 4096 channels, >= 8 DM groups, <= 7 distinct triples per group and
                                    quad, else forced QUADS returns INVALID_ARG; AUTO takes it when it pays and fits,
                                    else pair rows, else planes */
 } dedisp_kernel;

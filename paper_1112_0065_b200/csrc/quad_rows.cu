@@ -9,7 +9,7 @@
 // differences that occurs in the DM list (a "quad row" of nbits + 2 bit planes) and the tiled kernel adds nchans/4
 // ten-plane rows per output sample instead of nchans/2 nine-plane rows: 0.59 x the adder and shift instructions of the
 // pair-row kernel.  The price is memory and pre-pass traffic -- the 8-bit wideband config (4096 channels x 2048 trials)
-// has 88 042 distinct (quad, triple) rows of 229 KB, 20.1 GB -- which is why only 8-bit data, where the gather-sum is
+// has 88 042 distinct (quad, triple) rows of 230 KB, 20.3 GB -- which is why only 8-bit data, where the gather-sum is
 // slowest, takes this path (profiles/r2_wide8.md).
 //   * quad_prepare      : (host bookkeeping on the DEVICE-built delay table) the distinct triples of every quad ->
 //     the list of rows; per (DM group, quad) the <= NV rows the group's trials use, window start and per-lane
@@ -145,7 +145,7 @@ quad_rows_kernel(const uint32_t *__restrict__ raw, size_t raw_beam_pitch, int nc
 #pragma unroll
         for (int k = 0; k < NR; ++k) {
             const uint4 o = make_uint4(acc[k][0], acc[k][1], acc[k][2], acc[k][3]);
-            // streaming store: 20.1 GB of rows pass through L2 once; evict-first keeps the channel planes, which every
+            // streaming store: 20.3 GB of rows pass through L2 once; evict-first keeps the channel planes, which every
             // row of the quad re-reads, resident (pre-pass 5.57 -> 4.75 ms on the 8-bit wideband config)
             __stcs(reinterpret_cast<uint4 *>(dst + (size_t)k * row_pitch), o);
         }

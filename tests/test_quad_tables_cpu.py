@@ -189,4 +189,4 @@ def test_the_wideband_config_takes_quad_rows_with_the_documented_table_sizes():
     assert info["nrows"] <= 3 * lanes.shape[0] * info["nquads_pad"]
     ntiles = -(-w.nsamps_out // (32 * info["tile_words"]))
     pitch = ((md >> 5) + ntiles * info["tile_words"] + 72 + 4 + 3) & ~3
-    assert abs(info["nrows"] * 10 * pitch * 4 / 1e9 - 20.13) < 0.01 and info["nrows"] * 10 * pitch * 4 < 24 << 30
+    assert pitch == 5760 and abs(info["nrows"] * 10 * pitch * 4 / 1e9 - 20.28) < 0.01 and info["nrows"] * 10 * pitch * 4 < 24 << 30
