@@ -190,3 +190,8 @@ def test_the_wideband_config_takes_quad_rows_with_the_documented_table_sizes():
     ntiles = -(-w.nsamps_out // (32 * info["tile_words"]))
     pitch = ((md >> 5) + ntiles * info["tile_words"] + 72 + 4 + 3) & ~3
     assert pitch == 5760 and abs(info["nrows"] * 10 * pitch * 4 / 1e9 - 20.28) < 0.01 and info["nrows"] * 10 * pitch * 4 < 24 << 30
+    # shared-memory wavefronts per window load with the placement of the tables: 1.313 (with the one conflict-free rel
+    # load per 50 window loads: 1.307; ncu measured 4.520 G wavefronts for 3.456 G loads = 1.308, profiles/r2_wide8.md)
+    words = (rel >> 16).astype(np.int64) // 4
+    wf = np.mean([_wavefronts(words[g, q]) for g in range(0, lanes.shape[0], 2) for q in range(0, 1024, 2)])
+    assert abs(wf - 1.313) < 0.01
