@@ -71,3 +71,32 @@ def test_no_cpu_fallback_in_product():
             s = f.read_text()
             assert "import paper_1112_0065_b200" not in s and "from paper_1112_0065_b200" not in s \
                 and "dedisp.h" not in s and "libdedisp_b200" not in s, f
+
+
+def test_host_only_size_functions(dd):
+    """The workspace / stride / block-count queries are host arithmetic (no device): documented values for the HTRU
+    gulp, 0 on bad arguments, never shrinking with the problem."""
+    w7 = [1, 2, 4, 8, 16, 32, 64]
+    assert dd.dedisp_static_scratch_bytes() == 32 << 20
+    fe = dd.dedisp_find_events_workspace_bytes(8400, 65536)
+    assert 70e6 < fe < 80e6                                              # "73 MB" for 7 widths x 1200 rows
+    assert dd.dedisp_find_events_workspace_bytes(0, 65536) == 0 and dd.dedisp_find_events_workspace_bytes(8400, 0) == 0
+    assert dd.dedisp_find_events_workspace_bytes(8400, 131072) >= fe <= dd.dedisp_find_events_workspace_bytes(16800, 65536)
+    mf = dd.dedisp_matched_filter_rms_workspace_bytes(1200, 65536, 7)
+    assert mf > 0 and mf % 8 == 0
+    assert dd.dedisp_matched_filter_rms_workspace_bytes(0, 65536, 7) == 0
+    assert dd.dedisp_matched_filter_rms_workspace_bytes(1200, 65536, 0) == 0
+    assert dd.dedisp_matched_filter_rms_workspace_bytes(2400, 65536, 7) >= mf
+    # block maxima: blocks of 2048 outputs, offset by the largest width, enough blocks to cover nsamps + offset
+    assert dd.dedisp_matched_filter_hint_blocks(65536, w7) == (33, 2048, 64)
+    assert dd.dedisp_matched_filter_hint_blocks(100, [1]) == (1, 2048, 1)
+    assert dd.dedisp_matched_filter_hint_blocks(2048, [1, 64])[0] == 2
+    se = dd.dedisp_search_events_workspace_bytes(1200, 65536, w7, 16384)
+    assert se >= 16384 * 2048 * 4 + fe and se % 256 == 0                 # the compact z + the f2 workspace inside it
+    assert dd.dedisp_search_events_workspace_bytes(1200, 65536, w7, 0) == 0
+    assert dd.dedisp_search_events_workspace_bytes(0, 65536, w7, 16) == 0
+    assert dd.dedisp_search_events_workspace_bytes(1200, 65536, w7, 32768) > se
+    # strides need the delay table (max_delay): 0 before set_dm_list, which needs a device
+    p = dd.dedisp_plan_create(1024, 64e-6, 1581.8046875, -0.390625)
+    assert dd.dedisp_get_in_row_stride_bytes(p, 100, 2) == 0
+    dd.dedisp_destroy(p)
