@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(C::NTHREADS, 1) bitslice_dedisperse(const Bits
                             // never read -- the lanes' own words lie inside, quad_rows.cu::prepare_tables)
                             const int x = vr.y + tile * C::TILE_WORDS;
                             const int y = (beam * P.vrows + row) * NB;
-                            BS_CHECK(x > -S::PLW && x < P.row_pitch && y >= 0 &&
+                            BS_CHECK(x > -S::PLW && x < P.row_pitch && y >= 0 && (x & 3) == 0 &&
                                          (unsigned long long)(y + NB) * P.row_pitch <= P.scratch_words, CHK_TMA_SRC);
                             tma_box_g2s(sb + cl * S::CPITCH + v * S::VSLOT, &tmap, x, y, fb);
                         }
